@@ -1,0 +1,157 @@
+/* bta.h -- C-ABI boundary of the B200-native BTA / INLA library (libbta_b200.so).
+ *
+ * One thing is built behind this boundary: the exact value f(theta) and exact reverse-mode gradient of
+ * the INLA objective over a block-tridiagonal-arrowhead (BTA) precision matrix -- the data-parallel hot
+ * path of ADELIA (arxiv/paper_2605_06392).  Citations are PAPER.md:<line> (+ equation / algorithm) and
+ * DESIGN.md readings R<n>.  Every call runs hand-written sm_100a kernels; there is no CPU fallback:
+ * bta_create fails with BTA_ERR_NODEVICE when no compute-capability-10.x device is present.
+ *
+ * Conventions
+ *   - All matrices are FP64, row-major.  "host" / "device" is stated per pointer.
+ *   - Notation: nt diagonal blocks D_i (b x b), sub-diagonal blocks B_i = Q[i+1, i]
+ *     (b x b, i < nt-1), arrow blocks C_i = Q[T, i] (a x b), tip T (a x a); N = nt*b + a.  b = k*ns,
+ *     ns = g*g grid nodes, k response variables.  Latent ordering (R6): index = t*b + v*ns + s, the a
+ *     fixed effects last.
+ *   - Device block arrays:  D[t][i][j] = Q[t*b+i, t*b+j];  B[t][i][j] = Q[(t+1)*b+i, t*b+j];
+ *     C[t][p][j] = Q[nt*b+p, t*b+j];  T[p][q];  rhs[t*b+i], tip entries last (N doubles).
+ *   - Ownership: the caller owns every large device buffer (blocks, workspace, rhs) -- typically
+ *     torch tensors' data_ptr(); the library allocates only the theta-independent model data
+ *     (bta_create) and small scratch.  `stream` is a cudaStream_t passed as void*.
+ *   - Return value: 0 on success; BTA_ERR_* (> 0) otherwise; BTA_ERR_NOTSPD means a non-positive pivot
+ *     was met on the device (the 1-based global row is reported by bta_last_error / bta_last_pivot).
+ *     Calls that return scalars to host memory synchronise `stream` before returning.
+ */
+#ifndef BTA_H_
+#define BTA_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+enum {
+  BTA_OK = 0,
+  BTA_ERR_ARG = 1,           /* invalid argument (text in bta_last_error) */
+  BTA_ERR_CUDA = 2,          /* a CUDA runtime call or kernel failed */
+  BTA_ERR_NODEVICE = 3,      /* no sm_100-class device: the library has no fallback */
+  BTA_ERR_NOTSPD = 4,        /* non-positive pivot in a Cholesky step */
+  BTA_ERR_UNIMPLEMENTED = 5
+};
+
+enum { BTA_PRIOR = 0, BTA_COND = 1 }; /* which matrix: Q_p (BT, no arrow coupling) or Q_c (full BTA) */
+
+typedef struct bta_ctx bta_ctx; /* opaque: model shape, theta-independent observation aggregates, scratch */
+
+/* Model shape (BASELINE.json configs).  d = 3k + k(k-1)/2 + k hyperparameters,
+ * ordered (R13): theta_{1,1..3}, ..., theta_{k,1..3}, lambda_21, lambda_31, lambda_32, ..., log tau_1..k. */
+typedef struct {
+  int32_t nt;        /* time blocks (paper's n) */
+  int32_t g;         /* grid side, ns = g*g */
+  int32_t k;         /* response variables */
+  int32_t a;         /* arrow width = fixed effects (multiple of k; a/k covariates per observation row, R14) */
+  double h;          /* grid spacing: C = h^2 I (R3) */
+  double fixed_prec; /* prior precision of the fixed effects (R5) */
+} bta_model_desc;
+
+/* Gaussian observations y = A x + eps.  HOST pointers, read during bta_create only.
+ * Row i of A has a 1 at latent (time[i], var[i], node[i]) and cov[i][0..a/k) in fixed-effect columns
+ * var[i]*(a/k) ...  (R11, R14). */
+typedef struct {
+  int64_t m;
+  const int32_t* var;  /* [m] in [0,k) */
+  const int32_t* node; /* [m] in [0,ns) */
+  const int32_t* time; /* [m] in [0,nt) */
+  const double* cov;   /* [m][a/k] */
+  const double* y;     /* [m] */
+} bta_obs;
+
+/* DEVICE pointers to one BTA matrix (layouts above).  C may be NULL for BTA_PRIOR (C_i = 0). */
+typedef struct {
+  double* D;   /* [nt][b][b] */
+  double* B;   /* [nt-1][b][b] */
+  double* C;   /* [nt][a][b] */
+  double* T;   /* [a][a] */
+  double* rhs; /* [N] or NULL */
+} bta_blocks;
+
+/* Model setup: copies the observations to the device and reduces
+ * them to theta-independent aggregates (counts, covariate sums, Z^T Z, A^T y) with device kernels in a
+ * deterministic order.  `device` is the CUDA ordinal.  *out is NULL on failure. */
+int bta_create(bta_ctx** out, const bta_model_desc* desc, const bta_obs* obs, int device);
+int bta_destroy(bta_ctx* ctx);
+
+/* Bytes of caller-provided device workspace needed by inla_value_and_grad (the largest user: both matrices'
+ * blocks, per-chain temporaries).  bta_factor_logdet / bta_solve / bta_selinv need at most
+ * bta_workspace_bytes_op(ctx) (three b x b temporaries + small vectors). */
+size_t bta_workspace_bytes(const bta_ctx* ctx);
+size_t bta_workspace_bytes_op(const bta_ctx* ctx);
+
+/* Q_p(theta) or Q_c(theta) = Q_p + sum_v tau_v A_v^T A_v and r = sum_v tau_v A_v^T y_v as dense blocks
+ * (Eq. 10 for k > 1 with the weights of R12).  theta: HOST, d doubles.  D is written
+ * with its strict upper triangle ZERO (the lower triangle is authoritative everywhere in this library);
+ * B, C, T in full.  out.rhs (if not NULL) receives r for BTA_COND, zeros for BTA_PRIOR. */
+int bta_assemble(bta_ctx* ctx, const double* theta, int which, bta_blocks out, void* stream);
+
+/* Algorithm 1 (R8): block Cholesky Q = L L^T in place, and log det Q (HOST scalar).
+ * The factor is kept in INVERSE-DIAGONAL FORM: on return
+ *   D[t] = X_t = L_Dt^-1 (lower triangular, strict upper triangle zero),
+ *   B[t] = L_Bt = B_t L_Dt^-T,   C[t] = L_Ct,   T = L_T (lower, strict upper zero),
+ * and diagL (device, N doubles, may be NULL) receives diag(L_D1), ..., diag(L_Dnt), diag(L_T).
+ * `which` = BTA_PRIOR skips the arrow (C ignored, T factored on its own).  Only the lower triangles of the
+ * D[t] and T are read.  ws: device workspace (bta_workspace_bytes_op). */
+int bta_factor_logdet(bta_ctx* ctx, bta_blocks inout, int which, double* logdet, double* diagL, void* ws,
+                      void* stream);
+
+/* Both triangular sweeps L z = rhs, L^T x = z (Algorithm 1 line 5/11 and Eqs. 3-5) for
+ * nrhs right-hand sides, in place: rhs_inout is DEVICE [nrhs][N].  L as left by bta_factor_logdet. */
+int bta_solve(bta_ctx* ctx, bta_blocks L, int which, double* rhs_inout, int nrhs, void* ws, void* stream);
+
+/* BTA selected inversion (recurrences R10), in place over the factor left by
+ * bta_factor_logdet: on return D[t] = Z_Dt = [Q^-1]_{tt} (both triangles), B[t] = Z_Bt = [Q^-1]_{t+1,t},
+ * C[t] = Z_Ct = [Q^-1]_{T,t}, T = Z_T. */
+int bta_selinv(bta_ctx* ctx, bta_blocks inout, int which, void* ws, void* stream);
+
+/* The hot path (PAPER.md:44 Eq. 1, :121 Eq. 6): f(theta) and grad f(theta).  theta HOST [d]; f HOST scalar;
+ * grad HOST [d]; stage_ms HOST [BTA_NSTAGES] or NULL (CUDA-event times of the stages, see BTA_STAGE_*);
+ * ws DEVICE, bta_workspace_bytes(ctx) bytes.  Runs assemble -> fused forward sweep -> fused backward sweep
+ * (upper solve + selected inversion + trace contractions) on Q_c and on Q_p, then the scalar assembly. */
+int inla_value_and_grad(bta_ctx* ctx, const double* theta, double* f, double* grad, double* stage_ms, void* ws,
+                        void* stream);
+
+enum {
+  BTA_STAGE_ASSEMBLE = 0,
+  BTA_STAGE_FWD_QC = 1,
+  BTA_STAGE_BWD_QC = 2,
+  BTA_STAGE_FWD_QP = 3,
+  BTA_STAGE_BWD_QP = 4,
+  BTA_STAGE_SCALARS = 5,
+  BTA_STAGE_TOTAL = 6,
+  BTA_NSTAGES = 7
+};
+
+/* Intermediates of the last inla_value_and_grad (HOST outputs; any pointer may be NULL):
+ * ld[2] = {log det Q_p, log det Q_c}; x DEVICE->HOST copy of x* [N]; parts[3*d] = Phase A, B, C per
+ * hyperparameter (Eq. 6 terms before the -1/2, -1/2, +1/2 factors); rss[k] = ||y_v - A_v x*||^2;
+ * quad = x*^T Q_p x*. */
+int bta_last_intermediates(bta_ctx* ctx, double* ld, double* x, double* parts, double* rss, double* quad);
+
+int32_t bta_num_hyper(const bta_ctx* ctx);  /* d */
+int64_t bta_latent_size(const bta_ctx* ctx); /* N */
+int64_t bta_last_pivot(const bta_ctx* ctx);  /* 1-based global row of the first non-positive pivot, 0 if none */
+int64_t bta_kernel_launches(const bta_ctx* ctx); /* kernels launched by this ctx so far */
+const char* bta_last_error(void);
+
+/* Measurement helpers (bench.py): register-resident issue loops on all SMs, returning achieved FP64
+ * TFLOP/s of `mma.sync.m8n8k4.f64` (kind 0) or DFMA (kind 1) -- the FP64 roofline denominators. */
+int bta_fp64_peak(int kind, int iters, double* tflops, double* ms, void* stream);
+/* Plain C = alpha op(A) op(B) + beta C through the library's DMMA GEMM (DEVICE pointers, row-major);
+ * mode: 0 NN, 1 NT, 2 TN; klo/khi/out as in csrc/common.cuh (0 = full). */
+int bta_gemm(int mode, int M, int N, int K, double alpha, const double* A, int lda, const double* B, int ldb,
+             double beta, double* C, int ldc, int klo, int khi, int out, void* stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* BTA_H_ */

@@ -1,0 +1,254 @@
+"""ctypes binding with the same names as include/bta.h.  Marshalling only."""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from dataclasses import dataclass
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+
+
+def lib_path() -> str:
+    return os.path.join(_HERE, "libbta_b200.so")
+
+
+class BtaError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__(f"bta error {code}: {msg}")
+        self.code = code
+
+
+class _Desc(C.Structure):
+    _fields_ = [("nt", C.c_int32), ("g", C.c_int32), ("k", C.c_int32), ("a", C.c_int32),
+                ("h", C.c_double), ("fixed_prec", C.c_double)]
+
+
+class _Obs(C.Structure):
+    _fields_ = [("m", C.c_int64), ("var", C.c_void_p), ("node", C.c_void_p), ("time", C.c_void_p),
+                ("cov", C.c_void_p), ("y", C.c_void_p)]
+
+
+class _Blocks(C.Structure):
+    _fields_ = [("D", C.c_void_p), ("B", C.c_void_p), ("C", C.c_void_p), ("T", C.c_void_p), ("rhs", C.c_void_p)]
+
+
+_lib = None
+
+
+def lib():
+    """Load libbta_b200.so (built in-tree by build.py); fails loudly if it is missing."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    path = lib_path()
+    if not os.path.exists(path):
+        raise ImportError(f"{path} is missing: run `python -m paper_2605_06392_b200.build` "
+                          "(or __graft_entry__.build()); there is no fallback path")
+    L = C.CDLL(path)
+    vp, dp, i32, i64 = C.c_void_p, C.POINTER(C.c_double), C.c_int, C.c_int64
+    L.bta_create.argtypes = [C.POINTER(vp), C.POINTER(_Desc), C.POINTER(_Obs), i32]
+    L.bta_destroy.argtypes = [vp]
+    L.bta_workspace_bytes.argtypes = [vp]
+    L.bta_workspace_bytes.restype = C.c_size_t
+    L.bta_workspace_bytes_op.argtypes = [vp]
+    L.bta_workspace_bytes_op.restype = C.c_size_t
+    L.bta_assemble.argtypes = [vp, dp, i32, _Blocks, vp]
+    L.bta_factor_logdet.argtypes = [vp, _Blocks, i32, dp, vp, vp, vp]
+    L.bta_solve.argtypes = [vp, _Blocks, i32, vp, i32, vp, vp]
+    L.bta_selinv.argtypes = [vp, _Blocks, i32, vp, vp]
+    L.inla_value_and_grad.argtypes = [vp, dp, dp, dp, dp, vp, vp]
+    L.bta_last_intermediates.argtypes = [vp, dp, dp, dp, dp, dp]
+    L.bta_num_hyper.argtypes = [vp]
+    L.bta_num_hyper.restype = C.c_int32
+    L.bta_latent_size.argtypes = [vp]
+    L.bta_latent_size.restype = i64
+    L.bta_last_pivot.argtypes = [vp]
+    L.bta_last_pivot.restype = i64
+    L.bta_kernel_launches.argtypes = [vp]
+    L.bta_kernel_launches.restype = i64
+    L.bta_last_error.restype = C.c_char_p
+    L.bta_fp64_peak.argtypes = [i32, i32, dp, dp, vp]
+    L.bta_gemm.argtypes = [i32, i32, i32, i32, C.c_double, vp, i32, vp, i32, C.c_double, vp, i32, i32, i32, i32, vp]
+    _lib = L
+    return L
+
+
+def _check(rc):
+    if rc != 0:
+        raise BtaError(rc, lib().bta_last_error().decode())
+
+
+def _dptr(arr):
+    return arr.ctypes.data_as(C.POINTER(C.c_double))
+
+
+def _stream():
+    import torch
+    return torch.cuda.current_stream().cuda_stream
+
+
+@dataclass
+class Blocks:
+    """Device tensors of one BTA matrix (layouts of include/bta.h)."""
+    D: object
+    B: object
+    C: object
+    T: object
+    rhs: object = None
+
+    def c(self):
+        p = lambda t: t.data_ptr() if t is not None and t.numel() > 0 else None
+        return _Blocks(p(self.D), p(self.B), p(self.C), p(self.T), p(self.rhs))
+
+    def clone(self):
+        cl = lambda t: t.clone() if t is not None else None
+        return Blocks(cl(self.D), cl(self.B), cl(self.C), cl(self.T), cl(self.rhs))
+
+
+BTA_PRIOR, BTA_COND = 0, 1
+STAGES = ("assemble", "fwd_Qc", "bwd_Qc", "fwd_Qp", "bwd_Qp", "scalars", "total")
+
+
+class BtaModel:
+    """bta_create / bta_destroy plus the calls of include/bta.h on torch-owned device memory."""
+
+    def __init__(self, nt, g, k, a, h, fixed_prec, var, node, time, cov, y, device=0):
+        import torch
+        self._h = C.c_void_p()
+        self.nt, self.g, self.k, self.a = int(nt), int(g), int(k), int(a)
+        self.ns = self.g * self.g
+        self.b = self.k * self.ns
+        self.device = torch.device("cuda", device)
+        var = np.ascontiguousarray(var, dtype=np.int32)
+        node = np.ascontiguousarray(node, dtype=np.int32)
+        time = np.ascontiguousarray(time, dtype=np.int32)
+        cov = np.ascontiguousarray(cov, dtype=np.float64)
+        y = np.ascontiguousarray(y, dtype=np.float64)
+        desc = _Desc(self.nt, self.g, self.k, self.a, float(h), float(fixed_prec))
+        obs = _Obs(int(y.shape[0]), var.ctypes.data, node.ctypes.data, time.ctypes.data, cov.ctypes.data, y.ctypes.data)
+        _check(lib().bta_create(C.byref(self._h), C.byref(desc), C.byref(obs), device))
+        self.d = lib().bta_num_hyper(self._h)
+        self.N = lib().bta_latent_size(self._h)
+        self._ws = None
+        self._ws_op = None
+
+    @classmethod
+    def from_workload(cls, model, obs, device=0):
+        return cls(model.nt, model.g, model.k, model.a, model.h, model.fixed_prec, obs.var, obs.node, obs.time,
+                   obs.cov, obs.y, device=device)
+
+    def close(self):
+        if self._h:
+            lib().bta_destroy(self._h)
+            self._h = C.c_void_p()
+            self._ws = self._ws_op = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # ---- memory (torch owns it) ----
+    def workspace_bytes(self):
+        return lib().bta_workspace_bytes(self._h)
+
+    def workspace_bytes_op(self):
+        return lib().bta_workspace_bytes_op(self._h)
+
+    def _workspace(self, op=False):
+        import torch
+        if op:
+            if self._ws_op is None:
+                self._ws_op = torch.empty(self.workspace_bytes_op(), dtype=torch.uint8, device=self.device)
+            return self._ws_op
+        if self._ws is None:
+            self._ws = torch.empty(self.workspace_bytes(), dtype=torch.uint8, device=self.device)
+        return self._ws
+
+    def alloc_blocks(self, rhs=True):
+        import torch
+        kw = dict(dtype=torch.float64, device=self.device)
+        return Blocks(torch.empty(self.nt, self.b, self.b, **kw), torch.empty(max(self.nt - 1, 0), self.b, self.b, **kw),
+                      torch.empty(self.nt, self.a, self.b, **kw), torch.empty(self.a, self.a, **kw),
+                      torch.empty(self.N, **kw) if rhs else None)
+
+    # ---- the calls of include/bta.h ----
+    def bta_assemble(self, theta, which, out: Blocks):
+        th = np.ascontiguousarray(theta, dtype=np.float64)
+        assert th.shape == (self.d,)
+        _check(lib().bta_assemble(self._h, _dptr(th), which, out.c(), _stream()))
+        return out
+
+    def bta_factor_logdet(self, blocks: Blocks, which, diagL=None):
+        ld = C.c_double()
+        _check(lib().bta_factor_logdet(self._h, blocks.c(), which, C.byref(ld),
+                                       diagL.data_ptr() if diagL is not None else None,
+                                       self._workspace(op=True).data_ptr(), _stream()))
+        return ld.value
+
+    def bta_solve(self, factor: Blocks, which, rhs):
+        """rhs: device tensor [nrhs, N], solved in place."""
+        assert rhs.is_contiguous() and rhs.shape[-1] == self.N
+        nrhs = 1 if rhs.dim() == 1 else rhs.shape[0]
+        _check(lib().bta_solve(self._h, factor.c(), which, rhs.data_ptr(), nrhs, self._workspace(op=True).data_ptr(),
+                               _stream()))
+        return rhs
+
+    def bta_selinv(self, factor: Blocks, which):
+        _check(lib().bta_selinv(self._h, factor.c(), which, self._workspace(op=True).data_ptr(), _stream()))
+        return factor
+
+    def inla_value_and_grad(self, theta, stages=False):
+        th = np.ascontiguousarray(theta, dtype=np.float64)
+        assert th.shape == (self.d,)
+        f = C.c_double()
+        grad = np.zeros(self.d)
+        st = np.zeros(len(STAGES))
+        _check(lib().inla_value_and_grad(self._h, _dptr(th), C.byref(f), _dptr(grad), _dptr(st) if stages else None,
+                                         self._workspace().data_ptr(), _stream()))
+        if stages:
+            return f.value, grad, dict(zip(STAGES, st.tolist()))
+        return f.value, grad
+
+    def last_intermediates(self, want_x=True):
+        ld = np.zeros(2)
+        x = np.zeros(self.N) if want_x else None
+        parts = np.zeros(3 * self.d)
+        rss = np.zeros(self.k)
+        quad = C.c_double()
+        _check(lib().bta_last_intermediates(self._h, _dptr(ld), _dptr(x) if want_x else None, _dptr(parts), _dptr(rss),
+                                            C.byref(quad)))
+        return dict(ld_p=ld[0], ld_c=ld[1], x=x, phaseA=parts[: self.d], phaseB=parts[self.d: 2 * self.d],
+                    phaseC=parts[2 * self.d:], rss=rss, quad_p=quad.value)
+
+    def kernel_launches(self):
+        return lib().bta_kernel_launches(self._h)
+
+    def last_pivot(self):
+        return lib().bta_last_pivot(self._h)
+
+
+def fp64_peak(kind=0, iters=100000):
+    """(TFLOP/s, ms) of the register-resident DMMA (kind 0) or DFMA (kind 1) issue loop."""
+    tf, ms = C.c_double(), C.c_double()
+    _check(lib().bta_fp64_peak(kind, iters, C.byref(tf), C.byref(ms), _stream()))
+    return tf.value, ms.value
+
+
+def gemm(mode, A, B, Cm, alpha=1.0, beta=0.0, klo=0, khi=0, out=0):
+    """C = alpha op(A) op(B) + beta C through the library's DMMA GEMM (device tensors, row-major)."""
+    if mode == 0:
+        M, K = A.shape
+        N = B.shape[1]
+    elif mode == 1:
+        M, K = A.shape
+        N = B.shape[0]
+    else:
+        K, M = A.shape
+        N = B.shape[1]
+    _check(lib().bta_gemm(mode, M, N, K, alpha, A.data_ptr(), A.stride(0), B.data_ptr(), B.stride(0), beta,
+                          Cm.data_ptr(), Cm.stride(0), klo, khi, out, _stream()))
+    return Cm

@@ -1,0 +1,455 @@
+// The C-ABI entry points of include/bta.h: argument checks, workspace carving, stream/event plumbing.
+#include <algorithm>
+#include <cstdlib>
+#include <cstring>
+
+#include "sweep.h"
+
+namespace {
+
+struct Bump {
+  char* base;
+  size_t off = 0;
+  explicit Bump(void* p) : base((char*)p) {}
+  double* take(size_t doubles) {
+    double* r = (double*)(base + off);
+    off += (doubles * sizeof(double) + 255) / 256 * 256;
+    return r;
+  }
+};
+
+struct ChainWs {
+  double *D, *B, *W1, *W2, *W3, *Rin, *Rout, *ubuf, *Ebuf, *Ybuf, *ZC0, *ZC1, *part, *x, *dvec, *T, *rtip;
+};
+
+// Workspace of one chain of the fused gradient.  Q_c: nt D slots, nt B slots (L_Bt is written one slot below
+// B_t, so no copy), 3 scratch blocks, the arrow/rhs stacks; Q_p: the same without the stacks.
+ChainWs carve_chain(Bump& bp, const ModelDims& md, bool cond) {
+  ChainWs w{};
+  const size_t bb = (size_t)md.b * md.b;
+  const int P = md.a + 1;
+  w.D = bp.take(bb * md.nt);
+  w.B = bp.take(bb * md.nt);
+  w.W1 = bp.take(bb);
+  w.W2 = bp.take(bb);
+  w.W3 = bp.take(bb);
+  w.dvec = bp.take(md.N);
+  w.T = bp.take(md.a * md.a);
+  if (cond) {
+    w.Rin = bp.take((size_t)md.nt * P * md.b);
+    w.Rout = bp.take((size_t)md.nt * P * md.b);
+    w.ubuf = bp.take(md.b);
+    w.Ebuf = bp.take((size_t)md.a * md.b);
+    w.Ybuf = bp.take((size_t)md.a * md.b);
+    w.ZC0 = bp.take((size_t)md.a * md.b);
+    w.ZC1 = bp.take((size_t)md.a * md.b);
+    w.part = bp.take(skinny_nn_part_doubles(P, md.b, md.b));
+    w.x = bp.take(md.N);
+    w.rtip = bp.take(md.a);
+  }
+  return w;
+}
+
+size_t grad_ws_bytes(const ModelDims& md) {
+  Bump bp(nullptr);
+  carve_chain(bp, md, true);
+  carve_chain(bp, md, false);
+  return bp.off + 256;
+}
+
+struct OpWs {
+  double *W1, *W2, *W3, *Rtmp, *zbuf, *ubuf, *Ebuf, *Ybuf, *ZC0, *ZC1, *part, *dvec, *Tt, *xT, *scal;
+};
+constexpr int SOLVE_CHUNK = 8;
+
+OpWs carve_op(Bump& bp, const ModelDims& md) {
+  OpWs w{};
+  const size_t bb = (size_t)md.b * md.b;
+  w.W1 = bp.take(bb);
+  w.W2 = bp.take(bb);
+  w.W3 = bp.take(bb);
+  w.Rtmp = bp.take((size_t)(AMAX + 1) * md.b);
+  w.zbuf = bp.take((size_t)SOLVE_CHUNK * md.N);
+  w.ubuf = bp.take((size_t)SOLVE_CHUNK * md.b);
+  w.Ebuf = bp.take((size_t)md.a * md.b);
+  w.Ybuf = bp.take((size_t)md.a * md.b);
+  w.ZC0 = bp.take((size_t)md.a * md.b);
+  w.ZC1 = bp.take((size_t)md.a * md.b);
+  w.part = bp.take(skinny_nn_part_doubles(AMAX + 1, md.b, md.b));
+  w.dvec = bp.take(md.N);
+  w.Tt = bp.take((size_t)md.a * (md.a + SOLVE_CHUNK));
+  w.xT = bp.take((size_t)SOLVE_CHUNK * md.a);
+  w.scal = bp.take(8);
+  return w;
+}
+
+int check_pivot(bta_ctx* c, cudaStream_t st) {
+  unsigned long long flag = 0;
+  BTA_CUDA_OK(cudaMemcpyAsync(&flag, c->pivot_flag, sizeof flag, cudaMemcpyDeviceToHost, st));
+  BTA_CUDA_OK(cudaStreamSynchronize(st));
+  if (flag != ~0ull) {
+    c->last_pivot = (long long)flag;
+    char buf[160];
+    snprintf(buf, sizeof buf, "matrix is not positive definite: first non-positive pivot at global row %lld",
+             (long long)flag);
+    bta_set_error(buf);
+    return BTA_ERR_NOTSPD;
+  }
+  c->last_pivot = 0;
+  return BTA_OK;
+}
+
+int bad(const char* msg) {
+  bta_set_error(msg);
+  return BTA_ERR_ARG;
+}
+
+}  // namespace
+
+extern "C" size_t bta_workspace_bytes(const bta_ctx* c) { return c ? grad_ws_bytes(c->md) : 0; }
+extern "C" size_t bta_workspace_bytes_op(const bta_ctx* c) {
+  if (!c) return 0;
+  Bump bp(nullptr);
+  carve_op(bp, c->md);
+  return bp.off + 256;
+}
+
+extern "C" int bta_assemble(bta_ctx* c, const double* theta, int which, bta_blocks out, void* stream) {
+  if (!c || !theta) return bad("bta_assemble: null ctx or theta");
+  if (which != BTA_PRIOR && which != BTA_COND) return bad("bta_assemble: which must be BTA_PRIOR or BTA_COND");
+  if (!out.D || (c->md.nt > 1 && !out.B) || !out.T) return bad("bta_assemble: D, B and T are required");
+  cudaStream_t st = (cudaStream_t)stream;
+  const ModelDims& md = c->md;
+  BTA_CUDA_OK(cudaSetDevice(c->device));
+  memcpy(c->host_pinned, theta, md.d * sizeof(double));
+  BTA_CUDA_OK(cudaMemcpyAsync(c->theta_dev, c->host_pinned, md.d * sizeof(double), cudaMemcpyHostToDevice, st));
+  BTA_CUDA_OK(launch_theta_prep(c, st));
+  const long long bb = (long long)md.b * md.b;
+  BTA_CUDA_OK(launch_assemble(c, which, out.D, bb, out.B, bb, out.C, (long long)md.a * md.b, out.T, md.a, out.rhs, md.b,
+                              out.rhs ? out.rhs + (long long)md.nt * md.b : nullptr, 1, st));
+  BTA_CUDA_OK(cudaStreamSynchronize(st));  // host_pinned is reused by the next call
+  return BTA_OK;
+}
+
+extern "C" int bta_factor_logdet(bta_ctx* c, bta_blocks io, int which, double* logdet, double* diagL, void* ws,
+                                 void* stream) {
+  if (!c || !ws) return bad("bta_factor_logdet: null ctx or workspace");
+  if (which != BTA_PRIOR && which != BTA_COND) return bad("bta_factor_logdet: bad `which`");
+  if (!io.D || (c->md.nt > 1 && !io.B) || !io.T || (which == BTA_COND && !io.C))
+    return bad("bta_factor_logdet: D, B, T (and C for BTA_COND) are required");
+  cudaStream_t st = (cudaStream_t)stream;
+  const ModelDims& md = c->md;
+  BTA_CUDA_OK(cudaSetDevice(c->device));
+  Bump bp(ws);
+  OpWs w = carve_op(bp, md);
+  SmallLayout L = small_layout(md);
+  const int chs = which == BTA_COND ? CH_COND : CH_PRIOR;
+  BTA_CUDA_OK(cudaMemsetAsync(c->pivot_flag, 0xFF, sizeof(unsigned long long), st));
+  Chain ch;
+  ch.c = c;
+  ch.chain = chs;
+  ch.b = md.b;
+  ch.nt = md.nt;
+  ch.a = md.a;
+  ch.nr = 0;
+  ch.zero_upper = true;
+  ch.arrow_rows = which == BTA_COND;
+  ch.D = io.D;
+  ch.d_stride = (long long)md.b * md.b;
+  ch.Bin = ch.Bout = io.B;
+  ch.b_stride = ch.d_stride;
+  ch.Rin = ch.Rout = io.C;
+  ch.rin_stride = ch.rout_stride = (long long)md.a * md.b;
+  ch.ld_rin = ch.ld_rout = md.b;
+  ch.Rtmp = w.Rtmp;
+  ch.T = io.T;
+  ch.ldT = md.a;
+  ch.W1 = w.W1;
+  ch.W2 = w.W2;
+  ch.W3 = w.W3;
+  ch.part = w.part;
+  ch.dvec = diagL ? diagL : w.dvec;
+  ch.Tt = w.Tt;
+  ch.LT = io.T;
+  ch.ZT = c->small + L.ZT[chs];
+  BTA_CUDA_OK(chain_forward(ch, st));
+  // Rout == Rin for t = 0 would alias in the second stack product only when t > 0 uses Rtmp: fine (see sweep.cu)
+  BTA_CUDA_OK(launch_logdet_partial(c, chs, ch.dvec, st));
+  BTA_CUDA_OK(launch_logdet_final(c, chs, w.scal, st));
+  BTA_CUDA_OK(cudaMemcpyAsync(c->host_pinned, w.scal, sizeof(double), cudaMemcpyDeviceToHost, st));
+  int rc = check_pivot(c, st);
+  if (logdet) *logdet = c->host_pinned[0];
+  return rc;
+}
+
+extern "C" int bta_solve(bta_ctx* c, bta_blocks Lf, int which, double* rhs, int nrhs, void* ws, void* stream) {
+  if (!c || !ws || !rhs) return bad("bta_solve: null ctx, workspace or rhs");
+  if (which != BTA_PRIOR && which != BTA_COND) return bad("bta_solve: bad `which`");
+  if (nrhs < 0) return bad("bta_solve: nrhs < 0");
+  if (!Lf.D || (c->md.nt > 1 && !Lf.B) || !Lf.T || (which == BTA_COND && !Lf.C)) return bad("bta_solve: missing factor");
+  cudaStream_t st = (cudaStream_t)stream;
+  const ModelDims& md = c->md;
+  BTA_CUDA_OK(cudaSetDevice(c->device));
+  Bump bp(ws);
+  OpWs w = carve_op(bp, md);
+  for (int r0 = 0; r0 < nrhs; r0 += SOLVE_CHUNK) {
+    const int nr = std::min(SOLVE_CHUNK, nrhs - r0);
+    double* R = rhs + (long long)r0 * md.N;
+    Chain ch;
+    ch.c = c;
+    ch.b = md.b;
+    ch.nt = md.nt;
+    ch.a = md.a;
+    ch.nr = nr;
+    ch.factor_blocks = false;
+    ch.tip_chol = false;
+    ch.arrow_given = which == BTA_COND;
+    ch.LCgiven = Lf.C;
+    ch.lc_stride = (long long)md.a * md.b;
+    ch.D = Lf.D;
+    ch.d_stride = (long long)md.b * md.b;
+    ch.Bin = ch.Bout = Lf.B;
+    ch.b_stride = ch.d_stride;
+    ch.Rin = R;
+    ch.rin_stride = md.b;
+    ch.ld_rin = (int)md.N;
+    ch.Rout = w.zbuf;
+    ch.rout_stride = md.b;
+    ch.ld_rout = (int)md.N;
+    ch.Rtmp = w.Rtmp;
+    ch.T = Lf.T;
+    ch.ldT = md.a;
+    ch.rhs_tip = R + (long long)md.nt * md.b;
+    ch.rhs_tip_stride = (int)md.N;
+    ch.W1 = w.W1;
+    ch.W2 = w.W2;
+    ch.W3 = w.W3;
+    ch.part = w.part;
+    ch.ubuf = w.ubuf;
+    ch.Tt = w.Tt;
+    ch.LT = Lf.T;
+    ch.xT = w.xT;
+    ch.xout = R;
+    ch.ld_x = md.N;
+    BTA_CUDA_OK(chain_forward(ch, st));
+    BTA_CUDA_OK(chain_backward(ch, st));
+    BTA_CUDA_OK(cudaMemcpy2DAsync(R + (long long)md.nt * md.b, md.N * sizeof(double), w.xT, md.a * sizeof(double),
+                                  md.a * sizeof(double), nr, cudaMemcpyDeviceToDevice, st));
+  }
+  BTA_CUDA_OK(cudaStreamSynchronize(st));
+  return BTA_OK;
+}
+
+extern "C" int bta_selinv(bta_ctx* c, bta_blocks io, int which, void* ws, void* stream) {
+  if (!c || !ws) return bad("bta_selinv: null ctx or workspace");
+  if (which != BTA_PRIOR && which != BTA_COND) return bad("bta_selinv: bad `which`");
+  if (!io.D || (c->md.nt > 1 && !io.B) || !io.T || (which == BTA_COND && !io.C)) return bad("bta_selinv: missing factor");
+  cudaStream_t st = (cudaStream_t)stream;
+  const ModelDims& md = c->md;
+  BTA_CUDA_OK(cudaSetDevice(c->device));
+  Bump bp(ws);
+  OpWs w = carve_op(bp, md);
+  SmallLayout L = small_layout(md);
+  const int chs = which == BTA_COND ? CH_COND : CH_PRIOR;
+  Chain ch;
+  ch.c = c;
+  ch.chain = chs;
+  ch.b = md.b;
+  ch.nt = md.nt;
+  ch.a = md.a;
+  ch.factor_blocks = false;
+  ch.selinv = true;
+  ch.selinv_inplace = true;
+  ch.arrow_given = which == BTA_COND;
+  ch.LCgiven = io.C;
+  ch.lc_stride = (long long)md.a * md.b;
+  ch.Cout = io.C;
+  ch.cout_stride = ch.lc_stride;
+  ch.D = io.D;
+  ch.d_stride = (long long)md.b * md.b;
+  ch.Bin = ch.Bout = io.B;
+  ch.b_stride = ch.d_stride;
+  ch.W1 = w.W1;
+  ch.W2 = w.W2;
+  ch.W3 = w.W3;
+  ch.part = w.part;
+  ch.Ebuf = w.Ebuf;
+  ch.Ybuf = w.Ybuf;
+  ch.ZC[0] = w.ZC0;
+  ch.ZC[1] = w.ZC1;
+  ch.ZT = c->small + L.ZT[chs];
+  BTA_CUDA_OK(launch_tip_inverse(io.T, md.a, ch.ZT, st));
+  BTA_COUNT(c);
+  BTA_CUDA_OK(chain_backward(ch, st));
+  BTA_CUDA_OK(cudaMemcpyAsync(io.T, ch.ZT, sizeof(double) * md.a * md.a, cudaMemcpyDeviceToDevice, st));
+  BTA_CUDA_OK(cudaStreamSynchronize(st));
+  return BTA_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+// The hot path: f(theta), grad f(theta)   (PAPER.md:44 Eq. 1, :121 Eq. 6)
+// ------------------------------------------------------------------------------------------------
+extern "C" int inla_value_and_grad(bta_ctx* c, const double* theta, double* f, double* grad, double* stage_ms,
+                                   void* ws, void* stream) {
+  if (!c || !theta || !ws) return bad("inla_value_and_grad: null ctx, theta or workspace");
+  cudaStream_t s0 = (cudaStream_t)stream;
+  const ModelDims& md = c->md;
+  BTA_CUDA_OK(cudaSetDevice(c->device));
+  const char* env = getenv("BTA_SERIAL_CHAINS");
+  const bool serial = env && env[0] == '1';
+  cudaStream_t s1 = serial ? s0 : c->s_side;
+  Bump bp(ws);
+  ChainWs wc = carve_chain(bp, md, true);
+  ChainWs wp = carve_chain(bp, md, false);
+  SmallLayout L = small_layout(md);
+  const long long bb = (long long)md.b * md.b;
+  const int P = md.a + 1;
+  cudaEvent_t* ev = c->ev;
+
+  memcpy(c->host_pinned, theta, md.d * sizeof(double));
+  BTA_CUDA_OK(cudaEventRecord(ev[0], s0));
+  BTA_CUDA_OK(cudaMemcpyAsync(c->theta_dev, c->host_pinned, md.d * sizeof(double), cudaMemcpyHostToDevice, s0));
+  BTA_CUDA_OK(launch_theta_prep(c, s0));
+  BTA_CUDA_OK(cudaMemsetAsync(c->pivot_flag, 0xFF, sizeof(unsigned long long), s0));
+  BTA_CUDA_OK(cudaEventRecord(ev[9], s0));
+  if (!serial) BTA_CUDA_OK(cudaStreamWaitEvent(s1, ev[9], 0));
+
+  // ---- Q_c chain on s0 ----
+  Chain cc;
+  cc.c = c;
+  cc.chain = CH_COND;
+  cc.b = md.b;
+  cc.nt = md.nt;
+  cc.a = md.a;
+  cc.nr = 1;
+  cc.arrow_rows = true;
+  cc.selinv = cc.contract = true;
+  cc.D = wc.D;
+  cc.d_stride = bb;
+  cc.Bin = wc.B + bb;  // B_t assembled into slot t+1, L_Bt written to slot t
+  cc.Bout = wc.B;
+  cc.b_stride = bb;
+  cc.Rin = wc.Rin;
+  cc.rin_stride = (long long)P * md.b;
+  cc.ld_rin = md.b;
+  cc.Rout = wc.Rout;
+  cc.rout_stride = (long long)P * md.b;
+  cc.ld_rout = md.b;
+  cc.Rtmp = nullptr;
+  cc.T = wc.T;
+  cc.ldT = md.a;
+  cc.rhs_tip = wc.rtip;
+  cc.rhs_tip_stride = md.a;
+  cc.W1 = wc.W1;
+  cc.W2 = wc.W2;
+  cc.W3 = wc.W3;
+  cc.part = wc.part;
+  cc.ubuf = wc.ubuf;
+  cc.Ebuf = wc.Ebuf;
+  cc.Ybuf = wc.Ybuf;
+  cc.ZC[0] = wc.ZC0;
+  cc.ZC[1] = wc.ZC1;
+  cc.dvec = wc.dvec;
+  cc.Tt = c->small + L.Tt[CH_COND];
+  cc.LT = c->small + L.LT[CH_COND];
+  cc.zT = c->small + L.zT[CH_COND];
+  cc.xT = c->small + L.xT[CH_COND];
+  cc.ZT = c->small + L.ZT[CH_COND];
+  cc.xout = wc.x;
+  cc.ld_x = md.N;
+
+  BTA_CUDA_OK(launch_assemble(c, BTA_COND, cc.D, bb, cc.Bin, bb, wc.Rin, cc.rin_stride, wc.T, md.a,
+                              wc.Rin + (long long)md.a * md.b, cc.rin_stride, wc.rtip, 1, s0));
+  BTA_CUDA_OK(cudaEventRecord(ev[1], s0));
+  BTA_CUDA_OK(chain_forward(cc, s0));
+  BTA_CUDA_OK(launch_logdet_partial(c, CH_COND, wc.dvec, s0));
+  BTA_CUDA_OK(cudaEventRecord(ev[2], s0));
+  BTA_CUDA_OK(chain_backward(cc, s0));
+  BTA_CUDA_OK(cudaMemcpyAsync(wc.x + (long long)md.nt * md.b, cc.xT, md.a * sizeof(double), cudaMemcpyDeviceToDevice,
+                              s0));
+  BTA_CUDA_OK(launch_quad_stencil(c, wc.x, s0));
+  BTA_CUDA_OK(launch_residual(c, wc.x, s0));
+  BTA_CUDA_OK(cudaEventRecord(ev[3], s0));
+
+  // ---- Q_p chain (Phase C) on the side stream ----
+  Chain cp;
+  cp.c = c;
+  cp.chain = CH_PRIOR;
+  cp.b = md.b;
+  cp.nt = md.nt;
+  cp.a = md.a;
+  cp.nr = 0;
+  cp.selinv = cp.contract = true;
+  cp.D = wp.D;
+  cp.d_stride = bb;
+  cp.Bin = wp.B + bb;
+  cp.Bout = wp.B;
+  cp.b_stride = bb;
+  cp.T = wp.T;
+  cp.ldT = md.a;
+  cp.W1 = wp.W1;
+  cp.W2 = wp.W2;
+  cp.W3 = wp.W3;
+  cp.dvec = wp.dvec;
+  cp.Tt = c->small + L.Tt[CH_PRIOR];
+  cp.LT = c->small + L.LT[CH_PRIOR];
+  cp.ZT = c->small + L.ZT[CH_PRIOR];
+  BTA_CUDA_OK(cudaEventRecord(ev[4], s1));
+  BTA_CUDA_OK(launch_assemble(c, BTA_PRIOR, cp.D, bb, cp.Bin, bb, nullptr, 0, wp.T, md.a, nullptr, 0, nullptr, 0, s1));
+  BTA_CUDA_OK(cudaEventRecord(ev[5], s1));
+  BTA_CUDA_OK(chain_forward(cp, s1));
+  BTA_CUDA_OK(launch_logdet_partial(c, CH_PRIOR, wp.dvec, s1));
+  BTA_CUDA_OK(cudaEventRecord(ev[6], s1));
+  BTA_CUDA_OK(chain_backward(cp, s1));
+  BTA_CUDA_OK(cudaEventRecord(ev[7], s1));
+  if (!serial) BTA_CUDA_OK(cudaStreamWaitEvent(s0, ev[7], 0));
+
+  // ---- scalar assembly (a9) ----
+  BTA_CUDA_OK(cudaEventRecord(ev[10], s0));
+  BTA_CUDA_OK(launch_scalars(c, s0));
+  const int nout = 1 + md.d + 2 + 3 * md.d + md.k + 1;
+  BTA_CUDA_OK(cudaMemcpyAsync(c->host_pinned + 64, c->small + L.out, nout * sizeof(double), cudaMemcpyDeviceToHost,
+                              s0));
+  BTA_CUDA_OK(cudaEventRecord(ev[8], s0));
+  int rc = check_pivot(c, s0);  // synchronises s0 (and, through ev[7], the side stream)
+  const double* o = c->host_pinned + 64;
+  if (f) *f = o[0];
+  if (grad) memcpy(grad, o + 1, md.d * sizeof(double));
+  c->last_ld[0] = o[1 + md.d];
+  c->last_ld[1] = o[1 + md.d + 1];
+  c->last_parts.assign(o + 1 + md.d + 2, o + 1 + md.d + 2 + 3 * md.d);
+  c->last_rss.assign(o + 1 + md.d + 2 + 3 * md.d, o + 1 + md.d + 2 + 3 * md.d + md.k);
+  c->last_quad = o[1 + md.d + 2 + 3 * md.d + md.k];
+  c->last_x_dev = wc.x;
+  if (stage_ms) {
+    auto el = [&](int a_, int b_) {
+      float ms = 0.f;
+      cudaEventElapsedTime(&ms, ev[a_], ev[b_]);
+      return (double)ms;
+    };
+    stage_ms[BTA_STAGE_ASSEMBLE] = el(9, 1) + el(4, 5);
+    stage_ms[BTA_STAGE_FWD_QC] = el(1, 2);
+    stage_ms[BTA_STAGE_BWD_QC] = el(2, 3);
+    stage_ms[BTA_STAGE_FWD_QP] = el(5, 6);
+    stage_ms[BTA_STAGE_BWD_QP] = el(6, 7);
+    stage_ms[BTA_STAGE_SCALARS] = el(10, 8);
+    stage_ms[BTA_STAGE_TOTAL] = el(0, 8);
+  }
+  return rc;
+}
+
+extern "C" int bta_last_intermediates(bta_ctx* c, double* ld, double* x, double* parts, double* rss, double* quad) {
+  if (!c) return bad("bta_last_intermediates: null ctx");
+  if (ld) {
+    ld[0] = c->last_ld[0];
+    ld[1] = c->last_ld[1];
+  }
+  if (parts && !c->last_parts.empty()) memcpy(parts, c->last_parts.data(), c->last_parts.size() * sizeof(double));
+  if (rss && !c->last_rss.empty()) memcpy(rss, c->last_rss.data(), c->last_rss.size() * sizeof(double));
+  if (quad) *quad = c->last_quad;
+  if (x) {
+    if (!c->last_x_dev) return bad("bta_last_intermediates: no gradient has been computed yet");
+    BTA_CUDA_OK(cudaMemcpy(x, c->last_x_dev, c->md.N * sizeof(double), cudaMemcpyDeviceToHost));
+  }
+  return BTA_OK;
+}

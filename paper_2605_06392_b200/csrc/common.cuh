@@ -1,0 +1,173 @@
+// Shared declarations of the sm_100a BTA / INLA library (internal; the public boundary is include/bta.h).
+#pragma once
+#include <cuda_runtime.h>
+#include <cstdint>
+#include <cstdio>
+#include <string>
+#include <vector>
+
+#include "../../include/bta.h"
+
+#define BTA_CUDA_OK(call)                                                              \
+  do {                                                                                 \
+    cudaError_t e_ = (call);                                                           \
+    if (e_ != cudaSuccess) {                                                           \
+      bta_set_error_cuda(e_, #call, __FILE__, __LINE__);                               \
+      return BTA_ERR_CUDA;                                                             \
+    }                                                                                  \
+  } while (0)
+
+void bta_set_error_cuda(cudaError_t e, const char* what, const char* file, int line);
+void bta_set_error(const char* msg);
+
+// ------------------------------------------------------------------------------------------------
+// FP64 DMMA GEMM  (gemm.cu):  C = alpha * op(A) op(B) + beta * C, row-major, optionally batched
+// ------------------------------------------------------------------------------------------------
+enum : int {
+  GEMM_NN = 0,  // A [M][K], B [K][N]
+  GEMM_NT = 1,  // A [M][K], B [N][K]
+  GEMM_TN = 2,  // A [K][M], B [K][N]
+};
+// Restriction of the contraction range per output tile (triangular operands; tile-aligned).
+enum : int {
+  KLO_ZERO = 0,  // k >= 0
+  KLO_N0 = 1,    // k >= first column of the tile   (lower-triangular B in NN: B[k][n] = 0 for k < n)
+  KLO_M0 = 2,    // k >= first row of the tile      (X^T X lower part: k >= max(m, n) = m)
+};
+enum : int {
+  KHI_K = 0,      // k < K
+  KHI_NEND = 1,   // k < last column of the tile + 1 (lower-triangular B in NT: B[n][k] = 0 for k > n)
+  KHI_MEND = 2,   // k < last row of the tile + 1    (lower-triangular A in NN: A[m][k] = 0 for k > m)
+};
+enum : int {
+  OUT_FULL = 0,
+  OUT_LOWER = 1,         // write only elements with m >= n (tiles above the diagonal are skipped)
+  OUT_LOWER_MIRROR = 2,  // compute m >= n, write C[m][n] and C[n][m]
+};
+
+struct GemmSub {  // one problem of a batched launch: element offsets from the base pointers
+  long long offA, offB, offC;
+  int M, N, K, pad;
+};
+
+struct GemmArgs {
+  const double* A;
+  const double* B;
+  double* C;
+  int M, N, K;
+  int lda, ldb, ldc;
+  double alpha, beta;
+  int mode, klo, khi, out;
+  const GemmSub* subs;  // device array (nsub problems; M,N,K above = maxima for the grid) or nullptr
+  int nsub;
+};
+
+cudaError_t launch_gemm(const GemmArgs& g, cudaStream_t st);
+
+// ------------------------------------------------------------------------------------------------
+// Leaf / tip kernels (diag.cu)
+// ------------------------------------------------------------------------------------------------
+cudaError_t launch_potrf_inv_tile(double* A, int ld, int n, double* diagL, long long grow0,
+                                  unsigned long long* pivot_flag, cudaStream_t st);
+cudaError_t launch_tip(const double* Tt, int a, int nr, int do_chol, double* LT, double* zT, double* xT, double* ZT,
+                       double* diagL, long long grow0, unsigned long long* pivot_flag, cudaStream_t st);
+cudaError_t launch_zero_upper(double* A, int ld, int n, cudaStream_t st);
+cudaError_t launch_tip_inverse(const double* LT, int a, double* ZT, cudaStream_t st);
+
+// ------------------------------------------------------------------------------------------------
+// Skinny (arrow / vector) kernels (skinny.cu)
+// ------------------------------------------------------------------------------------------------
+cudaError_t launch_skinny_nt(int P, int J, int K, const double* R, int ldr, const double* M, int ldm, int tri,
+                             double alpha, double beta, const double* in, int ldin, double* out, int ldo,
+                             cudaStream_t st);
+size_t skinny_nn_part_doubles(int P, int K, int J);
+cudaError_t launch_skinny_nn(int P, int K, int J, const double* R, int ldr, const double* M, int ldm, int tri,
+                             double alpha, double beta, const double* in, int ldin, double* out, int ldo,
+                             double* part, cudaStream_t st);
+cudaError_t launch_small_nt(int PU, int PV, int K, const double* U, int ldu, const double* V, int ldv, double alpha,
+                            double* Tt, int ldt, cudaStream_t st);
+// Y[r][j] = beta * In[r][j] + alpha * sum_q S[r][q] * E[q][j]   (S: R x Q, lds; E: Q x J)
+cudaError_t launch_small_left_mul(int R, int Q, int J, const double* S, int lds, const double* E, int lde,
+                                  double alpha, double beta, const double* In, int ldin, double* Y, int ldy,
+                                  cudaStream_t st);
+
+// ------------------------------------------------------------------------------------------------
+// Model context, theta-derived parameters (model.cu), assembly (assemble.cu), contractions (contract.cu)
+// ------------------------------------------------------------------------------------------------
+constexpr int KMAX = 4;    // response variables
+constexpr int AMAX = 8;    // arrow width (skinny kernels hold a+1 <= 9 rows)
+constexpr int DMAX = 3 * KMAX + KMAX * (KMAX - 1) / 2 + KMAX;
+
+struct DevParams {          // lives in device memory; written by theta_prep_kernel
+  double theta[DMAX];
+  double E[KMAX][3];        // exp(theta_{m,c})
+  double Lam[KMAX][KMAX];   // unit lower-triangular coupling (R12)
+  double tau[KMAX];         // noise precisions
+  double W[3][KMAX][KMAX];  // W_c[i][j] = sum_m E[m][c] Lam[m][i] Lam[m][j]  (Eq. 10)
+};
+
+struct ModelDims {
+  int nt, g, ns, k, a, apr, b, d;
+  long long N;
+  double h, fixed_prec;
+};
+
+struct bta_ctx {
+  ModelDims md;
+  int device;
+  long long m;
+  // observations on the device
+  int *o_var, *o_node, *o_time;
+  double *o_cov, *o_y;
+  // theta-independent aggregates
+  double *cnt, *zsum, *ZZ, *ysum, *zy, *yy, *mv;  // [nt][b], [nt][a][b], [k][a][a], [nt][b], [k][a], [k], [k]
+  DevParams* P;
+  double* theta_dev;                 // staging for H2D of theta
+  unsigned long long* pivot_flag;    // device; ~0ull = none
+  double* small;                     // device scratch for tips, partial sums, outputs (carved in model.cu)
+  size_t small_doubles;
+  double* host_pinned;               // pinned host staging (theta in, f/grad/intermediates out)
+  cudaStream_t s_side;               // second chain's stream
+  cudaEvent_t ev[16];
+  long long launches;
+  long long last_pivot;
+  // last intermediates (host)
+  double last_ld[2], last_quad;
+  std::vector<double> last_parts, last_rss;
+  double* last_x_dev;                // device pointer into the caller's workspace (valid until it is reused)
+};
+
+#define BTA_COUNT(ctx) ((ctx)->launches++)
+
+// assemble.cu
+cudaError_t launch_theta_prep(bta_ctx* c, cudaStream_t st);
+// Writes D (strict upper zero), B, the arrow rows C (block stride c_stride, row stride b), T and the rhs
+// (time block t at rhs + t * rhs_stride; tip at rhs_tip).  Any of B, C, T, rhs may be NULL.
+cudaError_t launch_assemble(bta_ctx* c, int which, double* D, long long d_stride, double* B, long long b_stride,
+                            double* C, long long c_stride, double* T, int ldt, double* rhs, long long rhs_stride,
+                            double* rhs_tip, int rhs_tip_stride, cudaStream_t st);
+cudaError_t run_setup_aggregates(bta_ctx* c, cudaStream_t st);
+
+// contract.cu -- layout of the small device scratch (offsets in doubles into bta_ctx::small)
+struct SmallLayout {
+  int nx;                       // CTAs along the node axis of the stencil kernels = ceil(ns / 256)
+  size_t trc[2];                // [chain][nt][2][k][k][nx][3]   traces <Z^(ij), K_c> per block, per CTA
+  size_t qd;                    // [nt][2][k][k][nx][3]          x^(i)T K_c x^(j)
+  size_t noise;                 // [nt][k][nx]
+  size_t ldpart[2];             // [64]
+  size_t rsspart;               // [256][k]
+  size_t Tt[2], LT[2], zT[2], xT[2], ZT[2];   // tips per chain
+  size_t out;                   // f, grad[d], ld[2], parts[3d], rss[k], quad
+  size_t total;
+};
+SmallLayout small_layout(const ModelDims& md);
+enum { CH_PRIOR = 0, CH_COND = 1 };
+
+cudaError_t launch_trace_stencil(bta_ctx* c, int chain, int t, int kind, const double* Z, int ld, cudaStream_t st);
+cudaError_t launch_noise_trace(bta_ctx* c, int t, const double* ZD, int ld, const double* ZC, int ldzc,
+                               cudaStream_t st);
+cudaError_t launch_quad_stencil(bta_ctx* c, const double* x, cudaStream_t st);
+cudaError_t launch_logdet_partial(bta_ctx* c, int chain, const double* dvec, cudaStream_t st);
+cudaError_t launch_residual(bta_ctx* c, const double* x, cudaStream_t st);
+cudaError_t launch_scalars(bta_ctx* c, cudaStream_t st);
+cudaError_t launch_logdet_final(bta_ctx* c, int chain, double* out, cudaStream_t st);

@@ -1,0 +1,184 @@
+// Leaf kernels of the blocked POTRF/TRTRI recursion and the arrow tip.
+//
+// potrf_inv_tile: one CTA factors an n x n (n <= 64) diagonal tile A = L L^T and inverts L in the same
+// sweep, in place in shared memory: at step k the columns j <= k of the working array hold the rows of
+// L^-1 built so far (forward elimination applied to the identity) and the columns j > k hold the Schur
+// complement.  Output: X = L^-1 (lower; strict upper of the tile zeroed), diag(L) for the log-determinant
+// (PAPER.md:48), and the first non-positive pivot (Algorithm 1 line 3 needs D_i - S_{i-1} > 0).
+#include "common.cuh"
+
+namespace {
+
+constexpr int NB = 64;
+constexpr int LDW = NB + 1;
+
+__global__ void __launch_bounds__(256) potrf_inv_tile_kernel(double* __restrict__ A, int ld, int n,
+                                                             double* __restrict__ diagL, long long grow0,
+                                                             unsigned long long* __restrict__ pivot_flag) {
+  __shared__ double W[NB * LDW];
+  __shared__ double lcol[NB], xrow[NB];
+  const int tid = threadIdx.x;
+  for (int e = tid; e < NB * NB; e += 256) {
+    int i = e / NB, j = e % NB;
+    double v = (i == j) ? 1.0 : 0.0;
+    if (i < n && j <= i) v = A[(long long)i * ld + j];
+    W[i * LDW + j] = v;
+  }
+  __syncthreads();
+  const int ti = tid >> 2, tq = tid & 3;
+  for (int k = 0; k < n; ++k) {
+    double piv = W[k * LDW + k];
+    if (!(piv > 0.0)) {  // also catches NaN
+      if (tid == 0) atomicMin(pivot_flag, (unsigned long long)(grow0 + k + 1));
+      piv = 1.0;
+    }
+    const double d = sqrt(piv), rd = 1.0 / d;
+    if (tid < NB) {
+      if (tid > k) lcol[tid] = W[tid * LDW + k] * rd;
+    } else if (tid < 2 * NB) {
+      int j = tid - NB;
+      if (j < k) xrow[j] = W[k * LDW + j] * rd;
+      if (j == k) xrow[j] = rd;
+    }
+    if (tid == 0 && diagL) diagL[k] = d;
+    __syncthreads();
+    if (ti > k) {
+      const double li = lcol[ti];
+      double* w = W + ti * LDW;
+      for (int j = tq; j <= ti; j += 4) {
+        if (j < k)
+          w[j] -= li * xrow[j];
+        else if (j == k)
+          w[j] = -li * xrow[k];
+        else
+          w[j] -= li * lcol[j];
+      }
+    } else if (ti == k) {
+      for (int j = tq; j <= k; j += 4) W[k * LDW + j] = xrow[j];
+    }
+    __syncthreads();
+  }
+  for (int e = tid; e < n * n; e += 256) {
+    int i = e / n, j = e % n;
+    A[(long long)i * ld + j] = (j <= i) ? W[i * LDW + j] : 0.0;
+  }
+}
+
+// Arrow tip (Algorithm 1 line 11, Eq. 3, and Z_T = L_T^-T L_T^-1 of the selected inversion, R10).
+// Tt is [a][a+nr]: the reduced tip T~_n (lower triangle read; used when do_chol) and, in columns a..a+nr-1,
+// the reduced right-hand sides r_T - v_T.  do_chol = 0: L_T is given (solve with an existing factor).
+// Outputs zT[r][a], xT[r][a] per right-hand side r.  One thread: a <= 16, O(a^3) work, once per sweep.
+__global__ void tip_kernel(const double* __restrict__ Tt, int a, int nr, int do_chol, double* __restrict__ LT,
+                           double* __restrict__ zT, double* __restrict__ xT, double* __restrict__ ZT,
+                           double* __restrict__ diagL, long long grow0, unsigned long long* pivot_flag) {
+  if (threadIdx.x != 0 || blockIdx.x != 0) return;
+  const int ldt = a + nr;
+  double L[16][16], Xi[16][16];
+  for (int i = 0; i < a; ++i)
+    for (int j = 0; j < a; ++j) {
+      L[i][j] = (j <= i) ? (do_chol ? Tt[i * ldt + j] : LT[i * a + j]) : 0.0;
+      Xi[i][j] = 0.0;
+    }
+  if (do_chol) {
+    for (int k = 0; k < a; ++k) {
+      double piv = L[k][k];
+      for (int q = 0; q < k; ++q) piv -= L[k][q] * L[k][q];
+      if (!(piv > 0.0)) {
+        atomicMin(pivot_flag, (unsigned long long)(grow0 + k + 1));
+        piv = 1.0;
+      }
+      double d = sqrt(piv);
+      L[k][k] = d;
+      if (diagL) diagL[k] = d;
+      for (int i = k + 1; i < a; ++i) {
+        double s = L[i][k];
+        for (int q = 0; q < k; ++q) s -= L[i][q] * L[k][q];
+        L[i][k] = s / d;
+      }
+    }
+  }
+  for (int j = 0; j < a; ++j) {  // Xi = L^-1 column by column
+    Xi[j][j] = 1.0 / L[j][j];
+    for (int i = j + 1; i < a; ++i) {
+      double s = 0.0;
+      for (int q = j; q < i; ++q) s += L[i][q] * Xi[q][j];
+      Xi[i][j] = -s / L[i][i];
+    }
+  }
+  if (do_chol) {
+    for (int i = 0; i < a; ++i)
+      for (int j = 0; j < a; ++j) {
+        LT[i * a + j] = L[i][j];
+        double s = 0.0;
+        for (int q = (i > j ? i : j); q < a; ++q) s += Xi[q][i] * Xi[q][j];
+        if (ZT) ZT[i * a + j] = s;
+      }
+  }
+  for (int r = 0; r < nr; ++r) {
+    double z[16];
+    for (int i = 0; i < a; ++i) {
+      double s = 0.0;
+      for (int q = 0; q <= i; ++q) s += Xi[i][q] * Tt[q * ldt + a + r];
+      z[i] = s;
+      if (zT) zT[r * a + i] = s;
+    }
+    for (int i = 0; i < a; ++i) {
+      double s = 0.0;
+      for (int q = i; q < a; ++q) s += Xi[q][i] * z[q];
+      xT[r * a + i] = s;
+    }
+  }
+}
+
+// Zero the strict upper triangle of an n x n block (the library keeps lower triangles authoritative).
+__global__ void zero_upper_kernel(double* __restrict__ A, int ld, int n) {
+  const int j = blockIdx.x * blockDim.x + threadIdx.x, i = blockIdx.y;
+  if (j < n && j > i) A[(long long)i * ld + j] = 0.0;
+}
+
+// Z_T from a given L_T (selected inversion started from a stored factor).
+__global__ void tip_inverse_kernel(const double* __restrict__ LT, int a, double* __restrict__ ZT) {
+  if (threadIdx.x != 0 || blockIdx.x != 0) return;
+  double Xi[16][16];
+  for (int i = 0; i < a; ++i)
+    for (int j = 0; j < a; ++j) Xi[i][j] = 0.0;
+  for (int j = 0; j < a; ++j) {
+    Xi[j][j] = 1.0 / LT[j * a + j];
+    for (int i = j + 1; i < a; ++i) {
+      double s = 0.0;
+      for (int q = j; q < i; ++q) s += LT[i * a + q] * Xi[q][j];
+      Xi[i][j] = -s / LT[i * a + i];
+    }
+  }
+  for (int i = 0; i < a; ++i)
+    for (int j = 0; j < a; ++j) {
+      double s = 0.0;
+      for (int q = (i > j ? i : j); q < a; ++q) s += Xi[q][i] * Xi[q][j];
+      ZT[i * a + j] = s;
+    }
+}
+
+}  // namespace
+
+cudaError_t launch_potrf_inv_tile(double* A, int ld, int n, double* diagL, long long grow0,
+                                  unsigned long long* pivot_flag, cudaStream_t st) {
+  potrf_inv_tile_kernel<<<1, 256, 0, st>>>(A, ld, n, diagL, grow0, pivot_flag);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_tip(const double* Tt, int a, int nr, int do_chol, double* LT, double* zT, double* xT, double* ZT,
+                       double* diagL, long long grow0, unsigned long long* pivot_flag, cudaStream_t st) {
+  tip_kernel<<<1, 32, 0, st>>>(Tt, a, nr, do_chol, LT, zT, xT, ZT, diagL, grow0, pivot_flag);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_zero_upper(double* A, int ld, int n, cudaStream_t st) {
+  dim3 grid((n + 255) / 256, n);
+  zero_upper_kernel<<<grid, 256, 0, st>>>(A, ld, n);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_tip_inverse(const double* LT, int a, double* ZT, cudaStream_t st) {
+  tip_inverse_kernel<<<1, 32, 0, st>>>(LT, a, ZT);
+  return cudaGetLastError();
+}

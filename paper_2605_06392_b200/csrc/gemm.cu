@@ -1,0 +1,232 @@
+// FP64 tensor-core GEMM for sm_100a: C = alpha * op(A) op(B) + beta * C (row-major).
+//
+// The dense b x b block products of the BTA sweeps (Algorithm 1's TRSM/SYRK steps, and
+// the selected-inversion products) all run through this kernel.  sm_100a has no
+// tcgen05 f64 kind; the FP64 tensor path is warp-level `mma.sync.m8n8k4.f64` (SASS DMMA.8x8x4).
+// Operands are staged in shared memory by a 3-stage cp.async (LDGSTS) pipeline in layouts chosen so the
+// 64-bit fragment loads are bank-conflict-free (leading dimension = 4 mod 16 doubles); accumulators live
+// in registers.  Triangular operands are exploited by restricting the k-range per output tile
+// (KLO_*/KHI_*), symmetric outputs by computing the lower tiles only (OUT_LOWER*).
+#include "common.cuh"
+
+namespace {
+
+constexpr int BK = 16;
+constexpr int STAGES = 3;
+constexpr int KPAD = 4;  // leading dimensions are == 4 (mod 16) doubles
+
+__device__ __forceinline__ void cp_async16(void* smem, const void* gmem, int src_bytes) {
+  unsigned s = (unsigned)__cvta_generic_to_shared(smem);
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;\n" ::"r"(s), "l"(gmem), "r"(src_bytes));
+}
+__device__ __forceinline__ void cp_async8(void* smem, const void* gmem, int src_bytes) {
+  unsigned s = (unsigned)__cvta_generic_to_shared(smem);
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 8, %2;\n" ::"r"(s), "l"(gmem), "r"(src_bytes));
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait() {
+  asm volatile("cp.async.wait_group %0;\n" ::"n"(N));
+}
+
+__device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double b) {
+  asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
+               : "+d"(c0), "+d"(c1)
+               : "d"(a), "d"(b));
+}
+
+// One operand tile (ROWS rows of the output dimension x BK of k) -> shared memory.
+//  KM = false: global is [row][k] (k contiguous); smem [ROWS][BK+KPAD]
+//  KM = true : global is [k][row] (row contiguous); smem [BK][ROWS+KPAD]
+template <int ROWS, bool KM, int NT>
+__device__ __forceinline__ void load_tile(double* sm, const double* __restrict__ g, int ld, int row0, int nrows,
+                                          int k0, int kend, bool vec, int tid) {
+  constexpr int CHUNKS = ROWS * BK / 2;
+#pragma unroll
+  for (int c = tid; c < CHUNKS; c += NT) {
+    int r, k;
+    double* dst;
+    const double* src;
+    int n_ok;  // valid elements of this 2-element chunk (0, 1, 2)
+    if (!KM) {
+      r = c / (BK / 2);
+      k = (c % (BK / 2)) * 2;
+      dst = sm + r * (BK + KPAD) + k;
+      int gr = row0 + r, gk = k0 + k;
+      n_ok = (gr < nrows) ? max(0, min(2, kend - gk)) : 0;
+      src = g + (long long)gr * ld + gk;
+    } else {
+      k = c / (ROWS / 2);
+      r = (c % (ROWS / 2)) * 2;
+      dst = sm + k * (ROWS + KPAD) + r;
+      int gr = row0 + r, gk = k0 + k;
+      n_ok = (gk < kend) ? max(0, min(2, nrows - gr)) : 0;
+      src = g + (long long)gk * ld + gr;
+    }
+    if (vec) {
+      cp_async16(dst, n_ok ? src : g, n_ok * 8);
+    } else {
+      cp_async8(dst, n_ok > 0 ? src : g, n_ok > 0 ? 8 : 0);
+      cp_async8(dst + 1, n_ok > 1 ? src + 1 : g, n_ok > 1 ? 8 : 0);
+    }
+  }
+}
+
+template <int BM, int BN, int WM, int WN, bool A_KM, bool B_KM>
+struct Cfg {
+  static constexpr int NWM = BM / WM, NWN = BN / WN;
+  static constexpr int NT = NWM * NWN * 32;
+  static constexpr int A_ST = A_KM ? BK * (BM + KPAD) : BM * (BK + KPAD);
+  static constexpr int B_ST = B_KM ? BK * (BN + KPAD) : BN * (BK + KPAD);
+  static constexpr int SMEM = STAGES * (A_ST + B_ST) * (int)sizeof(double);
+};
+
+template <int BM, int BN, int WM, int WN, bool A_KM, bool B_KM, int MINB>
+__global__ void __launch_bounds__(Cfg<BM, BN, WM, WN, A_KM, B_KM>::NT, MINB) gemm_kernel(GemmArgs g) {
+  using C_ = Cfg<BM, BN, WM, WN, A_KM, B_KM>;
+  constexpr int NT = C_::NT;
+  extern __shared__ __align__(16) double smem[];
+  double* As = smem;
+  double* Bs = smem + STAGES * C_::A_ST;
+
+  const double* __restrict__ A = g.A;
+  const double* __restrict__ B = g.B;
+  double* __restrict__ C = g.C;
+  int M = g.M, N = g.N, K = g.K;
+  if (g.subs) {
+    GemmSub s = g.subs[blockIdx.z];
+    A += s.offA;
+    B += s.offB;
+    C += s.offC;
+    M = s.M;
+    N = s.N;
+    K = s.K;
+  }
+  const int m0 = blockIdx.y * BM, n0 = blockIdx.x * BN;
+  if (m0 >= M || n0 >= N) return;
+  if (g.out != OUT_FULL && n0 > m0 + BM - 1) return;  // tile entirely above the diagonal
+
+  int kbeg = 0, kend = K;
+  if (g.klo == KLO_N0) kbeg = n0;
+  if (g.klo == KLO_M0) kbeg = m0;
+  if (g.khi == KHI_NEND) kend = min(K, n0 + BN);
+  if (g.khi == KHI_MEND) kend = min(K, m0 + BM);
+  kbeg = (kbeg / BK) * BK;
+
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int wm0 = (warp / C_::NWN) * WM, wn0 = (warp % C_::NWN) * WN;
+  const int gid = lane >> 2, tig = lane & 3;
+
+  const bool vecA = ((g.lda & 1) == 0) && ((((uintptr_t)A) & 15) == 0);
+  const bool vecB = ((g.ldb & 1) == 0) && ((((uintptr_t)B) & 15) == 0);
+
+  double acc[WM / 8][WN / 8][2];
+#pragma unroll
+  for (int i = 0; i < WM / 8; ++i)
+#pragma unroll
+    for (int j = 0; j < WN / 8; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
+
+  const int nk = (kend > kbeg) ? (kend - kbeg + BK - 1) / BK : 0;
+
+  auto issue = [&](int it) {
+    if (it < nk) {
+      int s = it % STAGES;
+      int k0 = kbeg + it * BK;
+      load_tile<BM, A_KM, NT>(As + s * C_::A_ST, A, g.lda, m0, M, k0, kend, vecA, tid);
+      load_tile<BN, B_KM, NT>(Bs + s * C_::B_ST, B, g.ldb, n0, N, k0, kend, vecB, tid);
+    }
+    cp_async_commit();
+  };
+
+#pragma unroll
+  for (int s = 0; s < STAGES - 1; ++s) issue(s);
+
+  for (int it = 0; it < nk; ++it) {
+    cp_async_wait<STAGES - 2>();
+    __syncthreads();
+    issue(it + STAGES - 1);  // refills the stage consumed in iteration it-1 (all warps are past it)
+    const double* as = As + (it % STAGES) * C_::A_ST;
+    const double* bs = Bs + (it % STAGES) * C_::B_ST;
+#pragma unroll
+    for (int kk = 0; kk < BK; kk += 4) {
+      double af[WM / 8], bf[WN / 8];
+#pragma unroll
+      for (int i = 0; i < WM / 8; ++i) {
+        int m = wm0 + i * 8 + gid, k = kk + tig;
+        af[i] = A_KM ? as[k * (BM + KPAD) + m] : as[m * (BK + KPAD) + k];
+      }
+#pragma unroll
+      for (int j = 0; j < WN / 8; ++j) {
+        int n = wn0 + j * 8 + gid, k = kk + tig;
+        bf[j] = B_KM ? bs[k * (BN + KPAD) + n] : bs[n * (BK + KPAD) + k];
+      }
+#pragma unroll
+      for (int i = 0; i < WM / 8; ++i)
+#pragma unroll
+        for (int j = 0; j < WN / 8; ++j) dmma884(acc[i][j][0], acc[i][j][1], af[i], bf[j]);
+    }
+  }
+  cp_async_wait<0>();
+
+  // epilogue: C = alpha * acc + beta * C (guarded; optional lower mask / mirrored write)
+  const double alpha = g.alpha, beta = g.beta;
+  const int ldc = g.ldc;
+  const bool lower = g.out != OUT_FULL, mirror = g.out == OUT_LOWER_MIRROR;
+#pragma unroll
+  for (int i = 0; i < WM / 8; ++i) {
+    const int row = m0 + wm0 + i * 8 + gid;
+    if (row >= M) continue;
+#pragma unroll
+    for (int j = 0; j < WN / 8; ++j) {
+      const int col = n0 + wn0 + j * 8 + tig * 2;
+#pragma unroll
+      for (int e = 0; e < 2; ++e) {
+        const int c = col + e;
+        if (c >= N) continue;
+        if (lower && c > row) continue;
+        double* p = C + (long long)row * ldc + c;
+        double v = alpha * acc[i][j][e];
+        if (beta != 0.0) v += beta * (*p);
+        *p = v;
+        if (mirror && c < row) C[(long long)c * ldc + row] = v;
+      }
+    }
+  }
+}
+
+template <int BM, int BN, int WM, int WN, bool A_KM, bool B_KM, int MINB>
+cudaError_t launch_cfg(const GemmArgs& g, cudaStream_t st) {
+  using C_ = Cfg<BM, BN, WM, WN, A_KM, B_KM>;
+  auto kern = gemm_kernel<BM, BN, WM, WN, A_KM, B_KM, MINB>;
+  static bool attr_done = false;  // per instantiation
+  if (!attr_done) {
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C_::SMEM);
+    if (e != cudaSuccess) return e;
+    attr_done = true;
+  }
+  dim3 grid((g.N + BN - 1) / BN, (g.M + BM - 1) / BM, g.subs ? g.nsub : 1);
+  kern<<<grid, C_::NT, C_::SMEM, st>>>(g);
+  return cudaGetLastError();
+}
+
+template <int BM, int BN, int WM, int WN, int MINB>
+cudaError_t launch_mode(const GemmArgs& g, cudaStream_t st) {
+  switch (g.mode) {
+    case GEMM_NN: return launch_cfg<BM, BN, WM, WN, false, true, MINB>(g, st);
+    case GEMM_NT: return launch_cfg<BM, BN, WM, WN, false, false, MINB>(g, st);
+    case GEMM_TN: return launch_cfg<BM, BN, WM, WN, true, true, MINB>(g, st);
+  }
+  return cudaErrorInvalidValue;
+}
+
+}  // namespace
+
+// Tile choice: 128x128 (8 warps, 32x64 per warp) once the problem fills the chip with big tiles,
+// else 64x64 (4 warps, 32x32 per warp) for more CTAs on small problems.
+cudaError_t launch_gemm(const GemmArgs& g, cudaStream_t st) {
+  if (g.M <= 0 || g.N <= 0) return cudaSuccess;
+  long long tiles128 = (long long)((g.M + 127) / 128) * ((g.N + 127) / 128) * (g.subs ? g.nsub : 1);
+  if (g.out != OUT_FULL) tiles128 = tiles128 / 2 + 1;
+  if (tiles128 >= 120) return launch_mode<128, 128, 32, 64, 1>(g, st);
+  return launch_mode<64, 64, 32, 32, 2>(g, st);
+}

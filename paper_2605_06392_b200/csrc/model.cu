@@ -1,0 +1,129 @@
+// bta_create / bta_destroy: model context, device copies of the observations, theta-independent aggregates.
+#include <cstring>
+
+#include "common.cuh"
+
+namespace {
+template <typename T>
+cudaError_t dev_alloc(T** p, size_t n) {
+  return cudaMalloc((void**)p, (n ? n : 1) * sizeof(T));
+}
+}  // namespace
+
+extern "C" int bta_create(bta_ctx** out, const bta_model_desc* desc, const bta_obs* obs, int device) {
+  if (!out) return BTA_ERR_ARG;
+  *out = nullptr;
+  if (!desc || !obs) {
+    bta_set_error("bta_create: null descriptor or observations");
+    return BTA_ERR_ARG;
+  }
+  if (desc->nt < 1 || desc->g < 1 || desc->k < 1 || desc->k > KMAX || desc->a < desc->k || desc->a > AMAX ||
+      desc->a % desc->k != 0 || !(desc->h > 0.0) || !(desc->fixed_prec > 0.0) || obs->m < 0 ||
+      obs->m > 2000000000LL) {
+    bta_set_error("bta_create: need nt>=1, g>=1, 1<=k<=4, k<=a<=8, a%k==0, h>0, fixed_prec>0, 0<=m<2e9");
+    return BTA_ERR_ARG;
+  }
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || device < 0 || device >= ndev) {
+    bta_set_error("bta_create: no such CUDA device (this library has no CPU fallback)");
+    return BTA_ERR_NODEVICE;
+  }
+  cudaDeviceProp prop;
+  BTA_CUDA_OK(cudaGetDeviceProperties(&prop, device));
+  if (prop.major != 10) {
+    bta_set_error("bta_create: device is not sm_100-class (kernels are built for sm_100a only; no fallback)");
+    return BTA_ERR_NODEVICE;
+  }
+  BTA_CUDA_OK(cudaSetDevice(device));
+  bta_ctx* c = new bta_ctx();
+  ModelDims& md = c->md;
+  md.nt = desc->nt;
+  md.g = desc->g;
+  md.ns = desc->g * desc->g;
+  md.k = desc->k;
+  md.a = desc->a;
+  md.apr = desc->a / desc->k;
+  md.b = md.k * md.ns;
+  md.d = 3 * md.k + md.k * (md.k - 1) / 2 + md.k;
+  md.N = (long long)md.nt * md.b + md.a;
+  md.h = desc->h;
+  md.fixed_prec = desc->fixed_prec;
+  c->device = device;
+  c->m = obs->m;
+  c->launches = 0;
+  c->last_pivot = 0;
+  c->last_x_dev = nullptr;
+  const long long m = obs->m;
+  for (long long i = 0; i < m; ++i) {
+    if (obs->var[i] < 0 || obs->var[i] >= md.k || obs->node[i] < 0 || obs->node[i] >= md.ns || obs->time[i] < 0 ||
+        obs->time[i] >= md.nt) {
+      delete c;
+      bta_set_error("bta_create: observation index out of range");
+      return BTA_ERR_ARG;
+    }
+  }
+  const size_t S = (size_t)md.nt * md.b;
+  BTA_CUDA_OK(dev_alloc(&c->o_var, m));
+  BTA_CUDA_OK(dev_alloc(&c->o_node, m));
+  BTA_CUDA_OK(dev_alloc(&c->o_time, m));
+  BTA_CUDA_OK(dev_alloc(&c->o_cov, m * md.apr));
+  BTA_CUDA_OK(dev_alloc(&c->o_y, m));
+  BTA_CUDA_OK(dev_alloc(&c->cnt, S));
+  BTA_CUDA_OK(dev_alloc(&c->zsum, S * md.a));
+  BTA_CUDA_OK(dev_alloc(&c->ysum, S));
+  BTA_CUDA_OK(dev_alloc(&c->ZZ, (size_t)md.k * md.a * md.a));
+  BTA_CUDA_OK(dev_alloc(&c->zy, (size_t)md.k * md.a));
+  BTA_CUDA_OK(dev_alloc(&c->yy, md.k));
+  BTA_CUDA_OK(dev_alloc(&c->mv, md.k));
+  BTA_CUDA_OK(dev_alloc(&c->P, 1));
+  BTA_CUDA_OK(dev_alloc(&c->theta_dev, DMAX));
+  BTA_CUDA_OK(dev_alloc(&c->pivot_flag, 1));
+  SmallLayout L = small_layout(md);
+  c->small_doubles = L.total;
+  BTA_CUDA_OK(dev_alloc(&c->small, L.total));
+  BTA_CUDA_OK(cudaMemset(c->small, 0, L.total * sizeof(double)));
+  BTA_CUDA_OK(cudaMallocHost((void**)&c->host_pinned, 4096 * sizeof(double)));
+  BTA_CUDA_OK(cudaStreamCreateWithFlags(&c->s_side, cudaStreamNonBlocking));
+  for (auto& e : c->ev) BTA_CUDA_OK(cudaEventCreate(&e));
+  if (m > 0) {
+    BTA_CUDA_OK(cudaMemcpy(c->o_var, obs->var, m * sizeof(int), cudaMemcpyHostToDevice));
+    BTA_CUDA_OK(cudaMemcpy(c->o_node, obs->node, m * sizeof(int), cudaMemcpyHostToDevice));
+    BTA_CUDA_OK(cudaMemcpy(c->o_time, obs->time, m * sizeof(int), cudaMemcpyHostToDevice));
+    BTA_CUDA_OK(cudaMemcpy(c->o_cov, obs->cov, m * md.apr * sizeof(double), cudaMemcpyHostToDevice));
+    BTA_CUDA_OK(cudaMemcpy(c->o_y, obs->y, m * sizeof(double), cudaMemcpyHostToDevice));
+  }
+  BTA_CUDA_OK(run_setup_aggregates(c, 0));
+  *out = c;
+  return BTA_OK;
+}
+
+extern "C" int bta_destroy(bta_ctx* c) {
+  if (!c) return BTA_OK;
+  cudaSetDevice(c->device);
+  cudaFree(c->o_var);
+  cudaFree(c->o_node);
+  cudaFree(c->o_time);
+  cudaFree(c->o_cov);
+  cudaFree(c->o_y);
+  cudaFree(c->cnt);
+  cudaFree(c->zsum);
+  cudaFree(c->ysum);
+  cudaFree(c->ZZ);
+  cudaFree(c->zy);
+  cudaFree(c->yy);
+  cudaFree(c->mv);
+  cudaFree(c->P);
+  cudaFree(c->theta_dev);
+  cudaFree(c->pivot_flag);
+  cudaFree(c->small);
+  cudaFreeHost(c->host_pinned);
+  cudaStreamDestroy(c->s_side);
+  for (auto& e : c->ev) cudaEventDestroy(e);
+  delete c;
+  return BTA_OK;
+}
+
+extern "C" int32_t bta_num_hyper(const bta_ctx* c) { return c ? c->md.d : 0; }
+extern "C" int64_t bta_latent_size(const bta_ctx* c) { return c ? c->md.N : 0; }
+extern "C" int64_t bta_last_pivot(const bta_ctx* c) { return c ? c->last_pivot : 0; }
+extern "C" int64_t bta_kernel_launches(const bta_ctx* c) { return c ? c->launches : 0; }

@@ -1,0 +1,220 @@
+// Bandwidth-bound "skinny" products of the sweeps: a few rows (arrow rows L_C / Z_C, right-hand-side and
+// solution vectors) against one b x b block.  These are the arrow and vector parts of Algorithm 1
+// (PAPER.md:77-96, lines 4-5, 9), of Eqs. 3-5 and of the selected-inversion arrow
+// recurrences (R10).  P <= 16 rows; each kernel reads the b x b block exactly once (HBM roofline).
+#include "common.cuh"
+
+constexpr int NN_KCH = 128;  // rows of M per CTA of skinny_nn (one partial sum each)
+
+namespace {
+
+// out[p][j] = beta * in[p][j] + alpha * sum_{k < kend(j)} R[p][k] * M[j][k],  kend(j) = tri ? j+1 : K.
+// One warp per 4 rows j of M (k contiguous -> coalesced); the R chunk is staged in shared memory.
+template <int PT>
+__global__ void __launch_bounds__(256) skinny_nt_kernel(int P, int J, int K, const double* __restrict__ R, int ldr,
+                                                        const double* __restrict__ M, int ldm, int tri,
+                                                        double alpha, double beta, const double* __restrict__ in,
+                                                        int ldin, double* __restrict__ out, int ldo) {
+  constexpr int KC = 256, RPW = 4;
+  __shared__ double Rs[PT * KC];
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int jbase = blockIdx.x * 32 + warp * RPW;
+  const int jmax_cta = min(J, blockIdx.x * 32 + 32) - 1;
+  const int Kcta = tri ? min(K, jmax_cta + 1) : K;
+  double acc[RPW][PT];
+#pragma unroll
+  for (int r = 0; r < RPW; ++r)
+#pragma unroll
+    for (int p = 0; p < PT; ++p) acc[r][p] = 0.0;
+  for (int k0 = 0; k0 < Kcta; k0 += KC) {
+    __syncthreads();
+    for (int e = tid; e < PT * KC; e += 256) {
+      int p = e / KC, k = e % KC;
+      Rs[e] = (p < P && k0 + k < Kcta) ? R[(long long)p * ldr + k0 + k] : 0.0;
+    }
+    __syncthreads();
+#pragma unroll
+    for (int r = 0; r < RPW; ++r) {
+      const int j = jbase + r;
+      if (j >= J) continue;
+      const int kend = tri ? min(K, j + 1) : K;
+      const double* mrow = M + (long long)j * ldm;
+#pragma unroll
+      for (int q = 0; q < KC / 32; ++q) {
+        const int k = k0 + q * 32 + lane;
+        if (k < kend) {
+          const double m = mrow[k];
+#pragma unroll
+          for (int p = 0; p < PT; ++p) acc[r][p] = fma(m, Rs[p * KC + q * 32 + lane], acc[r][p]);
+        }
+      }
+    }
+  }
+#pragma unroll
+  for (int r = 0; r < RPW; ++r) {
+    const int j = jbase + r;
+#pragma unroll
+    for (int p = 0; p < PT; ++p) {
+      double v = acc[r][p];
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+      if (lane == 0 && j < J && p < P) {
+        double res = alpha * v;
+        if (beta != 0.0) res += beta * in[(long long)p * ldin + j];
+        out[(long long)p * ldo + j] = res;
+      }
+    }
+  }
+}
+
+// part[ks][p][j] = sum_{k in chunk ks, k >= kbeg(j)} R[p][k] * M[k][j],  kbeg(j) = tri ? j : 0.
+// CTA: 128 columns x NN_KCH rows of M; threads (64 x 4): 2 columns each, 4 k-phases reduced through smem.
+template <int PT>
+__global__ void __launch_bounds__(256) skinny_nn_kernel(int P, int K, int J, const double* __restrict__ R, int ldr,
+                                                        const double* __restrict__ M, int ldm, int tri,
+                                                        double* __restrict__ part) {
+  constexpr int KCH = NN_KCH;
+  __shared__ double Rs[PT * KCH];
+  __shared__ double red[4][PT][128];
+  const int tid = threadIdx.x, tx = tid & 63, ty = tid >> 6;
+  const int j0 = blockIdx.x * 128, k0 = blockIdx.y * KCH;
+  const int k1 = min(K, k0 + KCH);
+  const int ja = j0 + tx, jb = j0 + tx + 64;
+  double acc[PT][2];
+#pragma unroll
+  for (int p = 0; p < PT; ++p) acc[p][0] = acc[p][1] = 0.0;
+  const bool skip = tri && (k1 - 1 < j0);  // every row of this chunk is above the diagonal of every column
+  if (!skip) {
+    for (int e = tid; e < PT * KCH; e += 256) {
+      int p = e / KCH, k = e % KCH;
+      Rs[e] = (p < P && k0 + k < k1) ? R[(long long)p * ldr + k0 + k] : 0.0;
+    }
+    __syncthreads();
+    for (int k = k0 + ty; k < k1; k += 4) {
+      const double* mrow = M + (long long)k * ldm;
+      double ma = 0.0, mb = 0.0;
+      if (ja < J && (!tri || k >= ja)) ma = mrow[ja];
+      if (jb < J && (!tri || k >= jb)) mb = mrow[jb];
+#pragma unroll
+      for (int p = 0; p < PT; ++p) {
+        const double r = Rs[p * KCH + (k - k0)];
+        acc[p][0] = fma(r, ma, acc[p][0]);
+        acc[p][1] = fma(r, mb, acc[p][1]);
+      }
+    }
+  }
+#pragma unroll
+  for (int p = 0; p < PT; ++p) {
+    red[ty][p][tx] = acc[p][0];
+    red[ty][p][tx + 64] = acc[p][1];
+  }
+  __syncthreads();
+  for (int e = tid; e < PT * 128; e += 256) {
+    int p = e / 128, c = e % 128;
+    if (p < P && j0 + c < J) {
+      double s = (red[0][p][c] + red[1][p][c]) + (red[2][p][c] + red[3][p][c]);
+      part[((long long)blockIdx.y * P + p) * J + j0 + c] = s;
+    }
+  }
+}
+
+// out[p][j] = alpha * sum_ks part[ks][p][j] + beta * in[p][j]   (fixed order: deterministic)
+__global__ void skinny_nn_finish_kernel(int P, int J, int nks, const double* __restrict__ part, double alpha,
+                                        double beta, const double* __restrict__ in, int ldin,
+                                        double* __restrict__ out, int ldo) {
+  long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (e >= (long long)P * J) return;
+  int p = (int)(e / J), j = (int)(e % J);
+  double s = 0.0;
+  for (int ks = 0; ks < nks; ++ks) s += part[((long long)ks * P + p) * J + j];
+  double res = alpha * s;
+  if (beta != 0.0) res += beta * in[(long long)p * ldin + j];
+  out[(long long)p * ldo + j] = res;
+}
+
+// Tt[p][q] += alpha * sum_k U[p][k] * V[q][k]  for p < PU, q < PV (Algorithm 1 line 9 and v_T of line 5).
+__global__ void __launch_bounds__(256) small_nt_kernel(int PU, int PV, int K, const double* __restrict__ U, int ldu,
+                                                       const double* __restrict__ V, int ldv, double alpha,
+                                                       double* __restrict__ Tt, int ldt) {
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nw = blockDim.x >> 5;
+  for (int pq = blockIdx.x * nw + warp; pq < PU * PV; pq += gridDim.x * nw) {
+    int p = pq / PV, q = pq % PV;
+    double s = 0.0;
+    for (int k = lane; k < K; k += 32) s = fma(U[(long long)p * ldu + k], V[(long long)q * ldv + k], s);
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+    if (lane == 0) Tt[p * ldt + q] += alpha * s;
+  }
+}
+
+// Y[r][j] = beta * In[r][j] + alpha * sum_q S[r][q] * E[q][j]   (tiny left factor: Z_T E_i, x_T^T L_C, ...)
+__global__ void small_left_mul_kernel(int R, int Q, int J, const double* __restrict__ S, int lds,
+                                      const double* __restrict__ E, int lde, double alpha, double beta,
+                                      const double* __restrict__ In, int ldin, double* __restrict__ Y, int ldy) {
+  int j = blockIdx.x * blockDim.x + threadIdx.x;
+  if (j >= J) return;
+  for (int r = 0; r < R; ++r) {
+    double s = 0.0;
+    for (int q = 0; q < Q; ++q) s = fma(S[r * lds + q], E[(long long)q * lde + j], s);
+    double res = alpha * s;
+    if (beta != 0.0) res += beta * In[(long long)r * ldin + j];
+    Y[(long long)r * ldy + j] = res;
+  }
+}
+
+}  // namespace
+
+cudaError_t launch_skinny_nt(int P, int J, int K, const double* R, int ldr, const double* M, int ldm, int tri,
+                             double alpha, double beta, const double* in, int ldin, double* out, int ldo,
+                             cudaStream_t st) {
+  if (P <= 0 || J <= 0) return cudaSuccess;
+  dim3 grid((J + 31) / 32);
+  if (P <= 1)
+    skinny_nt_kernel<1><<<grid, 256, 0, st>>>(P, J, K, R, ldr, M, ldm, tri, alpha, beta, in, ldin, out, ldo);
+  else if (P <= 8)
+    skinny_nt_kernel<8><<<grid, 256, 0, st>>>(P, J, K, R, ldr, M, ldm, tri, alpha, beta, in, ldin, out, ldo);
+  else if (P <= 16)
+    skinny_nt_kernel<16><<<grid, 256, 0, st>>>(P, J, K, R, ldr, M, ldm, tri, alpha, beta, in, ldin, out, ldo);
+  else
+    return cudaErrorInvalidValue;
+  return cudaGetLastError();
+}
+
+size_t skinny_nn_part_doubles(int P, int K, int J) { return (size_t)((K + NN_KCH - 1) / NN_KCH) * P * J; }
+
+cudaError_t launch_skinny_nn(int P, int K, int J, const double* R, int ldr, const double* M, int ldm, int tri,
+                             double alpha, double beta, const double* in, int ldin, double* out, int ldo,
+                             double* part, cudaStream_t st) {
+  if (P <= 0 || J <= 0) return cudaSuccess;
+  const int nks = (K + NN_KCH - 1) / NN_KCH;
+  dim3 grid((J + 127) / 128, nks);
+  if (P <= 1)
+    skinny_nn_kernel<1><<<grid, 256, 0, st>>>(P, K, J, R, ldr, M, ldm, tri, part);
+  else if (P <= 4)
+    skinny_nn_kernel<4><<<grid, 256, 0, st>>>(P, K, J, R, ldr, M, ldm, tri, part);
+  else if (P <= 9)
+    skinny_nn_kernel<9><<<grid, 256, 0, st>>>(P, K, J, R, ldr, M, ldm, tri, part);
+  else
+    return cudaErrorInvalidValue;
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return e;
+  long long tot = (long long)P * J;
+  skinny_nn_finish_kernel<<<(unsigned)((tot + 255) / 256), 256, 0, st>>>(P, J, nks, part, alpha, beta, in, ldin, out,
+                                                                         ldo);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_small_nt(int PU, int PV, int K, const double* U, int ldu, const double* V, int ldv, double alpha,
+                            double* Tt, int ldt, cudaStream_t st) {
+  if (PU <= 0 || PV <= 0) return cudaSuccess;
+  small_nt_kernel<<<8, 256, 0, st>>>(PU, PV, K, U, ldu, V, ldv, alpha, Tt, ldt);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_small_left_mul(int R, int Q, int J, const double* S, int lds, const double* E, int lde,
+                                  double alpha, double beta, const double* In, int ldin, double* Y, int ldy,
+                                  cudaStream_t st) {
+  if (R <= 0 || J <= 0) return cudaSuccess;
+  small_left_mul_kernel<<<(J + 255) / 256, 256, 0, st>>>(R, Q, J, S, lds, E, lde, alpha, beta, In, ldin, Y, ldy);
+  return cudaGetLastError();
+}

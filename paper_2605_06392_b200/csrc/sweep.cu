@@ -1,0 +1,239 @@
+// Host orchestration of the sweeps over the nt time blocks (sequential in t, parallel inside each block).
+//   forward : Algorithm 1 (R8) -- blocked POTRF + TRTRI of D_t - S_{t-1}, L_B = B X^T,
+//             Schur update of D_{t+1}, arrow rows and right-hand-side rows, tip.
+//   backward: Eqs. 3-5 + BTA selected inversion (R10) + the Eq. 7
+//             trace contractions fused per block (only Z_Dt and Z_D{t+1} are live).
+// The factor is held in inverse-diagonal form X_t = L_Dt^-1, so every large step is a GEMM (gemm.cu).
+#include "sweep.h"
+
+#define CK(call)                      \
+  do {                                \
+    cudaError_t e_ = (call);          \
+    if (e_ != cudaSuccess) return e_; \
+  } while (0)
+
+namespace {
+inline GemmArgs G(int mode, int M, int N, int K, double alpha, const double* A, int lda, const double* B, int ldb,
+                  double beta, double* C, int ldc, int klo, int khi, int out) {
+  return GemmArgs{A, B, C, M, N, K, lda, ldb, ldc, alpha, beta, mode, klo, khi, out, nullptr, 0};
+}
+}  // namespace
+
+// A[lo:hi, lo:hi] (lower, SPD) -> X = L^-1 in place; T1, T2: scratch with the same leading dimension.
+// Recursive on 64-wide tiles:  chol/inv(A11);  L21 = A21 X11^T;  A22 -= L21 L21^T;  chol/inv(A22);
+// X21 = -X22 (L21 X11).  b^3/3 (POTRF) + b^3/3 (TRTRI) flops, all but the 64x64 leaves in DMMA GEMMs.
+cudaError_t potrf_inv(bta_ctx* c, double* A, int ld, int lo, int hi, double* T1, double* T2, double* diagL,
+                      long long grow0, cudaStream_t st) {
+  const int n = hi - lo;
+  if (n <= 0) return cudaSuccess;
+  if (n <= 64) {
+    BTA_COUNT(c);
+    return launch_potrf_inv_tile(A + (long long)lo * ld + lo, ld, n, diagL ? diagL + lo : nullptr, grow0 + lo,
+                                 c->pivot_flag, st);
+  }
+  const int ntile = (n + 63) / 64;
+  const int mid = lo + 64 * ((ntile + 1) / 2);
+  const int s1 = mid - lo, s2 = hi - mid;
+  CK(potrf_inv(c, A, ld, lo, mid, T1, T2, diagL, grow0, st));
+  double* A11 = A + (long long)lo * ld + lo;
+  double* A21 = A + (long long)mid * ld + lo;
+  double* A22 = A + (long long)mid * ld + mid;
+  double* L21 = T1 + (long long)mid * ld + lo;
+  double* LX = T2 + (long long)mid * ld + lo;
+  CK(launch_gemm(G(GEMM_NT, s2, s1, s1, 1.0, A21, ld, A11, ld, 0.0, L21, ld, KLO_ZERO, KHI_NEND, OUT_FULL), st));
+  CK(launch_gemm(G(GEMM_NT, s2, s2, s1, -1.0, L21, ld, L21, ld, 1.0, A22, ld, KLO_ZERO, KHI_K, OUT_LOWER), st));
+  c->launches += 2;
+  CK(potrf_inv(c, A, ld, mid, hi, T1, T2, diagL, grow0, st));
+  CK(launch_gemm(G(GEMM_NN, s2, s1, s1, 1.0, L21, ld, A11, ld, 0.0, LX, ld, KLO_N0, KHI_K, OUT_FULL), st));
+  CK(launch_gemm(G(GEMM_NN, s2, s1, s2, -1.0, A22, ld, LX, ld, 0.0, A21, ld, KLO_ZERO, KHI_MEND, OUT_FULL), st));
+  c->launches += 2;
+  return cudaSuccess;
+}
+
+namespace {
+__global__ void tip_init_kernel(int a, int nr, const double* __restrict__ T, int ldt_in,
+                                const double* __restrict__ rhs_tip, int tip_stride, double* __restrict__ Tt) {
+  const int p = threadIdx.x / (a + nr), q = threadIdx.x % (a + nr);
+  if (p >= a) return;
+  Tt[p * (a + nr) + q] = (q < a) ? T[p * ldt_in + q] : rhs_tip[(long long)(q - a) * tip_stride + p];
+}
+__global__ void scale_copy_kernel(long long n, double alpha, const double* __restrict__ in, double* __restrict__ out) {
+  long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (e < n) out[e] = alpha * in[e];
+}
+}  // namespace
+
+cudaError_t chain_forward(Chain& ch, cudaStream_t st) {
+  bta_ctx* c = ch.c;
+  const int b = ch.b, nt = ch.nt, a = ch.a, P = ch.P(), ldt = a + ch.nr;
+  const long long bb = (long long)b * b;
+  if (a > 0) {
+    tip_init_kernel<<<1, a * ldt, 0, st>>>(a, ch.nr, ch.T, ch.ldT, ch.rhs_tip, ch.rhs_tip_stride, ch.Tt);
+    BTA_COUNT(c);
+  }
+  for (int t = 0; t < nt; ++t) {
+    double* Dt = ch.D + t * ch.d_stride;
+    if (ch.zero_upper && ch.factor_blocks) {
+      CK(launch_zero_upper(Dt, b, b, st));
+      BTA_COUNT(c);
+    }
+    if (ch.factor_blocks)
+      CK(potrf_inv(c, Dt, b, 0, b, ch.W2, ch.W3, ch.dvec ? ch.dvec + (long long)t * b : nullptr, (long long)t * b,
+                   st));
+    if (P > 0) {
+      // stack rows: arrow rows (factor mode) then right-hand-side rows.
+      //   R~_t = R_t - R^_{t-1} L_B{t-1}^T  (lines 4-5);   R^_t = R~_t X_t^T
+      const double* src = ch.Rin + t * ch.rin_stride;
+      int ld_src = ch.ld_rin;
+      if (t == 0 && ch.Rin == ch.Rout) {  // in-place factor: the stack product below must not alias its input
+        CK(cudaMemcpy2DAsync(ch.Rtmp, b * sizeof(double), src, ld_src * sizeof(double), b * sizeof(double), P,
+                             cudaMemcpyDeviceToDevice, st));
+        src = ch.Rtmp;
+        ld_src = b;
+      }
+      if (t > 0) {
+        double* tmp = ch.Rtmp ? ch.Rtmp : ch.Rin + t * ch.rin_stride;
+        const int ld_tmp = ch.Rtmp ? b : ch.ld_rin;
+        CK(launch_skinny_nt(P, b, b, ch.Rout + (t - 1) * ch.rout_stride, ch.ld_rout, ch.Bout + (t - 1) * ch.b_stride, b,
+                            0, -1.0, 1.0, src, ld_src, tmp, ld_tmp, st));
+        BTA_COUNT(c);
+        src = tmp;
+        ld_src = ld_tmp;
+      }
+      double* Rh = ch.Rout + t * ch.rout_stride;
+      CK(launch_skinny_nt(P, b, b, src, ld_src, Dt, b, 1, 1.0, 0.0, nullptr, 0, Rh, ch.ld_rout, st));
+      BTA_COUNT(c);
+      if (a > 0) {
+        // T~ -= L_C L_C^T (line 9) and r_T - v_T, v_T += L_C z (line 5): columns [0,a) and [a, a+nr) of Tt
+        if (ch.arrow_rows) {
+          CK(launch_small_nt(a, P, b, Rh, ch.ld_rout, Rh, ch.ld_rout, -1.0, ch.Tt, ldt, st));
+          BTA_COUNT(c);
+        } else if (ch.arrow_given) {
+          CK(launch_small_nt(a, ch.nr, b, ch.LCgiven + t * ch.lc_stride, b, Rh, ch.ld_rout, -1.0, ch.Tt + a, ldt, st));
+          BTA_COUNT(c);
+        }
+      }
+    }
+    if (t < nt - 1 && ch.factor_blocks) {
+      double* Bi = ch.Bin + t * ch.b_stride;
+      double* Bo = ch.Bout + t * ch.b_stride;
+      double* dst = (Bi == Bo) ? ch.W1 : Bo;
+      CK(launch_gemm(G(GEMM_NT, b, b, b, 1.0, Bi, b, Dt, b, 0.0, dst, b, KLO_ZERO, KHI_NEND, OUT_FULL), st));
+      CK(launch_gemm(G(GEMM_NT, b, b, b, -1.0, dst, b, dst, b, 1.0, ch.D + (t + 1) * ch.d_stride, b, KLO_ZERO, KHI_K,
+                       OUT_LOWER),
+                     st));
+      c->launches += 2;
+      if (dst != Bo) CK(cudaMemcpyAsync(Bo, dst, bb * sizeof(double), cudaMemcpyDeviceToDevice, st));
+    }
+  }
+  if (a > 0) {
+    CK(launch_tip(ch.Tt, a, ch.nr, ch.tip_chol ? 1 : 0, ch.LT, ch.zT, ch.xT, ch.ZT,
+                  ch.dvec ? ch.dvec + (long long)nt * b : nullptr, (long long)nt * b, c->pivot_flag, st));
+    BTA_COUNT(c);
+  }
+  return cudaSuccess;
+}
+
+// Backward sweep t = nt-1 .. 0.  Needs from the forward sweep: X_t in D(t), L_Bt in Bout(t), the arrow factor
+// rows L_Ct, z_t (rows a.. of Rout(t) when arrow_rows, else rows 0..), and the tip outputs x_T, Z_T.
+cudaError_t chain_backward(Chain& ch, cudaStream_t st) {
+  bta_ctx* c = ch.c;
+  const int b = ch.b, nt = ch.nt, a = ch.a, nr = ch.nr;
+  const long long bb = (long long)b * b;
+  const bool arrow = ch.arrow();
+  const int zrow0 = ch.arrow_rows ? a : 0;  // first rhs row inside the Rout stack
+  for (int t = nt - 1; t >= 0; --t) {
+    const double* X = ch.D + t * ch.d_stride;
+    double* LB = (t < nt - 1) ? ch.Bout + t * ch.b_stride : nullptr;
+    const double* LC = nullptr;
+    int ld_lc = b;
+    if (ch.arrow_rows) {
+      LC = ch.Rout + t * ch.rout_stride;
+      ld_lc = ch.ld_rout;
+    } else if (ch.arrow_given) {
+      LC = ch.LCgiven + t * ch.lc_stride;
+    }
+    // ---- upper solve (Eqs. 3-5):  u = z_t - L_Bt^T x_{t+1} - L_Ct^T x_T ;  x_t = X_t^T u  (row-vector form)
+    if (nr > 0) {
+      const double* z = ch.Rout + t * ch.rout_stride + (long long)zrow0 * ch.ld_rout;
+      const double* u = z;
+      int ld_u = ch.ld_rout;
+      if (arrow) {
+        CK(launch_small_left_mul(nr, a, b, ch.xT, a, LC, ld_lc, -1.0, 1.0, u, ld_u, ch.ubuf, b, st));
+        BTA_COUNT(c);
+        u = ch.ubuf;
+        ld_u = b;
+      }
+      if (t < nt - 1) {
+        CK(launch_skinny_nn(nr, b, b, ch.xout + (long long)(t + 1) * b, (int)ch.ld_x, LB, b, 0, -1.0, 1.0, u, ld_u,
+                            ch.ubuf, b, ch.part, st));
+        c->launches += 2;
+        u = ch.ubuf;
+        ld_u = b;
+      }
+      CK(launch_skinny_nn(nr, b, b, u, ld_u, X, b, 1, 1.0, 0.0, nullptr, 0, ch.xout + (long long)t * b, (int)ch.ld_x,
+                          ch.part, st));
+      c->launches += 2;
+    }
+    if (!ch.selinv) continue;
+    // ---- selected inversion (R10), tensor-friendly form:  G = L_B X,  E = L_C X,
+    //      Z_B = -Z_D{t+1} G - Z_C{t+1}^T E,  Z_C = -Z_C{t+1} G - Z_T E,  Z_D = X^T X - Z_B^T G - Z_C^T E
+    double* ZDcur = (t & 1) ? ch.W2 : ch.W3;
+    double* ZDnext = (t & 1) ? ch.W3 : ch.W2;
+    double* ZCcur = ch.ZC[t & 1];
+    double* ZCnext = ch.ZC[(t & 1) ^ 1];
+    if (arrow) {
+      CK(launch_skinny_nn(a, b, b, LC, ld_lc, X, b, 1, 1.0, 0.0, nullptr, 0, ch.Ebuf, b, ch.part, st));  // E
+      CK(launch_small_left_mul(a, a, b, ch.ZT, a, ch.Ebuf, b, 1.0, 0.0, nullptr, 0, ch.Ybuf, b, st));   // Z_T E
+      c->launches += 3;
+    }
+    if (t < nt - 1) {
+      double* Gm = ch.W1;
+      CK(launch_gemm(G(GEMM_NN, b, b, b, 1.0, LB, b, X, b, 0.0, Gm, b, KLO_N0, KHI_K, OUT_FULL), st));
+      BTA_COUNT(c);
+      if (arrow) {
+        CK(launch_skinny_nn(a, b, b, ZCnext, b, Gm, b, 0, -1.0, -1.0, ch.Ybuf, b, ZCcur, b, ch.part, st));
+        c->launches += 2;
+      }
+      double* ZB = LB;  // L_Bt is dead from here on: Z_Bt takes its slot
+      CK(launch_gemm(G(GEMM_NN, b, b, b, -1.0, ZDnext, b, Gm, b, 0.0, ZB, b, KLO_ZERO, KHI_K, OUT_FULL), st));
+      BTA_COUNT(c);
+      if (arrow) {
+        CK(launch_gemm(G(GEMM_TN, b, b, a, -1.0, ZCnext, b, ch.Ebuf, b, 1.0, ZB, b, KLO_ZERO, KHI_K, OUT_FULL), st));
+        BTA_COUNT(c);
+      }
+      CK(launch_gemm(G(GEMM_TN, b, b, b, 1.0, X, b, X, b, 0.0, ZDcur, b, KLO_M0, KHI_K, OUT_LOWER), st));
+      CK(launch_gemm(G(GEMM_TN, b, b, b, -1.0, ZB, b, Gm, b, 1.0, ZDcur, b, KLO_ZERO, KHI_K,
+                       arrow ? OUT_LOWER : OUT_LOWER_MIRROR),
+                     st));
+      c->launches += 2;
+    } else {
+      if (arrow) {
+        scale_copy_kernel<<<(unsigned)(((long long)a * b + 255) / 256), 256, 0, st>>>((long long)a * b, -1.0, ch.Ybuf,
+                                                                                      ZCcur);
+        BTA_COUNT(c);
+      }
+      CK(launch_gemm(G(GEMM_TN, b, b, b, 1.0, X, b, X, b, 0.0, ZDcur, b, KLO_M0, KHI_K,
+                       arrow ? OUT_LOWER : OUT_LOWER_MIRROR),
+                     st));
+      BTA_COUNT(c);
+    }
+    if (arrow) {
+      CK(launch_gemm(G(GEMM_TN, b, b, a, -1.0, ZCcur, b, ch.Ebuf, b, 1.0, ZDcur, b, KLO_ZERO, KHI_K, OUT_LOWER_MIRROR),
+                     st));
+      BTA_COUNT(c);
+    }
+    if (ch.contract) {
+      CK(launch_trace_stencil(c, ch.chain, t, 0, ZDcur, b, st));
+      if (t < nt - 1) CK(launch_trace_stencil(c, ch.chain, t, 1, LB, b, st));
+      if (arrow) CK(launch_noise_trace(c, t, ZDcur, b, ZCcur, b, st));
+    }
+    if (ch.selinv_inplace) {
+      CK(cudaMemcpyAsync(ch.D + t * ch.d_stride, ZDcur, bb * sizeof(double), cudaMemcpyDeviceToDevice, st));
+      if (arrow && ch.Cout)
+        CK(cudaMemcpyAsync(ch.Cout + t * ch.cout_stride, ZCcur, (size_t)a * b * sizeof(double),
+                           cudaMemcpyDeviceToDevice, st));
+    }
+  }
+  return cudaSuccess;
+}

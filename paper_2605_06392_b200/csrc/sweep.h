@@ -1,0 +1,46 @@
+// One BTA chain (Q_p or Q_c) as the sweeps see it: pointers into caller-owned device memory.
+#pragma once
+#include "common.cuh"
+
+struct Chain {
+  bta_ctx* c = nullptr;
+  int chain = CH_COND;         // slot of the partial-sum buffers (CH_PRIOR / CH_COND)
+  int b = 0, nt = 0, a = 0;
+  int nr = 0;                  // right-hand-side rows carried through the sweeps
+  bool factor_blocks = true;   // forward: POTRF/TRTRI of the diagonal blocks, L_B, Schur updates
+  bool arrow_rows = false;     // forward: the stack holds the a arrow rows C_t, factored to L_Ct
+  bool arrow_given = false;    // the arrow factor rows L_Ct already exist (solve with a stored factor)
+  bool tip_chol = true;        // forward: factor the reduced tip (else L_T is given)
+  bool zero_upper = false;     // forward: clear the strict upper triangle of D_t first
+  bool selinv = false;         // backward: selected inversion
+  bool contract = false;       // backward: accumulate the Eq. 7 traces per block (fused gradient)
+  bool selinv_inplace = false; // backward: copy Z_D / Z_C back over D / C (bta_selinv)
+
+  int P() const { return (arrow_rows ? a : 0) + nr; }
+  bool arrow() const { return arrow_rows || arrow_given; }
+
+  double* D = nullptr;    long long d_stride = 0;      // D(t) = D + t * d_stride   (b x b, ld b)
+  double* Bin = nullptr;  double* Bout = nullptr; long long b_stride = 0;
+  // forward stack: rows [arrow rows | rhs rows] of time block t
+  double* Rin = nullptr;  long long rin_stride = 0;  int ld_rin = 0;
+  double* Rout = nullptr; long long rout_stride = 0; int ld_rout = 0;   // [L_Ct | z_t]
+  double* Rtmp = nullptr;                                               // P x b scratch, or NULL: in place in Rin
+  const double* LCgiven = nullptr; long long lc_stride = 0;             // arrow_given: L_Ct = LCgiven + t * lc_stride
+  double* T = nullptr; int ldT = 0;                                     // tip (a x a)
+  const double* rhs_tip = nullptr; int rhs_tip_stride = 0;              // rhs_tip[r * stride + p]
+  // scratch
+  double *W1 = nullptr, *W2 = nullptr, *W3 = nullptr;                   // b x b each
+  double* part = nullptr;                                               // skinny_nn partial sums
+  double *ubuf = nullptr, *Ebuf = nullptr, *Ybuf = nullptr;             // [nr][b], [a][b], [a][b]
+  double* ZC[2] = {nullptr, nullptr};                                   // [a][b] ping-pong
+  double* dvec = nullptr;                                               // diag(L), N doubles, or NULL
+  double *Tt = nullptr, *LT = nullptr, *zT = nullptr, *xT = nullptr, *ZT = nullptr;
+  // backward outputs
+  double* xout = nullptr; long long ld_x = 0;                           // x rows: xout + r * ld_x + t * b
+  double* Cout = nullptr; long long cout_stride = 0;                    // selinv_inplace: Z_Ct destination
+};
+
+cudaError_t potrf_inv(bta_ctx* c, double* A, int ld, int lo, int hi, double* T1, double* T2, double* diagL,
+                      long long grow0, cudaStream_t st);
+cudaError_t chain_forward(Chain& ch, cudaStream_t st);
+cudaError_t chain_backward(Chain& ch, cudaStream_t st);
