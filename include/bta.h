@@ -134,8 +134,9 @@ enum {
 /* Intermediates of the last inla_value_and_grad (HOST outputs; any pointer may be NULL):
  * ld[2] = {log det Q_p, log det Q_c}; x DEVICE->HOST copy of x* [N]; parts[3*d] = Phase A, B, C per
  * hyperparameter (Eq. 6 terms before the -1/2, -1/2, +1/2 factors); rss[k] = ||y_v - A_v x*||^2;
- * quad = x*^T Q_p x*. */
-int bta_last_intermediates(bta_ctx* ctx, double* ld, double* x, double* parts, double* rss, double* quad);
+ * quad = x*^T Q_p x*; ZT[a*a] = Z_T = [Q_c^-1]_{TT}. */
+int bta_last_intermediates(bta_ctx* ctx, double* ld, double* x, double* parts, double* rss, double* quad,
+                           double* ZT);
 
 int32_t bta_num_hyper(const bta_ctx* ctx);  /* d */
 int64_t bta_latent_size(const bta_ctx* ctx); /* N */

@@ -59,7 +59,7 @@ def lib():
     L.bta_solve.argtypes = [vp, _Blocks, i32, vp, i32, vp, vp]
     L.bta_selinv.argtypes = [vp, _Blocks, i32, vp, vp]
     L.inla_value_and_grad.argtypes = [vp, dp, dp, dp, dp, vp, vp]
-    L.bta_last_intermediates.argtypes = [vp, dp, dp, dp, dp, dp]
+    L.bta_last_intermediates.argtypes = [vp, dp, dp, dp, dp, dp, dp]
     L.bta_num_hyper.argtypes = [vp]
     L.bta_num_hyper.restype = C.c_int32
     L.bta_latent_size.argtypes = [vp]
@@ -219,9 +219,10 @@ class BtaModel:
         parts = np.zeros(3 * self.d)
         rss = np.zeros(self.k)
         quad = C.c_double()
+        ZT = np.zeros((self.a, self.a))
         _check(lib().bta_last_intermediates(self._h, _dptr(ld), _dptr(x) if want_x else None, _dptr(parts), _dptr(rss),
-                                            C.byref(quad)))
-        return dict(ld_p=ld[0], ld_c=ld[1], x=x, phaseA=parts[: self.d], phaseB=parts[self.d: 2 * self.d],
+                                            C.byref(quad), _dptr(ZT)))
+        return dict(ZT=ZT, ld_p=ld[0], ld_c=ld[1], x=x, phaseA=parts[: self.d], phaseB=parts[self.d: 2 * self.d],
                     phaseC=parts[2 * self.d:], rss=rss, quad_p=quad.value)
 
     def kernel_launches(self):

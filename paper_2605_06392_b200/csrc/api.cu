@@ -438,7 +438,8 @@ extern "C" int inla_value_and_grad(bta_ctx* c, const double* theta, double* f, d
   return rc;
 }
 
-extern "C" int bta_last_intermediates(bta_ctx* c, double* ld, double* x, double* parts, double* rss, double* quad) {
+extern "C" int bta_last_intermediates(bta_ctx* c, double* ld, double* x, double* parts, double* rss, double* quad,
+                                      double* ZT) {
   if (!c) return bad("bta_last_intermediates: null ctx");
   if (ld) {
     ld[0] = c->last_ld[0];
@@ -447,6 +448,10 @@ extern "C" int bta_last_intermediates(bta_ctx* c, double* ld, double* x, double*
   if (parts && !c->last_parts.empty()) memcpy(parts, c->last_parts.data(), c->last_parts.size() * sizeof(double));
   if (rss && !c->last_rss.empty()) memcpy(rss, c->last_rss.data(), c->last_rss.size() * sizeof(double));
   if (quad) *quad = c->last_quad;
+  if (ZT) {
+    SmallLayout L = small_layout(c->md);
+    BTA_CUDA_OK(cudaMemcpy(ZT, c->small + L.ZT[CH_COND], sizeof(double) * c->md.a * c->md.a, cudaMemcpyDeviceToHost));
+  }
   if (x) {
     if (!c->last_x_dev) return bad("bta_last_intermediates: no gradient has been computed yet");
     BTA_CUDA_OK(cudaMemcpy(x, c->last_x_dev, c->md.N * sizeof(double), cudaMemcpyDeviceToHost));

@@ -1,0 +1,188 @@
+"""GPU parity: the CUDA path (through the C-ABI binding) vs the CPU oracle, element by element, on the same
+seeded inputs.  Tolerances (BASELINE.json north_star): 1e-9 relative on log-determinants and f, 1e-6 per
+gradient component gated as in DESIGN.md reading R16; intermediates (factor, solve, selected inverse)
+1e-9 of the block scale."""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+from oracle import bta_oracle as O
+from workloads import draw_obs, make_config, make_model, make_w0, uniform_design
+from workloads.generate import draw_theta
+
+TOL_F, TOL_G = 1e-9, 1e-6
+
+
+def _model(model, obs):
+    from paper_2605_06392_b200 import BtaModel
+    return BtaModel.from_workload(model, obs, device=0)
+
+
+def grad_ok(g, ref):
+    gate = np.maximum(np.abs(ref), 1e-3 * np.max(np.abs(ref)))     # R16
+    return np.all(np.abs(g - ref) <= TOL_G * gate)
+
+
+CASES = {
+    "w0": lambda: make_w0(),
+    "cfg0": lambda: make_config(0),
+    "b25_ragged": lambda: (lambda m: (m, draw_obs(m, 300, 31), draw_theta(m, 31)))(make_model(5, 1, 7, 3)),
+    "b81_two_tiles": lambda: (lambda m: (m, draw_obs(m, 900, 32), draw_theta(m, 32)))(make_model(9, 1, 5, 4)),
+    "b144_h07": lambda: (lambda m: (m, draw_obs(m, 2000, 33), draw_theta(m, 33)))(make_model(12, 1, 4, 2, h=0.7)),
+    "nt1": lambda: (lambda m: (m, draw_obs(m, 100, 34), draw_theta(m, 34)))(make_model(6, 1, 1, 2)),
+    "nt2": lambda: (lambda m: (m, draw_obs(m, 100, 35), draw_theta(m, 35)))(make_model(6, 1, 2, 1)),
+    "mv_k3_tiny": lambda: (lambda m: (m, draw_obs(m, 40, 5), draw_theta(m, 5)))(make_model(3, 3, 4, 6)),
+    "mv_k2_b162": lambda: (lambda m: (m, draw_obs(m, 500, 6), draw_theta(m, 6)))(make_model(9, 2, 5, 4)),
+    "mv_k3_b300": lambda: (lambda m: (m, draw_obs(m, 700, 7), draw_theta(m, 7)))(make_model(10, 3, 6, 6)),
+    "a8": lambda: (lambda m: (m, draw_obs(m, 800, 36), draw_theta(m, 36)))(make_model(8, 1, 6, 8)),
+    "no_obs": lambda: (lambda m: (m, draw_obs(m, 0, 37), draw_theta(m, 37)))(make_model(5, 1, 4, 2)),
+    "uniform_design": lambda: (lambda m: (m, uniform_design(m, 2), draw_theta(m, 38)))(make_model(6, 1, 5, 2)),
+    "cfg1": lambda: make_config(1),
+}
+
+
+@pytest.mark.parametrize("name", list(CASES))
+def test_value_and_grad_parity(name):
+    model, obs, th = CASES[name]()
+    ref = O.value_and_grad(model, obs, th)
+    M = _model(model, obs)
+    f, g, st = M.inla_value_and_grad(th, stages=True)
+    im = M.last_intermediates()
+    n0 = M.kernel_launches()
+    f2, g2 = M.inla_value_and_grad(th)                                     # deterministic: bitwise repeatable
+    assert f2 == f and np.array_equal(g, g2)
+    assert M.kernel_launches() > n0 > 0
+    M.close()
+    assert abs(im["ld_p"] - ref["ld_p"]) <= TOL_F * abs(ref["ld_p"])
+    assert abs(im["ld_c"] - ref["ld_c"]) <= TOL_F * abs(ref["ld_c"])
+    assert abs(f - ref["f"]) <= TOL_F * abs(ref["f"])
+    assert grad_ok(g, ref["grad"]), (g, ref["grad"])
+    scale = max(np.max(np.abs(ref["x"])), 1e-30)
+    assert np.max(np.abs(im["x"] - ref["x"])) <= 1e-9 * scale
+    for key in ("phaseA", "phaseB", "phaseC"):
+        s = max(np.max(np.abs(ref[key])), 1e-30)
+        assert np.max(np.abs(im[key] - ref[key])) <= 1e-9 * s, key
+    assert np.allclose(im["rss"], ref["rss"], rtol=1e-10, atol=1e-12)
+    assert abs(im["quad_p"] - ref["quad_p"]) <= 1e-9 * max(abs(ref["quad_p"]), 1e-30)
+    assert st["total"] > 0
+
+
+def test_w0_printed_digits(golden):
+    g = golden("w0.txt")
+    model, obs, th = make_w0()
+    M = _model(model, obs)
+    f, grad = M.inla_value_and_grad(th)
+    im = M.last_intermediates()
+    M.close()
+    assert abs(f - g["f"][0]) <= TOL_F * abs(g["f"][0])
+    assert np.all(np.abs(grad - np.array(g["grad"])) <= TOL_G * np.abs(g["grad"]))
+    assert abs(im["ld_c"] - g["ld_c"][0]) <= TOL_F * g["ld_c"][0]
+    assert abs(im["ld_p"] - g["ld_p"][0]) <= TOL_F * g["ld_p"][0]
+
+
+OP_CASES = ["cfg0", "b81_two_tiles", "mv_k3_tiny", "mv_k2_b162", "b144_h07"]
+
+
+def _stack(lst):
+    return np.stack(lst) if len(lst) else np.zeros((0,) + (1, 1))
+
+
+@pytest.mark.parametrize("name", OP_CASES)
+@pytest.mark.parametrize("which", [0, 1])
+def test_assemble_factor_solve_selinv_parity(name, which):
+    import torch
+    model, obs, th = CASES[name]()
+    agg = O.aggregates(model, obs)
+    ref = O.assemble(model, agg, th, "cond" if which else "prior")
+    b, nt, a, N = model.b, model.nt, model.a, model.N
+    M = _model(model, obs)
+    blk = M.alloc_blocks()
+    M.bta_assemble(th, which, blk)
+    D = blk.D.cpu().numpy()
+    for t in range(nt):
+        assert np.max(np.abs(D[t] - np.tril(ref.D[t]))) <= 1e-13 * np.max(np.abs(ref.D[t]))   # strict upper zero
+    if nt > 1:
+        assert np.max(np.abs(blk.B.cpu().numpy() - np.stack(ref.B))) <= 1e-13 * np.max(np.abs(np.stack(ref.B)))
+    assert np.allclose(blk.C.cpu().numpy(), np.stack(ref.C), rtol=1e-13, atol=1e-15)
+    assert np.allclose(blk.T.cpu().numpy(), ref.T, rtol=1e-13, atol=1e-15)
+    if which:
+        assert np.allclose(blk.rhs.cpu().numpy(), ref.r, rtol=1e-13, atol=1e-15)
+    # ---- factor + logdet (Algorithm 1); factor kept as X = L_D^-1, L_B, L_C, L_T
+    F = O.factor_forward(O.Blocks(ref.D, ref.B, ref.C, ref.T, None))
+    diagL = torch.empty(N, dtype=torch.float64, device=blk.D.device)
+    ld = M.bta_factor_logdet(blk, which, diagL=diagL)
+    assert abs(ld - F.logdet) <= TOL_F * abs(F.logdet)
+    X = blk.D.cpu().numpy()
+    dl = diagL.cpu().numpy()
+    for t in range(nt):
+        Xref = np.linalg.inv(F.LD[t])
+        assert np.max(np.abs(X[t] - Xref)) <= 1e-9 * np.max(np.abs(Xref))
+        assert np.allclose(dl[t * b:(t + 1) * b], np.diag(F.LD[t]), rtol=1e-11)
+    assert np.allclose(dl[nt * b:], np.diag(F.LT), rtol=1e-11)
+    LB = blk.B.cpu().numpy()
+    for t in range(nt - 1):
+        assert np.max(np.abs(LB[t] - F.LB[t])) <= 1e-9 * max(np.max(np.abs(F.LB[t])), 1e-30)
+    if which:
+        assert np.max(np.abs(blk.C.cpu().numpy() - np.stack(F.LC))) <= 1e-9 * np.max(np.abs(np.stack(F.LC)))
+    assert np.max(np.abs(blk.T.cpu().numpy() - F.LT)) <= 1e-9 * np.max(np.abs(F.LT))
+    # ---- solve with 1, 3 and 11 right-hand sides (two chunks)
+    for nrhs in (1, 3, 11):
+        rhs = np.cos(0.37 * np.arange(nrhs * N)).reshape(nrhs, N) + 0.1
+        xr = np.stack([O.solve(ref, rhs[r]) for r in range(nrhs)])
+        rd = torch.tensor(rhs, device=blk.D.device)
+        M.bta_solve(blk, which, rd)
+        assert np.max(np.abs(rd.cpu().numpy() - xr)) <= 1e-9 * np.max(np.abs(xr))
+    # ---- selected inversion in place
+    Z = O.selinv(F)
+    M.bta_selinv(blk, which)
+    ZD = blk.D.cpu().numpy()
+    sc = max(np.max(np.abs(z)) for z in Z.ZD)
+    for t in range(nt):
+        assert np.max(np.abs(ZD[t] - Z.ZD[t])) <= 1e-9 * sc
+    ZB = blk.B.cpu().numpy()
+    for t in range(nt - 1):
+        assert np.max(np.abs(ZB[t] - Z.ZB[t])) <= 1e-9 * sc
+    if which:
+        assert np.max(np.abs(blk.C.cpu().numpy() - np.stack(Z.ZC))) <= 1e-9 * sc
+    assert np.max(np.abs(blk.T.cpu().numpy() - Z.ZT)) <= 1e-9 * np.max(np.abs(Z.ZT))
+    M.close()
+
+
+def test_not_spd_is_reported():
+    import torch
+    from paper_2605_06392_b200 import BtaError
+    model, obs, th = make_config(0)
+    M = _model(model, obs)
+    blk = M.alloc_blocks()
+    M.bta_assemble(th, 1, blk)
+    blk.D[2, 5, 5] = -1.0                       # global row 2*16 + 5 + 1 = 38 (1-based)
+    with pytest.raises(BtaError) as ei:
+        M.bta_factor_logdet(blk, 1)
+    assert ei.value.code == 4 and M.last_pivot() == 38
+    M.close()
+
+
+def test_gemm_kernel_modes():
+    import torch
+    from paper_2605_06392_b200 import gemm
+    rng = np.random.default_rng(0)
+    for (Mm, Nn, Kk) in [(64, 64, 64), (100, 52, 37), (129, 257, 75), (27, 27, 27), (400, 400, 400)]:
+        for mode in (0, 1, 2):
+            A = rng.standard_normal((Mm, Kk) if mode != 2 else (Kk, Mm))
+            B = rng.standard_normal((Kk, Nn) if mode != 1 else (Nn, Kk))
+            C0 = rng.standard_normal((Mm, Nn))
+            ref = -1.5 * (A if mode != 2 else A.T) @ (B if mode != 1 else B.T) + 0.5 * C0
+            Cd = torch.tensor(C0, device="cuda")
+            gemm(mode, torch.tensor(A, device="cuda"), torch.tensor(B, device="cuda"), Cd, alpha=-1.5, beta=0.5)
+            assert np.max(np.abs(Cd.cpu().numpy() - ref)) <= 1e-12 * Kk
+    n = 320
+    L = np.tril(rng.standard_normal((n, n)))
+    Bm = rng.standard_normal((n, n))
+    t = lambda x: torch.tensor(x, device="cuda")
+    z = lambda: torch.zeros(n, n, dtype=torch.float64, device="cuda")
+    assert np.max(np.abs(gemm(1, t(Bm), t(L), z(), khi=1).cpu().numpy() - Bm @ L.T)) < 1e-11
+    assert np.max(np.abs(gemm(0, t(Bm), t(L), z(), klo=1).cpu().numpy() - Bm @ L)) < 1e-11
+    assert np.max(np.abs(gemm(0, t(L), t(Bm), z(), khi=2).cpu().numpy() - L @ Bm)) < 1e-11
+    assert np.max(np.abs(gemm(2, t(L), t(L), z(), klo=2, out=2).cpu().numpy() - L.T @ L)) < 1e-11
+    assert np.max(np.abs(gemm(1, t(Bm), t(Bm), z(), out=1).cpu().numpy() - np.tril(Bm @ Bm.T))) < 1e-11
