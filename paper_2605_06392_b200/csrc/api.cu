@@ -358,19 +358,6 @@ extern "C" int inla_value_and_grad(bta_ctx* c, const double* theta, double* f, d
   cc.xout = wc.x;
   cc.ld_x = md.N;
 
-  BTA_CUDA_OK(launch_assemble(c, BTA_COND, cc.D, bb, cc.Bin, bb, wc.Rin, cc.rin_stride, wc.T, md.a,
-                              wc.Rin + (long long)md.a * md.b, cc.rin_stride, wc.rtip, 1, s0));
-  BTA_CUDA_OK(cudaEventRecord(ev[1], s0));
-  BTA_CUDA_OK(chain_forward(cc, s0));
-  BTA_CUDA_OK(launch_logdet_partial(c, CH_COND, wc.dvec, s0));
-  BTA_CUDA_OK(cudaEventRecord(ev[2], s0));
-  BTA_CUDA_OK(chain_backward(cc, s0));
-  BTA_CUDA_OK(cudaMemcpyAsync(wc.x + (long long)md.nt * md.b, cc.xT, md.a * sizeof(double), cudaMemcpyDeviceToDevice,
-                              s0));
-  BTA_CUDA_OK(launch_quad_stencil(c, wc.x, s0));
-  BTA_CUDA_OK(launch_residual(c, wc.x, s0));
-  BTA_CUDA_OK(cudaEventRecord(ev[3], s0));
-
   // ---- Q_p chain (Phase C) on the side stream ----
   Chain cp;
   cp.c = c;
@@ -394,13 +381,37 @@ extern "C" int inla_value_and_grad(bta_ctx* c, const double* theta, double* f, d
   cp.Tt = c->small + L.Tt[CH_PRIOR];
   cp.LT = c->small + L.LT[CH_PRIOR];
   cp.ZT = c->small + L.ZT[CH_PRIOR];
+
+  // The two chains are independent (they meet only in the scalar assembly).  Their launches are interleaved
+  // block by block from this one host thread so that both streams always have work queued: the latency-bound
+  // parts of one chain (POTRF leaves, skinny kernels) overlap the GEMMs of the other.
+  BTA_CUDA_OK(launch_assemble(c, BTA_COND, cc.D, bb, cc.Bin, bb, wc.Rin, cc.rin_stride, wc.T, md.a,
+                              wc.Rin + (long long)md.a * md.b, cc.rin_stride, wc.rtip, 1, s0));
+  BTA_CUDA_OK(cudaEventRecord(ev[1], s0));
   BTA_CUDA_OK(cudaEventRecord(ev[4], s1));
   BTA_CUDA_OK(launch_assemble(c, BTA_PRIOR, cp.D, bb, cp.Bin, bb, nullptr, 0, wp.T, md.a, nullptr, 0, nullptr, 0, s1));
   BTA_CUDA_OK(cudaEventRecord(ev[5], s1));
-  BTA_CUDA_OK(chain_forward(cp, s1));
+  BTA_CUDA_OK(chain_forward_begin(cc, s0));
+  BTA_CUDA_OK(chain_forward_begin(cp, s1));
+  for (int t = 0; t < md.nt; ++t) {
+    BTA_CUDA_OK(chain_forward_step(cc, t, s0));
+    BTA_CUDA_OK(chain_forward_step(cp, t, s1));
+  }
+  BTA_CUDA_OK(chain_forward_end(cc, s0));
+  BTA_CUDA_OK(launch_logdet_partial(c, CH_COND, wc.dvec, s0));
+  BTA_CUDA_OK(cudaEventRecord(ev[2], s0));
+  BTA_CUDA_OK(chain_forward_end(cp, s1));
   BTA_CUDA_OK(launch_logdet_partial(c, CH_PRIOR, wp.dvec, s1));
   BTA_CUDA_OK(cudaEventRecord(ev[6], s1));
-  BTA_CUDA_OK(chain_backward(cp, s1));
+  for (int t = md.nt - 1; t >= 0; --t) {
+    BTA_CUDA_OK(chain_backward_step(cc, t, s0));
+    BTA_CUDA_OK(chain_backward_step(cp, t, s1));
+  }
+  BTA_CUDA_OK(cudaMemcpyAsync(wc.x + (long long)md.nt * md.b, cc.xT, md.a * sizeof(double), cudaMemcpyDeviceToDevice,
+                              s0));
+  BTA_CUDA_OK(launch_quad_stencil(c, wc.x, s0));
+  BTA_CUDA_OK(launch_residual(c, wc.x, s0));
+  BTA_CUDA_OK(cudaEventRecord(ev[3], s0));
   BTA_CUDA_OK(cudaEventRecord(ev[7], s1));
   if (!serial) BTA_CUDA_OK(cudaStreamWaitEvent(s0, ev[7], 0));
 

@@ -9,59 +9,81 @@
 
 namespace {
 
-constexpr int NB = 64;
-constexpr int LDW = NB + 1;
-
-__global__ void __launch_bounds__(256) potrf_inv_tile_kernel(double* __restrict__ A, int ld, int n,
-                                                             double* __restrict__ diagL, long long grow0,
-                                                             unsigned long long* __restrict__ pivot_flag) {
-  __shared__ double W[NB * LDW];
-  __shared__ double lcol[NB], xrow[NB];
-  const int tid = threadIdx.x;
-  for (int e = tid; e < NB * NB; e += 256) {
-    int i = e / NB, j = e % NB;
-    double v = (i == j) ? 1.0 : 0.0;
-    if (i < n && j <= i) v = A[(long long)i * ld + j];
-    W[i * LDW + j] = v;
-  }
-  __syncthreads();
-  const int ti = tid >> 2, tq = tid & 3;
+// NB x NB leaf, NW warps.  Warp w owns rows w, w+NW, ...; lane l owns columns l, l+32, ...: the whole working
+// array lives in registers (NB*NB / (32*NW) = 16 doubles per thread).  Per elimination step k the only shared
+// data are column k (rows >= k) and row k (columns < k) of the array as they stood after step k-1; their owners
+// publish them (double-buffered) at the end of step k-1, so one __syncthreads per step suffices, and every
+// thread derives 1/sqrt(pivot) itself.
+template <int NB, int NW>
+__global__ void __launch_bounds__(32 * NW) potrf_inv_tile_kernel(double* __restrict__ A, int ld, int n,
+                                                                 double* __restrict__ diagL, long long grow0,
+                                                                 unsigned long long* __restrict__ pivot_flag) {
+  constexpr int R = NB / NW, CC = NB / 32;
+  __shared__ double colraw[2][NB], rowraw[2][NB];
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  double w[R][CC];
+#pragma unroll
+  for (int r = 0; r < R; ++r)
+#pragma unroll
+    for (int c = 0; c < CC; ++c) {
+      const int i = warp + NW * r, j = lane + 32 * c;
+      double v = (i == j) ? 1.0 : 0.0;
+      if (i < n && j <= i) v = A[(long long)i * ld + j];
+      w[r][c] = v;
+      if (j == 0) colraw[0][i] = v;
+    }
   for (int k = 0; k < n; ++k) {
-    double piv = W[k * LDW + k];
+    __syncthreads();
+    const double* cr = colraw[k & 1];
+    const double* rr = rowraw[k & 1];
+    double piv = cr[k];
     if (!(piv > 0.0)) {  // also catches NaN
       if (tid == 0) atomicMin(pivot_flag, (unsigned long long)(grow0 + k + 1));
       piv = 1.0;
     }
-    const double d = sqrt(piv), rd = 1.0 / d;
-    if (tid < NB) {
-      if (tid > k) lcol[tid] = W[tid * LDW + k] * rd;
-    } else if (tid < 2 * NB) {
-      int j = tid - NB;
-      if (j < k) xrow[j] = W[k * LDW + j] * rd;
-      if (j == k) xrow[j] = rd;
+    const double rs = rsqrt(piv);
+    if (tid == 0 && diagL) diagL[k] = piv * rs;
+    double cv[CC];
+#pragma unroll
+    for (int c = 0; c < CC; ++c) {
+      const int j = lane + 32 * c;
+      cv[c] = ((j < k) ? rr[j] : cr[j]) * rs;
     }
-    if (tid == 0 && diagL) diagL[k] = d;
-    __syncthreads();
-    if (ti > k) {
-      const double li = lcol[ti];
-      double* w = W + ti * LDW;
-      for (int j = tq; j <= ti; j += 4) {
-        if (j < k)
-          w[j] -= li * xrow[j];
-        else if (j == k)
-          w[j] = -li * xrow[k];
-        else
-          w[j] -= li * lcol[j];
+    const int k1 = k + 1;
+    double* crn = colraw[k1 & 1];
+    double* rrn = rowraw[k1 & 1];
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+      const int i = warp + NW * r;
+      if (i > k) {
+        const double li = cr[i] * rs;
+#pragma unroll
+        for (int c = 0; c < CC; ++c) {
+          const int j = lane + 32 * c;
+          if (j <= i) {
+            const double v = (j == k) ? -li * rs : fma(-li, cv[c], w[r][c]);
+            w[r][c] = v;
+            if (j == k1) crn[i] = v;
+            if (i == k1 && j < k1) rrn[j] = v;
+          }
+        }
+      } else if (i == k) {
+#pragma unroll
+        for (int c = 0; c < CC; ++c) {
+          const int j = lane + 32 * c;
+          if (j < k) w[r][c] = cv[c];
+          if (j == k) w[r][c] = rs;
+        }
       }
-    } else if (ti == k) {
-      for (int j = tq; j <= k; j += 4) W[k * LDW + j] = xrow[j];
     }
-    __syncthreads();
   }
-  for (int e = tid; e < n * n; e += 256) {
-    int i = e / n, j = e % n;
-    A[(long long)i * ld + j] = (j <= i) ? W[i * LDW + j] : 0.0;
-  }
+#pragma unroll
+  for (int r = 0; r < R; ++r)
+#pragma unroll
+    for (int c = 0; c < CC; ++c) {
+      const int i = warp + NW * r, j = lane + 32 * c;
+      if (i < n && j < n) A[(long long)i * ld + j] = (j <= i) ? w[r][c] : 0.0;
+    }
 }
 
 // Arrow tip (Algorithm 1 line 11, Eq. 3, and Z_T = L_T^-T L_T^-1 of the selected inversion, R10).
@@ -162,7 +184,12 @@ __global__ void tip_inverse_kernel(const double* __restrict__ LT, int a, double*
 
 cudaError_t launch_potrf_inv_tile(double* A, int ld, int n, double* diagL, long long grow0,
                                   unsigned long long* pivot_flag, cudaStream_t st) {
-  potrf_inv_tile_kernel<<<1, 256, 0, st>>>(A, ld, n, diagL, grow0, pivot_flag);
+  if (n <= 64)
+    potrf_inv_tile_kernel<64, 8><<<1, 256, 0, st>>>(A, ld, n, diagL, grow0, pivot_flag);
+  else if (n <= 128)
+    potrf_inv_tile_kernel<128, 32><<<1, 1024, 0, st>>>(A, ld, n, diagL, grow0, pivot_flag);
+  else
+    return cudaErrorInvalidValue;
   return cudaGetLastError();
 }
 

@@ -4,6 +4,8 @@
 //   backward: Eqs. 3-5 + BTA selected inversion (R10) + the Eq. 7
 //             trace contractions fused per block (only Z_Dt and Z_D{t+1} are live).
 // The factor is held in inverse-diagonal form X_t = L_Dt^-1, so every large step is a GEMM (gemm.cu).
+#include <cstdlib>
+
 #include "sweep.h"
 
 #define CK(call)                      \
@@ -26,13 +28,17 @@ cudaError_t potrf_inv(bta_ctx* c, double* A, int ld, int lo, int hi, double* T1,
                       long long grow0, cudaStream_t st) {
   const int n = hi - lo;
   if (n <= 0) return cudaSuccess;
-  if (n <= 64) {
+  static const int LEAF = [] {
+    const char* e = getenv("BTA_LEAF");
+    return (e && atoi(e) == 64) ? 64 : 128;
+  }();
+  if (n <= LEAF) {
     BTA_COUNT(c);
     return launch_potrf_inv_tile(A + (long long)lo * ld + lo, ld, n, diagL ? diagL + lo : nullptr, grow0 + lo,
                                  c->pivot_flag, st);
   }
-  const int ntile = (n + 63) / 64;
-  const int mid = lo + 64 * ((ntile + 1) / 2);
+  const int ntile = (n + LEAF - 1) / LEAF;
+  const int mid = lo + LEAF * ((ntile + 1) / 2);
   const int s1 = mid - lo, s2 = hi - mid;
   CK(potrf_inv(c, A, ld, lo, mid, T1, T2, diagL, grow0, st));
   double* A11 = A + (long long)lo * ld + lo;
@@ -63,15 +69,21 @@ __global__ void scale_copy_kernel(long long n, double alpha, const double* __res
 }
 }  // namespace
 
-cudaError_t chain_forward(Chain& ch, cudaStream_t st) {
+cudaError_t chain_forward_begin(Chain& ch, cudaStream_t st) {
   bta_ctx* c = ch.c;
-  const int b = ch.b, nt = ch.nt, a = ch.a, P = ch.P(), ldt = a + ch.nr;
-  const long long bb = (long long)b * b;
+  const int a = ch.a, ldt = a + ch.nr;
   if (a > 0) {
     tip_init_kernel<<<1, a * ldt, 0, st>>>(a, ch.nr, ch.T, ch.ldT, ch.rhs_tip, ch.rhs_tip_stride, ch.Tt);
     BTA_COUNT(c);
   }
-  for (int t = 0; t < nt; ++t) {
+  return cudaGetLastError();
+}
+
+cudaError_t chain_forward_step(Chain& ch, int t, cudaStream_t st) {
+  bta_ctx* c = ch.c;
+  const int b = ch.b, nt = ch.nt, a = ch.a, P = ch.P(), ldt = a + ch.nr;
+  const long long bb = (long long)b * b;
+  {
     double* Dt = ch.D + t * ch.d_stride;
     if (ch.zero_upper && ch.factor_blocks) {
       CK(launch_zero_upper(Dt, b, b, st));
@@ -126,6 +138,12 @@ cudaError_t chain_forward(Chain& ch, cudaStream_t st) {
       if (dst != Bo) CK(cudaMemcpyAsync(Bo, dst, bb * sizeof(double), cudaMemcpyDeviceToDevice, st));
     }
   }
+  return cudaSuccess;
+}
+
+cudaError_t chain_forward_end(Chain& ch, cudaStream_t st) {
+  bta_ctx* c = ch.c;
+  const int b = ch.b, nt = ch.nt, a = ch.a;
   if (a > 0) {
     CK(launch_tip(ch.Tt, a, ch.nr, ch.tip_chol ? 1 : 0, ch.LT, ch.zT, ch.xT, ch.ZT,
                   ch.dvec ? ch.dvec + (long long)nt * b : nullptr, (long long)nt * b, c->pivot_flag, st));
@@ -134,15 +152,21 @@ cudaError_t chain_forward(Chain& ch, cudaStream_t st) {
   return cudaSuccess;
 }
 
+cudaError_t chain_forward(Chain& ch, cudaStream_t st) {
+  CK(chain_forward_begin(ch, st));
+  for (int t = 0; t < ch.nt; ++t) CK(chain_forward_step(ch, t, st));
+  return chain_forward_end(ch, st);
+}
+
 // Backward sweep t = nt-1 .. 0.  Needs from the forward sweep: X_t in D(t), L_Bt in Bout(t), the arrow factor
 // rows L_Ct, z_t (rows a.. of Rout(t) when arrow_rows, else rows 0..), and the tip outputs x_T, Z_T.
-cudaError_t chain_backward(Chain& ch, cudaStream_t st) {
+cudaError_t chain_backward_step(Chain& ch, int t, cudaStream_t st) {
   bta_ctx* c = ch.c;
   const int b = ch.b, nt = ch.nt, a = ch.a, nr = ch.nr;
   const long long bb = (long long)b * b;
   const bool arrow = ch.arrow();
   const int zrow0 = ch.arrow_rows ? a : 0;  // first rhs row inside the Rout stack
-  for (int t = nt - 1; t >= 0; --t) {
+  {
     const double* X = ch.D + t * ch.d_stride;
     double* LB = (t < nt - 1) ? ch.Bout + t * ch.b_stride : nullptr;
     const double* LC = nullptr;
@@ -175,7 +199,7 @@ cudaError_t chain_backward(Chain& ch, cudaStream_t st) {
                           ch.part, st));
       c->launches += 2;
     }
-    if (!ch.selinv) continue;
+    if (!ch.selinv) return cudaSuccess;
     // ---- selected inversion (R10), tensor-friendly form:  G = L_B X,  E = L_C X,
     //      Z_B = -Z_D{t+1} G - Z_C{t+1}^T E,  Z_C = -Z_C{t+1} G - Z_T E,  Z_D = X^T X - Z_B^T G - Z_C^T E
     double* ZDcur = (t & 1) ? ch.W2 : ch.W3;
@@ -235,5 +259,10 @@ cudaError_t chain_backward(Chain& ch, cudaStream_t st) {
                            cudaMemcpyDeviceToDevice, st));
     }
   }
+  return cudaSuccess;
+}
+
+cudaError_t chain_backward(Chain& ch, cudaStream_t st) {
+  for (int t = ch.nt - 1; t >= 0; --t) CK(chain_backward_step(ch, t, st));
   return cudaSuccess;
 }

@@ -43,4 +43,8 @@ struct Chain {
 cudaError_t potrf_inv(bta_ctx* c, double* A, int ld, int lo, int hi, double* T1, double* T2, double* diagL,
                       long long grow0, cudaStream_t st);
 cudaError_t chain_forward(Chain& ch, cudaStream_t st);
+cudaError_t chain_forward_begin(Chain& ch, cudaStream_t st);
+cudaError_t chain_forward_step(Chain& ch, int t, cudaStream_t st);
+cudaError_t chain_forward_end(Chain& ch, cudaStream_t st);
+cudaError_t chain_backward_step(Chain& ch, int t, cudaStream_t st);
 cudaError_t chain_backward(Chain& ch, cudaStream_t st);
