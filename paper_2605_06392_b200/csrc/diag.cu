@@ -9,17 +9,109 @@
 
 namespace {
 
-// NB x NB leaf, NW warps.  Warp w owns rows w, w+NW, ...; lane l owns columns l, l+32, ...: the whole working
-// array lives in registers (NB*NB / (32*NW) = 16 doubles per thread).  Per elimination step k the only shared
-// data are column k (rows >= k) and row k (columns < k) of the array as they stood after step k-1; their owners
-// publish them (double-buffered) at the end of step k-1, so one __syncthreads per step suffices, and every
-// thread derives 1/sqrt(pivot) itself.
+// NB x NB leaf, NW warps.  Warp w owns rows w, w+NW, ... (register slot r = row / NW); lane l owns columns l,
+// l+32, ... (slot c = col / 32): the whole working array lives in registers.  Elimination step k: the owners of
+// column k, row k and the pivot publish them (double-buffered shared vectors) together with 1/sqrt(pivot); one
+// __syncthreads; then every thread updates its registers with bare DFMAs.  The steps are generated in blocks of
+// NW consecutive k (template parameter BLK) so that the register slots of column k and row k are compile-time
+// constants and the per-step instruction count stays small.
+template <int NB, int NW>
+struct LeafSmem {
+  double colraw[2][NB], rowraw[2][NB], rsq[2];
+};
+
+template <int NB, int NW, int BLK>
+__device__ __forceinline__ bool leaf_steps(double (&w)[NB / NW][NB / 32], LeafSmem<NB, NW>& sm, int n, int lane,
+                                           int warp, double* __restrict__ diagL, long long grow0,
+                                           unsigned long long* __restrict__ pivot_flag) {
+  constexpr int R = NB / NW, CC = NB / 32;
+  constexpr int K0 = BLK * NW, KC = K0 / 32, KR = BLK, L0 = K0 % 32;
+#pragma unroll 1
+  for (int q = 0; q < NW; ++q) {
+    const int k = K0 + q, kl = L0 + q, buf = q & 1;
+    if (k >= n) return false;
+    if (lane == kl) {
+#pragma unroll
+      for (int r = KR; r < R; ++r) sm.colraw[buf][warp + NW * r] = w[r][KC];
+    }
+    if (warp == q) {
+#pragma unroll
+      for (int c = 0; c <= KC; ++c) sm.rowraw[buf][lane + 32 * c] = w[KR][c];
+      if (lane == kl) {
+        double piv = w[KR][KC];
+        if (!(piv > 0.0)) {  // also catches NaN
+          atomicMin(pivot_flag, (unsigned long long)(grow0 + k + 1));
+          piv = 1.0;
+        }
+        const double rsn = rsqrt(piv);
+        sm.rsq[buf] = rsn;
+        if (diagL) diagL[k] = piv * rsn;
+      }
+    }
+    __syncthreads();
+    const double* cr = sm.colraw[buf];
+    const double* rr = sm.rowraw[buf];
+    const double rs = sm.rsq[buf];
+    double cv[CC];
+#pragma unroll
+    for (int c = 0; c < CC; ++c) {
+      const int j = lane + 32 * c;
+      if (c < KC)
+        cv[c] = rr[j] * rs;
+      else if (c > KC)
+        cv[c] = cr[j] * rs;
+      else
+        cv[c] = (lane < kl ? rr[j] : cr[j]) * rs;
+    }
+    if (lane == kl) {  // column k restarts: X[i][k] = -l_ik / l_kk for i > k, X[k][k] = 1 / l_kk
+      cv[KC] = rs;
+#pragma unroll
+      for (int r = KR; r < R; ++r) w[r][KC] = 0.0;
+    }
+#pragma unroll
+    for (int r = KR; r < R; ++r) {
+      constexpr int dummy = 0;
+      (void)dummy;
+      const int i = warp + NW * r;
+      // columns beyond the diagonal slot of this row are never read: skip them
+      const int cmax = (NW * r + NW - 1) / 32;
+      if (r > KR || warp > q) {
+        const double nli = -cr[i] * rs;
+#pragma unroll
+        for (int c = 0; c < CC; ++c)
+          if (c <= cmax) w[r][c] = fma(nli, cv[c], w[r][c]);
+      } else if (warp == q) {
+#pragma unroll
+        for (int c = 0; c <= KC; ++c)
+          if (lane + 32 * c <= k) w[r][c] = cv[c];
+      }
+    }
+  }
+  return true;
+}
+
+template <int NB, int NW, int BLK>
+struct LeafRun {
+  static __device__ __forceinline__ void run(double (&w)[NB / NW][NB / 32], LeafSmem<NB, NW>& sm, int n, int lane,
+                                             int warp, double* diagL, long long grow0,
+                                             unsigned long long* pivot_flag) {
+    if (leaf_steps<NB, NW, BLK>(w, sm, n, lane, warp, diagL, grow0, pivot_flag))
+      LeafRun<NB, NW, BLK + 1>::run(w, sm, n, lane, warp, diagL, grow0, pivot_flag);
+  }
+};
+template <int NB, int NW>
+struct LeafRun<NB, NW, NB / NW> {
+  static __device__ __forceinline__ void run(double (&)[NB / NW][NB / 32], LeafSmem<NB, NW>&, int, int, int, double*,
+                                             long long, unsigned long long*) {}
+};
+
 template <int NB, int NW>
 __global__ void __launch_bounds__(32 * NW) potrf_inv_tile_kernel(double* __restrict__ A, int ld, int n,
                                                                  double* __restrict__ diagL, long long grow0,
                                                                  unsigned long long* __restrict__ pivot_flag) {
   constexpr int R = NB / NW, CC = NB / 32;
-  __shared__ double colraw[2][NB], rowraw[2][NB];
+  static_assert(NW % 2 == 0 && 32 % NW == 0, "steps alternate the two shared buffers inside a block of NW");
+  __shared__ LeafSmem<NB, NW> sm;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   double w[R][CC];
 #pragma unroll
@@ -30,53 +122,8 @@ __global__ void __launch_bounds__(32 * NW) potrf_inv_tile_kernel(double* __restr
       double v = (i == j) ? 1.0 : 0.0;
       if (i < n && j <= i) v = A[(long long)i * ld + j];
       w[r][c] = v;
-      if (j == 0) colraw[0][i] = v;
     }
-  for (int k = 0; k < n; ++k) {
-    __syncthreads();
-    const double* cr = colraw[k & 1];
-    const double* rr = rowraw[k & 1];
-    double piv = cr[k];
-    if (!(piv > 0.0)) {  // also catches NaN
-      if (tid == 0) atomicMin(pivot_flag, (unsigned long long)(grow0 + k + 1));
-      piv = 1.0;
-    }
-    const double rs = rsqrt(piv);
-    if (tid == 0 && diagL) diagL[k] = piv * rs;
-    double cv[CC];
-#pragma unroll
-    for (int c = 0; c < CC; ++c) {
-      const int j = lane + 32 * c;
-      cv[c] = ((j < k) ? rr[j] : cr[j]) * rs;
-    }
-    const int k1 = k + 1;
-    double* crn = colraw[k1 & 1];
-    double* rrn = rowraw[k1 & 1];
-#pragma unroll
-    for (int r = 0; r < R; ++r) {
-      const int i = warp + NW * r;
-      if (i > k) {
-        const double li = cr[i] * rs;
-#pragma unroll
-        for (int c = 0; c < CC; ++c) {
-          const int j = lane + 32 * c;
-          if (j <= i) {
-            const double v = (j == k) ? -li * rs : fma(-li, cv[c], w[r][c]);
-            w[r][c] = v;
-            if (j == k1) crn[i] = v;
-            if (i == k1 && j < k1) rrn[j] = v;
-          }
-        }
-      } else if (i == k) {
-#pragma unroll
-        for (int c = 0; c < CC; ++c) {
-          const int j = lane + 32 * c;
-          if (j < k) w[r][c] = cv[c];
-          if (j == k) w[r][c] = rs;
-        }
-      }
-    }
-  }
+  LeafRun<NB, NW, 0>::run(w, sm, n, lane, warp, diagL, grow0, pivot_flag);
 #pragma unroll
   for (int r = 0; r < R; ++r)
 #pragma unroll
@@ -187,7 +234,7 @@ cudaError_t launch_potrf_inv_tile(double* A, int ld, int n, double* diagL, long 
   if (n <= 64)
     potrf_inv_tile_kernel<64, 8><<<1, 256, 0, st>>>(A, ld, n, diagL, grow0, pivot_flag);
   else if (n <= 128)
-    potrf_inv_tile_kernel<128, 32><<<1, 1024, 0, st>>>(A, ld, n, diagL, grow0, pivot_flag);
+    potrf_inv_tile_kernel<128, 16><<<1, 512, 0, st>>>(A, ld, n, diagL, grow0, pivot_flag);
   else
     return cudaErrorInvalidValue;
   return cudaGetLastError();
