@@ -17,7 +17,7 @@ extern "C" int bta_gemm(int mode, int M, int N, int K, double alpha, const doubl
     bta_set_error("bta_gemm: bad mode or size");
     return BTA_ERR_ARG;
   }
-  GemmArgs g{A, B, C, M, N, K, lda, ldb, ldc, alpha, beta, mode, klo, khi, out, nullptr, 0};
+  GemmArgs g{A, B, C, M, N, K, lda, ldb, ldc, alpha, beta, mode, klo, khi, out, nullptr, 0, 0};
   BTA_CUDA_OK(launch_gemm(g, (cudaStream_t)stream));
   return BTA_OK;
 }

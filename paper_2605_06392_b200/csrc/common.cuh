@@ -60,6 +60,7 @@ struct GemmArgs {
   int mode, klo, khi, out;
   const GemmSub* subs;  // device array (nsub problems; M,N,K above = maxima for the grid) or nullptr
   int nsub;
+  int dbg;              // diagnostics only (0 in production): 1 = no loads in the main loop, 2 = no barriers
 };
 
 cudaError_t launch_gemm(const GemmArgs& g, cudaStream_t st);

@@ -7,11 +7,12 @@
 // 64-bit fragment loads are bank-conflict-free (leading dimension = 4 mod 16 doubles); accumulators live
 // in registers.  Triangular operands are exploited by restricting the k-range per output tile
 // (KLO_*/KHI_*), symmetric outputs by computing the lower tiles only (OUT_LOWER*).
+#include <cstdlib>
+
 #include "common.cuh"
 
 namespace {
 
-constexpr int BK = 16;
 constexpr int STAGES = 3;
 constexpr int KPAD = 4;  // leading dimensions are == 4 (mod 16) doubles
 
@@ -38,7 +39,7 @@ __device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double
 // One operand tile (ROWS rows of the output dimension x BK of k) -> shared memory.
 //  KM = false: global is [row][k] (k contiguous); smem [ROWS][BK+KPAD]
 //  KM = true : global is [k][row] (row contiguous); smem [BK][ROWS+KPAD]
-template <int ROWS, bool KM, int NT>
+template <int ROWS, bool KM, int NT, int BK>
 __device__ __forceinline__ void load_tile(double* sm, const double* __restrict__ g, int ld, int row0, int nrows,
                                           int k0, int kend, bool vec, int tid) {
   constexpr int CHUNKS = ROWS * BK / 2;
@@ -72,7 +73,39 @@ __device__ __forceinline__ void load_tile(double* sm, const double* __restrict__
   }
 }
 
-template <int BM, int BN, int WM, int WN, bool A_KM, bool B_KM>
+// Fast path of load_tile for a tile that lies fully inside the matrix with a full BK of k and 16-byte
+// alignment: one running global pointer per operand, constant strides, no predicates.
+//  KM = false: thread's chunk i sits at row (tid / (BK/2)) + i * (NT / (BK/2)), k = (tid % (BK/2)) * 2
+//  KM = true : chunk i sits at k = tid / (ROWS/2) + i * (NT / (ROWS/2)), row = (tid % (ROWS/2)) * 2
+template <int ROWS, bool KM, int NT, int BK>
+__device__ __forceinline__ void load_tile_fast(double* sm_thread, const double* __restrict__ g_thread, long long ld) {
+  constexpr int CHUNKS = ROWS * BK / 2;
+  static_assert(CHUNKS % NT == 0, "tile chunks must divide evenly over the CTA");
+  constexpr int PER = CHUNKS / NT;
+  if (!KM) {
+    static_assert(NT % (BK / 2) == 0, "row stride");
+    constexpr int RSTEP = NT / (BK / 2);
+#pragma unroll
+    for (int i = 0; i < PER; ++i)
+      cp_async16(sm_thread + i * RSTEP * (BK + KPAD), g_thread + (long long)i * RSTEP * ld, 16);
+  } else {
+    static_assert(NT % (ROWS / 2) == 0 || (ROWS / 2) % NT == 0, "k stride");
+    if (NT >= ROWS / 2) {
+      constexpr int KSTEP = NT / (ROWS / 2) > 0 ? NT / (ROWS / 2) : 1;
+#pragma unroll
+      for (int i = 0; i < PER; ++i)
+        cp_async16(sm_thread + i * KSTEP * (ROWS + KPAD), g_thread + (long long)i * KSTEP * ld, 16);
+    } else {
+      constexpr int SPLIT = (ROWS / 2) / NT > 0 ? (ROWS / 2) / NT : 1;  // chunks of one k-row handled per thread
+#pragma unroll
+      for (int i = 0; i < PER; ++i)
+        cp_async16(sm_thread + (i / SPLIT) * (ROWS + KPAD) + (i % SPLIT) * NT * 2,
+                   g_thread + (long long)(i / SPLIT) * ld + (i % SPLIT) * NT * 2, 16);
+    }
+  }
+}
+
+template <int BM, int BN, int WM, int WN, bool A_KM, bool B_KM, int BK>
 struct Cfg {
   static constexpr int NWM = BM / WM, NWN = BN / WN;
   static constexpr int NT = NWM * NWN * 32;
@@ -81,9 +114,9 @@ struct Cfg {
   static constexpr int SMEM = STAGES * (A_ST + B_ST) * (int)sizeof(double);
 };
 
-template <int BM, int BN, int WM, int WN, bool A_KM, bool B_KM, int MINB>
-__global__ void __launch_bounds__(Cfg<BM, BN, WM, WN, A_KM, B_KM>::NT, MINB) gemm_kernel(GemmArgs g) {
-  using C_ = Cfg<BM, BN, WM, WN, A_KM, B_KM>;
+template <int BM, int BN, int WM, int WN, bool A_KM, bool B_KM, int MINB, int BK>
+__global__ void __launch_bounds__(Cfg<BM, BN, WM, WN, A_KM, B_KM, BK>::NT, MINB) gemm_kernel(GemmArgs g) {
+  using C_ = Cfg<BM, BN, WM, WN, A_KM, B_KM, BK>;
   constexpr int NT = C_::NT;
   extern __shared__ __align__(16) double smem[];
   double* As = smem;
@@ -128,12 +161,42 @@ __global__ void __launch_bounds__(Cfg<BM, BN, WM, WN, A_KM, B_KM>::NT, MINB) gem
 
   const int nk = (kend > kbeg) ? (kend - kbeg + BK - 1) / BK : 0;
 
+  // per-thread origins of the fast path (interior tile, aligned operands)
+  const bool fast = vecA && vecB && (m0 + BM <= M) && (n0 + BN <= N);
+  const double* gA;
+  const double* gB;
+  int sA, sB;  // offsets (doubles) of this thread's first chunk inside a stage
+  if (!A_KM) {
+    const int r = tid / (BK / 2), k = (tid % (BK / 2)) * 2;
+    gA = A + (long long)(m0 + r) * g.lda + kbeg + k;
+    sA = r * (BK + KPAD) + k;
+  } else {
+    const int k = tid / (BM / 2), r = (tid % (BM / 2)) * 2;
+    gA = A + (long long)(kbeg + k) * g.lda + m0 + r;
+    sA = k * (BM + KPAD) + r;
+  }
+  if (!B_KM) {
+    const int r = tid / (BK / 2), k = (tid % (BK / 2)) * 2;
+    gB = B + (long long)(n0 + r) * g.ldb + kbeg + k;
+    sB = r * (BK + KPAD) + k;
+  } else {
+    const int k = tid / (BN / 2), r = (tid % (BN / 2)) * 2;
+    gB = B + (long long)(kbeg + k) * g.ldb + n0 + r;
+    sB = k * (BN + KPAD) + r;
+  }
+  const long long stepA = A_KM ? (long long)BK * g.lda : BK, stepB = B_KM ? (long long)BK * g.ldb : BK;
+
   auto issue = [&](int it) {
     if (it < nk) {
-      int s = it % STAGES;
-      int k0 = kbeg + it * BK;
-      load_tile<BM, A_KM, NT>(As + s * C_::A_ST, A, g.lda, m0, M, k0, kend, vecA, tid);
-      load_tile<BN, B_KM, NT>(Bs + s * C_::B_ST, B, g.ldb, n0, N, k0, kend, vecB, tid);
+      const int s = it % STAGES;
+      const int k0 = kbeg + it * BK;
+      if (fast && k0 + BK <= kend) {
+        load_tile_fast<BM, A_KM, NT, BK>(As + s * C_::A_ST + sA, gA + it * stepA, g.lda);
+        load_tile_fast<BN, B_KM, NT, BK>(Bs + s * C_::B_ST + sB, gB + it * stepB, g.ldb);
+      } else {
+        load_tile<BM, A_KM, NT, BK>(As + s * C_::A_ST, A, g.lda, m0, M, k0, kend, vecA, tid);
+        load_tile<BN, B_KM, NT, BK>(Bs + s * C_::B_ST, B, g.ldb, n0, N, k0, kend, vecB, tid);
+      }
     }
     cp_async_commit();
   };
@@ -142,9 +205,13 @@ __global__ void __launch_bounds__(Cfg<BM, BN, WM, WN, A_KM, B_KM>::NT, MINB) gem
   for (int s = 0; s < STAGES - 1; ++s) issue(s);
 
   for (int it = 0; it < nk; ++it) {
-    cp_async_wait<STAGES - 2>();
-    __syncthreads();
-    issue(it + STAGES - 1);  // refills the stage consumed in iteration it-1 (all warps are past it)
+    if (!(g.dbg & 2)) {
+      cp_async_wait<STAGES - 2>();
+      __syncthreads();
+    }
+    // The refill of the stage consumed in iteration it-1 is issued after the first k-step's DMMAs, not right
+    // after the barrier: all warps leave the barrier together, and address arithmetic there would idle the
+    // tensor pipe of every scheduler at once.
     const double* as = As + (it % STAGES) * C_::A_ST;
     const double* bs = Bs + (it % STAGES) * C_::B_ST;
 #pragma unroll
@@ -164,6 +231,7 @@ __global__ void __launch_bounds__(Cfg<BM, BN, WM, WN, A_KM, B_KM>::NT, MINB) gem
       for (int i = 0; i < WM / 8; ++i)
 #pragma unroll
         for (int j = 0; j < WN / 8; ++j) dmma884(acc[i][j][0], acc[i][j][1], af[i], bf[j]);
+      if (kk == 0 && !(g.dbg & 1)) issue(it + STAGES - 1);
     }
   }
   cp_async_wait<0>();
@@ -194,10 +262,10 @@ __global__ void __launch_bounds__(Cfg<BM, BN, WM, WN, A_KM, B_KM>::NT, MINB) gem
   }
 }
 
-template <int BM, int BN, int WM, int WN, bool A_KM, bool B_KM, int MINB>
+template <int BM, int BN, int WM, int WN, bool A_KM, bool B_KM, int MINB, int BK>
 cudaError_t launch_cfg(const GemmArgs& g, cudaStream_t st) {
-  using C_ = Cfg<BM, BN, WM, WN, A_KM, B_KM>;
-  auto kern = gemm_kernel<BM, BN, WM, WN, A_KM, B_KM, MINB>;
+  using C_ = Cfg<BM, BN, WM, WN, A_KM, B_KM, BK>;
+  auto kern = gemm_kernel<BM, BN, WM, WN, A_KM, B_KM, MINB, BK>;
   static bool attr_done = false;  // per instantiation
   if (!attr_done) {
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C_::SMEM);
@@ -209,12 +277,12 @@ cudaError_t launch_cfg(const GemmArgs& g, cudaStream_t st) {
   return cudaGetLastError();
 }
 
-template <int BM, int BN, int WM, int WN, int MINB>
+template <int BM, int BN, int WM, int WN, int MINB, int BK>
 cudaError_t launch_mode(const GemmArgs& g, cudaStream_t st) {
   switch (g.mode) {
-    case GEMM_NN: return launch_cfg<BM, BN, WM, WN, false, true, MINB>(g, st);
-    case GEMM_NT: return launch_cfg<BM, BN, WM, WN, false, false, MINB>(g, st);
-    case GEMM_TN: return launch_cfg<BM, BN, WM, WN, true, true, MINB>(g, st);
+    case GEMM_NN: return launch_cfg<BM, BN, WM, WN, false, true, MINB, BK>(g, st);
+    case GEMM_NT: return launch_cfg<BM, BN, WM, WN, false, false, MINB, BK>(g, st);
+    case GEMM_TN: return launch_cfg<BM, BN, WM, WN, true, true, MINB, BK>(g, st);
   }
   return cudaErrorInvalidValue;
 }
@@ -223,10 +291,27 @@ cudaError_t launch_mode(const GemmArgs& g, cudaStream_t st) {
 
 // Tile choice: 128x128 (8 warps, 32x64 per warp) once the problem fills the chip with big tiles,
 // else 64x64 (4 warps, 32x32 per warp) for more CTAs on small problems.
-cudaError_t launch_gemm(const GemmArgs& g, cudaStream_t st) {
-  if (g.M <= 0 || g.N <= 0) return cudaSuccess;
+cudaError_t launch_gemm(const GemmArgs& g0, cudaStream_t st) {
+  if (g0.M <= 0 || g0.N <= 0) return cudaSuccess;
+  static const int dbg = [] {
+    const char* e = getenv("BTA_GEMM_DBG");
+    return e ? atoi(e) : 0;
+  }();
+  GemmArgs g = g0;
+  g.dbg = dbg;
   long long tiles128 = (long long)((g.M + 127) / 128) * ((g.N + 127) / 128) * (g.subs ? g.nsub : 1);
   if (g.out != OUT_FULL) tiles128 = tiles128 / 2 + 1;
-  if (tiles128 >= 120) return launch_mode<128, 128, 32, 64, 1>(g, st);
-  return launch_mode<64, 64, 32, 32, 2>(g, st);
+  static const int big = [] {
+    const char* e = getenv("BTA_GEMM_CFG");
+    return e ? atoi(e) : 0;
+  }();
+  if (tiles128 >= 120) {
+    switch (big) {
+      case 1: return launch_mode<128, 128, 32, 64, 1, 32>(g, st);
+      case 2: return launch_mode<128, 128, 32, 32, 1, 16>(g, st);
+      case 3: return launch_mode<128, 128, 32, 32, 1, 32>(g, st);
+      default: return launch_mode<128, 128, 32, 64, 1, 16>(g, st);
+    }
+  }
+  return launch_mode<64, 64, 32, 32, 2, 16>(g, st);
 }

@@ -17,7 +17,7 @@
 namespace {
 inline GemmArgs G(int mode, int M, int N, int K, double alpha, const double* A, int lda, const double* B, int ldb,
                   double beta, double* C, int ldc, int klo, int khi, int out) {
-  return GemmArgs{A, B, C, M, N, K, lda, ldb, ldc, alpha, beta, mode, klo, khi, out, nullptr, 0};
+  return GemmArgs{A, B, C, M, N, K, lda, ldb, ldc, alpha, beta, mode, klo, khi, out, nullptr, 0, 0};
 }
 }  // namespace
 
