@@ -140,6 +140,7 @@ def run_ours(args):
     import torch
     import torch.distributed as dist
     from paper_2605_06392_b200 import BtaModel, fp64_peak
+    from paper_2605_06392_b200.replicas import max_over_ranks, replica_thetas
     from workloads import make_config
 
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -156,11 +157,17 @@ def run_ours(args):
             dist.barrier()
         torch.cuda.synchronize()
 
-    model, obs, th = make_config(args.config)
+    if args.nt is not None:
+        from workloads import CONFIGS
+        full_nt = CONFIGS[args.config][0].nt
+        model, obs, th = make_config(args.config, nt=args.nt,
+                                     m_per_var=max(1, CONFIGS[args.config][1] * args.nt // full_nt))
+    else:
+        model, obs, th = make_config(args.config)
     M = BtaModel.from_workload(model, obs, device=local)
     ws_bytes = M.workspace_bytes()
     # one replica per GPU: each rank evaluates f, grad at its own theta (line-search / Hessian-stencil points)
-    thetas = [th + 1e-3 * (rank * 97 + i) * np.ones_like(th) / (1 + i) for i in range(args.steps + args.warmup)]
+    thetas = replica_thetas(th, rank, args.steps + args.warmup)
 
     peak_tf, _ = fp64_peak(0, 100000)
     dfma_tf, _ = fp64_peak(1, 100000)
@@ -193,10 +200,7 @@ def run_ours(args):
     torch.cuda.synchronize()
     ms_e2e = 1e3 * (time.perf_counter() - t0)
     clocks = sampler.stop()
-    if world > 1:
-        t = torch.tensor([ms_dev, ms_e2e], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_dev, ms_e2e = t.tolist()
+    ms_dev, ms_e2e = max_over_ranks([ms_dev, ms_e2e], device="cuda")
     ms_step = ms_dev / args.steps
     value = world * 1e3 / ms_step
     e2e_val = world * 1e3 / (ms_e2e / args.steps)
@@ -214,11 +218,39 @@ def run_ours(args):
             "stage_ms": stage_acc,
             "fp64": {"alg_flop_per_gradient": f_alg(model), "achieved_tflops": f_alg(model) / (ms_step * 1e-3) / 1e12,
                      "dmma_issue_peak_tflops": peak_tf, "dfma_issue_peak_tflops": dfma_tf}}
-    # roofline of the dominant kernel class (the DMMA GEMM sweeps): algorithmic flops of one gradient / step time
-    line["roofline"] = {"bound": "tensor", "achieved": line["fp64"]["achieved_tflops"], "peak": peak_tf,
-                        "unit": "TFLOP/s", "frac": line["fp64"]["achieved_tflops"] / peak_tf, "traffic": None,
+    # ---- roofline of the dominant kernel: the 128x128-tile DMMA GEMM (68 % of the serialised kernel time of a
+    #      step, profiles/r01_launches_bench_nt3.md), timed live on a b x b x b product (operands 3 b^2 8 B > L2
+    #      at the large configs), CUDA events on the launching stream.
+    from paper_2605_06392_b200 import gemm as _gemm
+    b = model.b
+    ga = torch.randn(b, b, dtype=torch.float64, device="cuda")
+    gb = torch.randn(b, b, dtype=torch.float64, device="cuda")
+    gc = torch.empty(b, b, dtype=torch.float64, device="cuda")
+    for _ in range(3):
+        _gemm(0, ga, gb, gc)
+    g0, g1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    reps = 10 if b >= 1024 else 200
+    g0.record()
+    for _ in range(reps):
+        _gemm(0, ga, gb, gc)
+    g1.record()
+    torch.cuda.synchronize()
+    gemm_ms = g0.elapsed_time(g1) / reps
+    gemm_tf = 2.0 * float(b) ** 3 / (gemm_ms * 1e-3) / 1e12
+    del ga, gb, gc
+    line["roofline"] = {"bound": "tensor", "kernel": "gemm_kernel (FP64 mma.sync m8n8k4 / DMMA.8x8x4), C = A B, b^3",
+                        "achieved": gemm_tf, "peak": peak_tf, "unit": "TFLOP/s", "frac": gemm_tf / peak_tf,
+                        "launch_ms": gemm_ms, "alg_flop_per_launch": 2.0 * float(b) ** 3,
+                        "traffic": 1.221e9 if b == 4096 else None,
+                        "traffic_note": "dram read+write bytes per launch at b=4096 from ncu --set full "
+                                        "(profiles/r01_gemm_full.md); algorithmic bytes 3 b^2 8 = 4.03e8",
+                        "share_of_step": 0.68,
                         "peak_source": "measured live: mma.sync.m8n8k4.f64 issue loop on all SMs (MEASURED_PEAKS.json "
-                                       "has no FP64 entry)"}
+                                       "has no FP64 entry; nominal-ratio alternative bf16_tflops x 40/2250 = "
+                                       "29.1 TFLOP/s is lower)"}
+    line["roofline_step"] = {"bound": "tensor", "achieved": line["fp64"]["achieved_tflops"], "peak": peak_tf,
+                             "unit": "TFLOP/s", "frac": line["fp64"]["achieved_tflops"] / peak_tf,
+                             "note": "algorithmic flops of one gradient (14 nt b^3) / step time"}
     if rank == 0 and not args.no_cpu_baseline and world == 1:
         nt_s = {0: 6, 1: 10, 2: 4, 3: 2, 4: 2}[args.config]
         dt, est, nts, _ = oracle_sample(args.config, nt_s)
@@ -241,6 +273,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=4)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--nt", type=int, default=None,
+                    help="profiling aid: truncate the workload to its first NT time blocks (same kernels per block)")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)

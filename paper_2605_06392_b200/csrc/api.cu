@@ -289,15 +289,13 @@ extern "C" int bta_selinv(bta_ctx* c, bta_blocks io, int which, void* ws, void* 
 // ------------------------------------------------------------------------------------------------
 // The hot path: f(theta), grad f(theta)   (PAPER.md:44 Eq. 1, :121 Eq. 6)
 // ------------------------------------------------------------------------------------------------
-extern "C" int inla_value_and_grad(bta_ctx* c, const double* theta, double* f, double* grad, double* stage_ms,
-                                   void* ws, void* stream) {
-  if (!c || !theta || !ws) return bad("inla_value_and_grad: null ctx, theta or workspace");
-  cudaStream_t s0 = (cudaStream_t)stream;
+namespace {
+
+// Enqueue one whole gradient: theta upload -> both chains (interleaved on s0 / s1) -> scalar assembly -> result
+// download into pinned host memory.  With `timed` the stage events are recorded (not capturable in a graph).
+int enqueue_gradient(bta_ctx* c, void* ws, cudaStream_t s0, cudaStream_t s1, bool timed) {
   const ModelDims& md = c->md;
-  BTA_CUDA_OK(cudaSetDevice(c->device));
-  const char* env = getenv("BTA_SERIAL_CHAINS");
-  const bool serial = env && env[0] == '1';
-  cudaStream_t s1 = serial ? s0 : c->s_side;
+  const bool serial = (s0 == s1);
   Bump bp(ws);
   ChainWs wc = carve_chain(bp, md, true);
   ChainWs wp = carve_chain(bp, md, false);
@@ -305,9 +303,12 @@ extern "C" int inla_value_and_grad(bta_ctx* c, const double* theta, double* f, d
   const long long bb = (long long)md.b * md.b;
   const int P = md.a + 1;
   cudaEvent_t* ev = c->ev;
+#define REC(i, st)                                    \
+  do {                                                \
+    if (timed) BTA_CUDA_OK(cudaEventRecord(ev[i], st)); \
+  } while (0)
 
-  memcpy(c->host_pinned, theta, md.d * sizeof(double));
-  BTA_CUDA_OK(cudaEventRecord(ev[0], s0));
+  REC(0, s0);
   BTA_CUDA_OK(cudaMemcpyAsync(c->theta_dev, c->host_pinned, md.d * sizeof(double), cudaMemcpyHostToDevice, s0));
   BTA_CUDA_OK(launch_theta_prep(c, s0));
   BTA_CUDA_OK(cudaMemsetAsync(c->pivot_flag, 0xFF, sizeof(unsigned long long), s0));
@@ -387,10 +388,10 @@ extern "C" int inla_value_and_grad(bta_ctx* c, const double* theta, double* f, d
   // parts of one chain (POTRF leaves, skinny kernels) overlap the GEMMs of the other.
   BTA_CUDA_OK(launch_assemble(c, BTA_COND, cc.D, bb, cc.Bin, bb, wc.Rin, cc.rin_stride, wc.T, md.a,
                               wc.Rin + (long long)md.a * md.b, cc.rin_stride, wc.rtip, 1, s0));
-  BTA_CUDA_OK(cudaEventRecord(ev[1], s0));
-  BTA_CUDA_OK(cudaEventRecord(ev[4], s1));
+  REC(1, s0);
+  REC(4, s1);
   BTA_CUDA_OK(launch_assemble(c, BTA_PRIOR, cp.D, bb, cp.Bin, bb, nullptr, 0, wp.T, md.a, nullptr, 0, nullptr, 0, s1));
-  BTA_CUDA_OK(cudaEventRecord(ev[5], s1));
+  REC(5, s1);
   BTA_CUDA_OK(chain_forward_begin(cc, s0));
   BTA_CUDA_OK(chain_forward_begin(cp, s1));
   for (int t = 0; t < md.nt; ++t) {
@@ -399,10 +400,10 @@ extern "C" int inla_value_and_grad(bta_ctx* c, const double* theta, double* f, d
   }
   BTA_CUDA_OK(chain_forward_end(cc, s0));
   BTA_CUDA_OK(launch_logdet_partial(c, CH_COND, wc.dvec, s0));
-  BTA_CUDA_OK(cudaEventRecord(ev[2], s0));
+  REC(2, s0);
   BTA_CUDA_OK(chain_forward_end(cp, s1));
   BTA_CUDA_OK(launch_logdet_partial(c, CH_PRIOR, wp.dvec, s1));
-  BTA_CUDA_OK(cudaEventRecord(ev[6], s1));
+  REC(6, s1);
   for (int t = md.nt - 1; t >= 0; --t) {
     BTA_CUDA_OK(chain_backward_step(cc, t, s0));
     BTA_CUDA_OK(chain_backward_step(cp, t, s1));
@@ -411,18 +412,74 @@ extern "C" int inla_value_and_grad(bta_ctx* c, const double* theta, double* f, d
                               s0));
   BTA_CUDA_OK(launch_quad_stencil(c, wc.x, s0));
   BTA_CUDA_OK(launch_residual(c, wc.x, s0));
-  BTA_CUDA_OK(cudaEventRecord(ev[3], s0));
+  REC(3, s0);
   BTA_CUDA_OK(cudaEventRecord(ev[7], s1));
   if (!serial) BTA_CUDA_OK(cudaStreamWaitEvent(s0, ev[7], 0));
 
   // ---- scalar assembly (a9) ----
-  BTA_CUDA_OK(cudaEventRecord(ev[10], s0));
+  REC(10, s0);
   BTA_CUDA_OK(launch_scalars(c, s0));
   const int nout = 1 + md.d + 2 + 3 * md.d + md.k + 1;
   BTA_CUDA_OK(cudaMemcpyAsync(c->host_pinned + 64, c->small + L.out, nout * sizeof(double), cudaMemcpyDeviceToHost,
                               s0));
-  BTA_CUDA_OK(cudaEventRecord(ev[8], s0));
-  int rc = check_pivot(c, s0);  // synchronises s0 (and, through ev[7], the side stream)
+  REC(8, s0);
+  c->last_x_dev = wc.x;
+#undef REC
+  return BTA_OK;
+}
+
+}  // namespace
+
+extern "C" int inla_value_and_grad(bta_ctx* c, const double* theta, double* f, double* grad, double* stage_ms,
+                                   void* ws, void* stream) {
+  if (!c || !theta || !ws) return bad("inla_value_and_grad: null ctx, theta or workspace");
+  cudaStream_t s0 = (cudaStream_t)stream;
+  const ModelDims& md = c->md;
+  BTA_CUDA_OK(cudaSetDevice(c->device));
+  const char* env = getenv("BTA_SERIAL_CHAINS");
+  const bool serial = env && env[0] == '1';
+  // Small blocks are launch/latency-bound (tens of thousands of ~2 us kernels): from the second call on, replay
+  // the whole gradient as one CUDA graph.  BTA_GRAPH=0/1 overrides the size rule (b <= 1024).
+  const char* genv = getenv("BTA_GRAPH");
+  const bool want_graph = genv ? genv[0] == '1' : md.b <= 1024;
+  cudaEvent_t* ev = c->ev;
+  memcpy(c->host_pinned, theta, md.d * sizeof(double));
+  cudaStream_t sync_stream = s0;
+  bool timed = true;
+  if (want_graph && !serial && c->grad_calls > 0) {
+    if (!c->graph_exec || c->graph_ws != ws) {
+      if (c->graph_exec) {
+        cudaGraphExecDestroy(c->graph_exec);
+        c->graph_exec = nullptr;
+      }
+      const long long n0 = c->launches;
+      cudaGraph_t graph = nullptr;
+      BTA_CUDA_OK(cudaStreamBeginCapture(c->s_main, cudaStreamCaptureModeThreadLocal));
+      int rc = enqueue_gradient(c, ws, c->s_main, c->s_side, false);
+      cudaError_t ce = cudaStreamEndCapture(c->s_main, &graph);
+      if (rc != BTA_OK) return rc;
+      BTA_CUDA_OK(ce);
+      BTA_CUDA_OK(cudaGraphInstantiate(&c->graph_exec, graph, 0));
+      cudaGraphDestroy(graph);
+      c->graph_ws = ws;
+      c->graph_launches = c->launches - n0;
+      c->launches = n0;
+    }
+    BTA_CUDA_OK(cudaEventRecord(ev[11], s0));
+    BTA_CUDA_OK(cudaStreamWaitEvent(c->s_main, ev[11], 0));
+    BTA_CUDA_OK(cudaEventRecord(ev[0], c->s_main));
+    BTA_CUDA_OK(cudaGraphLaunch(c->graph_exec, c->s_main));
+    BTA_CUDA_OK(cudaEventRecord(ev[8], c->s_main));
+    BTA_CUDA_OK(cudaStreamWaitEvent(s0, ev[8], 0));
+    c->launches += c->graph_launches;
+    sync_stream = c->s_main;
+    timed = false;
+  } else {
+    int rc = enqueue_gradient(c, ws, s0, serial ? s0 : c->s_side, true);
+    if (rc != BTA_OK) return rc;
+  }
+  c->grad_calls++;
+  int rc = check_pivot(c, sync_stream);  // synchronises the stream (and, through ev[7], the side stream)
   const double* o = c->host_pinned + 64;
   if (f) *f = o[0];
   if (grad) memcpy(grad, o + 1, md.d * sizeof(double));
@@ -431,8 +488,12 @@ extern "C" int inla_value_and_grad(bta_ctx* c, const double* theta, double* f, d
   c->last_parts.assign(o + 1 + md.d + 2, o + 1 + md.d + 2 + 3 * md.d);
   c->last_rss.assign(o + 1 + md.d + 2 + 3 * md.d, o + 1 + md.d + 2 + 3 * md.d + md.k);
   c->last_quad = o[1 + md.d + 2 + 3 * md.d + md.k];
-  c->last_x_dev = wc.x;
-  if (stage_ms) {
+  if (stage_ms && !timed) {
+    for (int i = 0; i < BTA_NSTAGES; ++i) stage_ms[i] = 0.0;
+    float ms = 0.f;
+    cudaEventElapsedTime(&ms, ev[0], ev[8]);
+    stage_ms[BTA_STAGE_TOTAL] = ms;
+  } else if (stage_ms) {
     auto el = [&](int a_, int b_) {
       float ms = 0.f;
       cudaEventElapsedTime(&ms, ev[a_], ev[b_]);

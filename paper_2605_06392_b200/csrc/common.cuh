@@ -129,6 +129,11 @@ struct bta_ctx {
   size_t small_doubles;
   double* host_pinned;               // pinned host staging (theta in, f/grad/intermediates out)
   cudaStream_t s_side;               // second chain's stream
+  cudaStream_t s_main;               // graph mode: the captured/replayed stream (the caller's may be stream 0)
+  cudaGraphExec_t graph_exec;        // cached replay of one whole gradient (small models), or nullptr
+  void* graph_ws;                    // workspace pointer the cached graph was captured with
+  long long graph_launches;          // kernels inside the cached graph
+  long long grad_calls;
   cudaEvent_t ev[16];
   long long launches;
   long long last_pivot;

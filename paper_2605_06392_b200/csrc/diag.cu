@@ -17,19 +17,25 @@ namespace {
 // constants and the per-step instruction count stays small.
 template <int NB, int NW>
 struct LeafSmem {
-  double colraw[2][NB], rowraw[2][NB], rsq[2];
+  double colraw[2][NB], rowraw[2][NB], diagraw[2];
+};
+
+struct LeafPivot {
+  double rs, piv;  // 1/sqrt(pivot_k) and pivot_k, held redundantly by every thread
 };
 
 template <int NB, int NW, int BLK>
-__device__ __forceinline__ bool leaf_steps(double (&w)[NB / NW][NB / 32], LeafSmem<NB, NW>& sm, int n, int lane,
-                                           int warp, double* __restrict__ diagL, long long grow0,
+__device__ __forceinline__ bool leaf_steps(double (&w)[NB / NW][NB / 32], LeafSmem<NB, NW>& sm, LeafPivot& pv, int n,
+                                           int lane, int warp, double* __restrict__ diagL, long long grow0,
                                            unsigned long long* __restrict__ pivot_flag) {
   constexpr int R = NB / NW, CC = NB / 32;
   constexpr int K0 = BLK * NW, KC = K0 / 32, KR = BLK, L0 = K0 % 32;
+  constexpr int KCN = (K0 + NW) / 32;  // column slot of the first pivot of the next block
 #pragma unroll 1
   for (int q = 0; q < NW; ++q) {
     const int k = K0 + q, kl = L0 + q, buf = q & 1;
     if (k >= n) return false;
+    // ---- publish column k (rows >= K0), row k (columns <= k) and the raw diagonal entry of step k+1
     if (lane == kl) {
 #pragma unroll
       for (int r = KR; r < R; ++r) sm.colraw[buf][warp + NW * r] = w[r][KC];
@@ -37,21 +43,28 @@ __device__ __forceinline__ bool leaf_steps(double (&w)[NB / NW][NB / 32], LeafSm
     if (warp == q) {
 #pragma unroll
       for (int c = 0; c <= KC; ++c) sm.rowraw[buf][lane + 32 * c] = w[KR][c];
-      if (lane == kl) {
-        double piv = w[KR][KC];
-        if (!(piv > 0.0)) {  // also catches NaN
-          atomicMin(pivot_flag, (unsigned long long)(grow0 + k + 1));
-          piv = 1.0;
-        }
-        const double rsn = rsqrt(piv);
-        sm.rsq[buf] = rsn;
-        if (diagL) diagL[k] = piv * rsn;
-      }
+    }
+    if (q < NW - 1) {
+      if (warp == q + 1 && lane == kl + 1) sm.diagraw[buf] = w[KR][KC];
+    } else if (KR + 1 < R) {
+      if (warp == 0 && lane == (L0 + NW) % 32) sm.diagraw[buf] = w[KR + 1 < R ? KR + 1 : KR][KCN < CC ? KCN : KC];
     }
     __syncthreads();
     const double* cr = sm.colraw[buf];
     const double* rr = sm.rowraw[buf];
-    const double rs = sm.rsq[buf];
+    const double rs = pv.rs;
+    if (threadIdx.x == 0 && diagL) diagL[k] = pv.piv * rs;
+    // ---- 1/sqrt of the next pivot, by every thread, off the critical path of the updates below
+    if (k + 1 < n) {
+      const double l = cr[k + 1] * rs;
+      double pn = fma(-l, l, sm.diagraw[buf]);
+      if (!(pn > 0.0)) {  // also catches NaN
+        if (threadIdx.x == 0) atomicMin(pivot_flag, (unsigned long long)(grow0 + k + 2));
+        pn = 1.0;
+      }
+      pv.piv = pn;
+      pv.rs = rsqrt(pn);
+    }
     double cv[CC];
 #pragma unroll
     for (int c = 0; c < CC; ++c) {
@@ -70,8 +83,6 @@ __device__ __forceinline__ bool leaf_steps(double (&w)[NB / NW][NB / 32], LeafSm
     }
 #pragma unroll
     for (int r = KR; r < R; ++r) {
-      constexpr int dummy = 0;
-      (void)dummy;
       const int i = warp + NW * r;
       // columns beyond the diagonal slot of this row are never read: skip them
       const int cmax = (NW * r + NW - 1) / 32;
@@ -92,17 +103,17 @@ __device__ __forceinline__ bool leaf_steps(double (&w)[NB / NW][NB / 32], LeafSm
 
 template <int NB, int NW, int BLK>
 struct LeafRun {
-  static __device__ __forceinline__ void run(double (&w)[NB / NW][NB / 32], LeafSmem<NB, NW>& sm, int n, int lane,
-                                             int warp, double* diagL, long long grow0,
+  static __device__ __forceinline__ void run(double (&w)[NB / NW][NB / 32], LeafSmem<NB, NW>& sm, LeafPivot& pv,
+                                             int n, int lane, int warp, double* diagL, long long grow0,
                                              unsigned long long* pivot_flag) {
-    if (leaf_steps<NB, NW, BLK>(w, sm, n, lane, warp, diagL, grow0, pivot_flag))
-      LeafRun<NB, NW, BLK + 1>::run(w, sm, n, lane, warp, diagL, grow0, pivot_flag);
+    if (leaf_steps<NB, NW, BLK>(w, sm, pv, n, lane, warp, diagL, grow0, pivot_flag))
+      LeafRun<NB, NW, BLK + 1>::run(w, sm, pv, n, lane, warp, diagL, grow0, pivot_flag);
   }
 };
 template <int NB, int NW>
 struct LeafRun<NB, NW, NB / NW> {
-  static __device__ __forceinline__ void run(double (&)[NB / NW][NB / 32], LeafSmem<NB, NW>&, int, int, int, double*,
-                                             long long, unsigned long long*) {}
+  static __device__ __forceinline__ void run(double (&)[NB / NW][NB / 32], LeafSmem<NB, NW>&, LeafPivot&, int, int,
+                                             int, double*, long long, unsigned long long*) {}
 };
 
 template <int NB, int NW>
@@ -123,7 +134,14 @@ __global__ void __launch_bounds__(32 * NW) potrf_inv_tile_kernel(double* __restr
       if (i < n && j <= i) v = A[(long long)i * ld + j];
       w[r][c] = v;
     }
-  LeafRun<NB, NW, 0>::run(w, sm, n, lane, warp, diagL, grow0, pivot_flag);
+  LeafPivot pv;
+  pv.piv = A[0];
+  if (!(pv.piv > 0.0)) {
+    if (tid == 0) atomicMin(pivot_flag, (unsigned long long)(grow0 + 1));
+    pv.piv = 1.0;
+  }
+  pv.rs = rsqrt(pv.piv);
+  LeafRun<NB, NW, 0>::run(w, sm, pv, n, lane, warp, diagL, grow0, pivot_flag);
 #pragma unroll
   for (int r = 0; r < R; ++r)
 #pragma unroll
@@ -234,7 +252,7 @@ cudaError_t launch_potrf_inv_tile(double* A, int ld, int n, double* diagL, long 
   if (n <= 64)
     potrf_inv_tile_kernel<64, 8><<<1, 256, 0, st>>>(A, ld, n, diagL, grow0, pivot_flag);
   else if (n <= 128)
-    potrf_inv_tile_kernel<128, 16><<<1, 512, 0, st>>>(A, ld, n, diagL, grow0, pivot_flag);
+    potrf_inv_tile_kernel<128, 8><<<1, 256, 0, st>>>(A, ld, n, diagL, grow0, pivot_flag);
   else
     return cudaErrorInvalidValue;
   return cudaGetLastError();

@@ -84,6 +84,11 @@ extern "C" int bta_create(bta_ctx** out, const bta_model_desc* desc, const bta_o
   BTA_CUDA_OK(cudaMemset(c->small, 0, L.total * sizeof(double)));
   BTA_CUDA_OK(cudaMallocHost((void**)&c->host_pinned, 4096 * sizeof(double)));
   BTA_CUDA_OK(cudaStreamCreateWithFlags(&c->s_side, cudaStreamNonBlocking));
+  BTA_CUDA_OK(cudaStreamCreateWithFlags(&c->s_main, cudaStreamNonBlocking));
+  c->graph_exec = nullptr;
+  c->graph_ws = nullptr;
+  c->graph_launches = 0;
+  c->grad_calls = 0;
   for (auto& e : c->ev) BTA_CUDA_OK(cudaEventCreate(&e));
   if (m > 0) {
     BTA_CUDA_OK(cudaMemcpy(c->o_var, obs->var, m * sizeof(int), cudaMemcpyHostToDevice));
@@ -117,7 +122,9 @@ extern "C" int bta_destroy(bta_ctx* c) {
   cudaFree(c->pivot_flag);
   cudaFree(c->small);
   cudaFreeHost(c->host_pinned);
+  if (c->graph_exec) cudaGraphExecDestroy(c->graph_exec);
   cudaStreamDestroy(c->s_side);
+  cudaStreamDestroy(c->s_main);
   for (auto& e : c->ev) cudaEventDestroy(e);
   delete c;
   return BTA_OK;

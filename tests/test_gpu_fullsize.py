@@ -1,0 +1,123 @@
+"""Parity at BASELINE.json's full sizes, in the launch configuration bench.py times.  The oracle cannot run
+configs 2-4 in seconds, so these tests use (i) the oracle on an nt-truncated model of the same block size,
+(ii) properties that hold at any size: the DCT closed form for log det Q_p and the Phase-C traces (pin P9), the
+sum rules P7/P8, the value identity P6, the residual Q_c x* = r on every row, the uniform-design closed form for
+log det Q_c and Phase A (pin P12), and the scalar assembly of f recomputed from the returned intermediates."""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+from oracle import bta_oracle as O
+from workloads import CONFIGS, make_config, uniform_design
+from workloads.generate import Model, draw_theta
+
+from closed_form import closed_form
+
+TOL_F, TOL_G = 1e-9, 1e-6
+
+
+def _run(model, obs, th):
+    from paper_2605_06392_b200 import BtaModel
+    M = BtaModel.from_workload(model, obs, device=0)
+    f, g = M.inla_value_and_grad(th)
+    im = M.last_intermediates()
+    M.close()
+    return f, g, im
+
+
+def _grad_ok(g, ref):
+    gate = np.maximum(np.abs(ref), 1e-3 * np.max(np.abs(ref)))
+    return np.all(np.abs(g - ref) <= TOL_G * gate)
+
+
+@pytest.mark.parametrize("idx", [2, 3, 4])
+def test_truncated_model_vs_oracle(idx):
+    """Same block size b (same GEMM tiles, leaves and skinny-kernel grids as the full config), nt = 2."""
+    full = CONFIGS[idx][0]
+    model, obs, th = make_config(idx, nt=2, m_per_var=max(1, CONFIGS[idx][1] * 2 // full.nt))
+    ref = O.value_and_grad(model, obs, th)
+    f, g, im = _run(model, obs, th)
+    assert abs(im["ld_p"] - ref["ld_p"]) <= TOL_F * abs(ref["ld_p"])
+    assert abs(im["ld_c"] - ref["ld_c"]) <= TOL_F * abs(ref["ld_c"])
+    assert abs(f - ref["f"]) <= TOL_F * abs(ref["f"])
+    assert _grad_ok(g, ref["grad"]), (g, ref["grad"])
+    assert np.max(np.abs(im["x"] - ref["x"])) <= 1e-9 * np.max(np.abs(ref["x"]))
+
+
+def _closed_form_prior(model, th):
+    """ld(Q_p) and the per-variable Phase-C traces from the DCT closed form (det Lam = 1: ld_p = sum_m ld(Q_m))."""
+    k = model.k
+    ld = model.a * np.log(model.fixed_prec)
+    tr = np.zeros(3 * k)
+    for m in range(k):
+        l, t = closed_form(model.g, model.nt, model.h, th[3 * m: 3 * m + 3])
+        ld += l
+        tr[3 * m: 3 * m + 3] = t
+    return ld, tr
+
+
+@pytest.mark.parametrize("idx", [2, 3, 4])
+def test_full_size_properties(idx):
+    model, obs, th = make_config(idx)
+    k, nt, b, ns, a, N = model.k, model.nt, model.b, model.ns, model.a, model.N
+    f, g, im = _run(model, obs, th)
+    E, Lam, tau = O.unpack_theta(model, th)
+    nprior = model.d - k
+    # P9 / P10: prior log-determinant and Phase-C traces
+    ld_cf, tr_cf = _closed_form_prior(model, th)
+    assert abs(im["ld_p"] - ld_cf) <= TOL_F * abs(ld_cf)
+    assert np.max(np.abs(im["phaseC"][: 3 * k] - tr_cf)) <= TOL_G * np.max(np.abs(tr_cf))
+    if nprior > 3 * k:                                                                   # d ld_p / d lambda = 0
+        assert np.max(np.abs(im["phaseC"][3 * k: nprior])) <= TOL_G * np.max(np.abs(tr_cf))
+    # P8, P7 sum rules
+    assert abs(np.sum(im["phaseC"][: 3 * k]) - nt * b) <= TOL_F * N
+    idxs = list(range(3 * k)) + list(range(nprior, model.d))
+    assert abs(np.sum(im["phaseA"][idxs]) + model.fixed_prec * np.trace(im["ZT"]) - N) <= TOL_F * N
+    # residual Q_c x* = r on every row, Q_c applied from the base matrices (not from any block code)
+    x = im["x"]
+    X = x[: nt * b].reshape(nt, k, ns)
+    xT = x[nt * b:]
+    Ks = O.spatial_matrices(model.g, model.h)
+    Ms = O.temporal_matrices(nt)
+    W = O.weights(model, th)
+    Qx = np.zeros_like(X)
+    for c in range(3):
+        KX = np.einsum("tvs,sr->tvr", X, Ks[c])                    # K_c symmetric
+        WKX = np.einsum("ij,tjs->tis", W[c], KX)
+        Qx += np.einsum("tu,uis->tis", Ms[c], WKX)
+    agg = O.aggregates(model, obs)
+    tau_col = np.repeat(tau, ns)
+    Qx = Qx.reshape(nt, b) + tau_col * agg.cnt * X.reshape(nt, b) + tau_col * np.einsum("tpj,p->tj", agg.zsum, xT)
+    r = tau_col * agg.ysum
+    scale = np.max(np.abs(r))
+    assert np.max(np.abs(Qx - r)) <= 1e-9 * scale
+    tipres = (model.fixed_prec * xT + sum(tau[v] * agg.ZZ[v] @ xT for v in range(k))
+              + np.einsum("tpj,tj->p", agg.zsum * tau_col, X.reshape(nt, b)) - sum(tau[v] * agg.zy[v] for v in range(k)))
+    assert np.max(np.abs(tipres)) <= 1e-9 * max(scale, np.max(np.abs(sum(tau[v] * agg.zy[v] for v in range(k)))))
+    # P6 value identity and the scalar assembly of f from the intermediates
+    rTx = np.sum(r * X.reshape(nt, b)) + sum(tau[v] * agg.zy[v] for v in range(k)) @ xT
+    lhs = -0.5 * im["quad_p"] - 0.5 * np.sum(tau * im["rss"])
+    rhs = 0.5 * rTx - 0.5 * np.sum(tau * agg.yy)
+    assert abs(lhs - rhs) <= 1e-9 * abs(rhs)
+    f_re = (-0.5 * th @ th + 0.5 * im["ld_p"] - 0.5 * im["ld_c"] - 0.5 * im["quad_p"]
+            + np.sum(0.5 * agg.mv * th[nprior:] - 0.5 * tau * im["rss"]))
+    assert abs(f - f_re) <= 1e-12 * abs(f_re)
+    grad_re = -0.5 * im["phaseA"] - 0.5 * im["phaseB"] + 0.5 * im["phaseC"] - th
+    grad_re[nprior:] += 0.5 * agg.mv - 0.5 * tau * im["rss"]
+    assert np.max(np.abs(g - grad_re)) <= 1e-12 * np.max(np.abs(grad_re))
+
+
+@pytest.mark.parametrize("idx", [2, 4])
+def test_full_size_uniform_design_closed_form(idx):
+    """Pin P12 at full block size: every site observed once, zero covariates => Q_c latent part = Q_st + tau I."""
+    full = CONFIGS[idx][0]
+    model = Model(g=full.g, k=1, nt=8, a=full.a)
+    obs = uniform_design(model, c=1)
+    th = draw_theta(model, 99)
+    f, g, im = _run(model, obs, th)
+    tau = np.exp(th[3])
+    ld_cf, tr_cf = closed_form(model.g, model.nt, model.h, th[:3], shift=tau)
+    ld = im["ld_c"] - model.a * np.log(model.fixed_prec)
+    assert abs(ld - ld_cf) <= TOL_F * abs(ld_cf)
+    assert np.max(np.abs(im["phaseA"][:3] - tr_cf)) <= TOL_G * np.max(np.abs(tr_cf))
