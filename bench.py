@@ -165,6 +165,8 @@ def run_ours(args):
     else:
         model, obs, th = make_config(args.config)
     M = BtaModel.from_workload(model, obs, device=local)
+    if args.store == "carry":
+        M.bta_set_store_mode(1)
     ws_bytes = M.workspace_bytes()
     # one replica per GPU: each rank evaluates f, grad at its own theta (line-search / Hessian-stencil points)
     thetas = replica_thetas(th, rank, args.steps + args.warmup)
@@ -210,7 +212,7 @@ def run_ours(args):
             "dtype": "f64", "data": "synthetic",
             "config": {"workload": workload_name(args.config, model), "parallelism": f"replicas x{world}",
                        "l2": "inputs larger than L2 (blocks of both matrices: %.1f GB per replica)" % (ws_bytes / 1e9),
-                       "workspace_bytes": ws_bytes, "chains": "Q_c and Q_p sweeps on two streams"},
+                       "workspace_bytes": ws_bytes, "chains": "Q_c and Q_p sweeps on two streams", "store_mode": args.store},
             "clocks": clocks,
             "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": 8 * d,
                     "d2h_bytes_per_step": 8 * (1 + d + 2 + 3 * d + model.k + 1) + 8},
@@ -273,6 +275,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=4)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--store", default="factor", choices=["factor", "carry"],
+                    help="storage policy a7: keep the factor blocks (default) or only the Schur carries")
     ap.add_argument("--nt", type=int, default=None,
                     help="profiling aid: truncate the workload to its first NT time blocks (same kernels per block)")
     args = ap.parse_args()

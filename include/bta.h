@@ -82,6 +82,17 @@ typedef struct {
 int bta_create(bta_ctx** out, const bta_model_desc* desc, const bta_obs* obs, int device);
 int bta_destroy(bta_ctx* ctx);
 
+/* Storage policy of inla_value_and_grad.
+ *   BTA_STORE_FACTOR (default): the factor blocks X_t = L_Dt^-1 and L_Bt are kept for the backward sweep
+ *     ((2nt-1) b^2 doubles per matrix, no recomputation).
+ *   BTA_STORE_CARRY: the paper's carry-based reconstruction -- only the Schur-updated diagonal blocks
+ *     D_t - S_{t-1} ("carries", nt b^2 doubles per matrix) and the O(a b) arrow rows / z_t are kept; the backward
+ *     sweep rebuilds X_t (one more Cholesky + inverse) and L_Bt (B_t is re-assembled, one more product) per block.
+ * Changes bta_workspace_bytes.  Returns BTA_ERR_ARG for an unknown mode. */
+enum { BTA_STORE_FACTOR = 0, BTA_STORE_CARRY = 1 };
+int bta_set_store_mode(bta_ctx* ctx, int mode);
+int bta_get_store_mode(const bta_ctx* ctx);
+
 /* Bytes of caller-provided device workspace needed by inla_value_and_grad (the largest user: both matrices'
  * blocks, per-chain temporaries).  bta_factor_logdet / bta_solve / bta_selinv need at most
  * bta_workspace_bytes_op(ctx) (three b x b temporaries + small vectors). */

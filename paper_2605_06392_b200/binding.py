@@ -69,6 +69,8 @@ def lib():
     L.bta_kernel_launches.argtypes = [vp]
     L.bta_kernel_launches.restype = i64
     L.bta_last_error.restype = C.c_char_p
+    L.bta_set_store_mode.argtypes = [vp, i32]
+    L.bta_get_store_mode.argtypes = [vp]
     L.bta_fp64_peak.argtypes = [i32, i32, dp, dp, vp]
     L.bta_gemm.argtypes = [i32, i32, i32, i32, C.c_double, vp, i32, vp, i32, C.c_double, vp, i32, i32, i32, i32, vp]
     _lib = L
@@ -108,6 +110,7 @@ class Blocks:
 
 
 BTA_PRIOR, BTA_COND = 0, 1
+BTA_STORE_FACTOR, BTA_STORE_CARRY = 0, 1
 STAGES = ("assemble", "fwd_Qc", "bwd_Qc", "fwd_Qp", "bwd_Qp", "scalars", "total")
 
 
@@ -224,6 +227,14 @@ class BtaModel:
                                             C.byref(quad), _dptr(ZT)))
         return dict(ZT=ZT, ld_p=ld[0], ld_c=ld[1], x=x, phaseA=parts[: self.d], phaseB=parts[self.d: 2 * self.d],
                     phaseC=parts[2 * self.d:], rss=rss, quad_p=quad.value)
+
+    def bta_set_store_mode(self, mode):
+        """BTA_STORE_FACTOR (0) or BTA_STORE_CARRY (1); the gradient workspace is re-sized on next use."""
+        _check(lib().bta_set_store_mode(self._h, int(mode)))
+        self._ws = None
+
+    def bta_get_store_mode(self):
+        return lib().bta_get_store_mode(self._h)
 
     def kernel_launches(self):
         return lib().bta_kernel_launches(self._h)

@@ -19,17 +19,23 @@ struct Bump {
 };
 
 struct ChainWs {
-  double *D, *B, *W1, *W2, *W3, *Rin, *Rout, *ubuf, *Ebuf, *Ybuf, *ZC0, *ZC1, *part, *x, *dvec, *T, *rtip;
+  double *D, *B, *W1, *W2, *W3, *Rin, *Rout, *ubuf, *Ebuf, *Ybuf, *ZC0, *ZC1, *part, *x, *dvec, *T, *rtip, *Xs, *LBs, *Bs;
 };
 
 // Workspace of one chain of the fused gradient.  Q_c: nt D slots, nt B slots (L_Bt is written one slot below
 // B_t, so no copy), 3 scratch blocks, the arrow/rhs stacks; Q_p: the same without the stacks.
-ChainWs carve_chain(Bump& bp, const ModelDims& md, bool cond) {
+ChainWs carve_chain(Bump& bp, const ModelDims& md, bool cond, int store_mode) {
   ChainWs w{};
   const size_t bb = (size_t)md.b * md.b;
   const int P = md.a + 1;
   w.D = bp.take(bb * md.nt);
-  w.B = bp.take(bb * md.nt);
+  if (store_mode == BTA_STORE_CARRY) {
+    w.Xs = bp.take(bb);
+    w.LBs = bp.take(bb);
+    w.Bs = bp.take(bb);
+  } else {
+    w.B = bp.take(bb * md.nt);
+  }
   w.W1 = bp.take(bb);
   w.W2 = bp.take(bb);
   w.W3 = bp.take(bb);
@@ -50,10 +56,10 @@ ChainWs carve_chain(Bump& bp, const ModelDims& md, bool cond) {
   return w;
 }
 
-size_t grad_ws_bytes(const ModelDims& md) {
+size_t grad_ws_bytes(const ModelDims& md, int store_mode) {
   Bump bp(nullptr);
-  carve_chain(bp, md, true);
-  carve_chain(bp, md, false);
+  carve_chain(bp, md, true, store_mode);
+  carve_chain(bp, md, false, store_mode);
   return bp.off + 256;
 }
 
@@ -106,7 +112,7 @@ int bad(const char* msg) {
 
 }  // namespace
 
-extern "C" size_t bta_workspace_bytes(const bta_ctx* c) { return c ? grad_ws_bytes(c->md) : 0; }
+extern "C" size_t bta_workspace_bytes(const bta_ctx* c) { return c ? grad_ws_bytes(c->md, c->store_mode) : 0; }
 extern "C" size_t bta_workspace_bytes_op(const bta_ctx* c) {
   if (!c) return 0;
   Bump bp(nullptr);
@@ -297,8 +303,9 @@ int enqueue_gradient(bta_ctx* c, void* ws, cudaStream_t s0, cudaStream_t s1, boo
   const ModelDims& md = c->md;
   const bool serial = (s0 == s1);
   Bump bp(ws);
-  ChainWs wc = carve_chain(bp, md, true);
-  ChainWs wp = carve_chain(bp, md, false);
+  const bool carry = c->store_mode == BTA_STORE_CARRY;
+  ChainWs wc = carve_chain(bp, md, true, c->store_mode);
+  ChainWs wp = carve_chain(bp, md, false, c->store_mode);
   SmallLayout L = small_layout(md);
   const long long bb = (long long)md.b * md.b;
   const int P = md.a + 1;
@@ -327,7 +334,12 @@ int enqueue_gradient(bta_ctx* c, void* ws, cudaStream_t s0, cudaStream_t s1, boo
   cc.selinv = cc.contract = true;
   cc.D = wc.D;
   cc.d_stride = bb;
-  cc.Bin = wc.B + bb;  // B_t assembled into slot t+1, L_Bt written to slot t
+  cc.carry = carry;
+  cc.which = BTA_COND;
+  cc.Xs = wc.Xs;
+  cc.LBs = wc.LBs;
+  cc.Bs = wc.Bs;
+  cc.Bin = carry ? nullptr : wc.B + bb;  // B_t assembled into slot t+1, L_Bt written to slot t
   cc.Bout = wc.B;
   cc.b_stride = bb;
   cc.Rin = wc.Rin;
@@ -370,7 +382,12 @@ int enqueue_gradient(bta_ctx* c, void* ws, cudaStream_t s0, cudaStream_t s1, boo
   cp.selinv = cp.contract = true;
   cp.D = wp.D;
   cp.d_stride = bb;
-  cp.Bin = wp.B + bb;
+  cp.carry = carry;
+  cp.which = BTA_PRIOR;
+  cp.Xs = wp.Xs;
+  cp.LBs = wp.LBs;
+  cp.Bs = wp.Bs;
+  cp.Bin = carry ? nullptr : wp.B + bb;
   cp.Bout = wp.B;
   cp.b_stride = bb;
   cp.T = wp.T;

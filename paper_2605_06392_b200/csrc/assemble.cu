@@ -31,8 +31,8 @@ __global__ void theta_prep_kernel(const double* __restrict__ theta, DevParams* _
 // kind 0: D_t (lower triangle + diagonal, strict upper = 0; + tau cnt on the diagonal for Q_c);  kind 1: B_t.
 __global__ void __launch_bounds__(256) assemble_blocks_kernel(ModelDims md, const DevParams* __restrict__ P, int kind,
                                                               int cond, const double* __restrict__ cnt,
-                                                              double* __restrict__ out, long long stride) {
-  const int j = blockIdx.x * 256 + threadIdx.x, i = blockIdx.y, t = blockIdx.z;
+                                                              double* __restrict__ out, long long stride, int t0) {
+  const int j = blockIdx.x * 256 + threadIdx.x, i = blockIdx.y, t = blockIdx.z + t0;
   if (j >= md.b) return;
   double v = 0.0;
   if (kind == 1 || j <= i) {
@@ -50,7 +50,7 @@ __global__ void __launch_bounds__(256) assemble_blocks_kernel(ModelDims md, cons
     }
     if (kind == 0 && cond && i == j) v += P->tau[vi] * cnt[(long long)t * md.b + i];
   }
-  out[(long long)t * stride + (long long)i * md.b + j] = v;
+  out[(long long)(t - t0) * stride + (long long)i * md.b + j] = v;
 }
 
 __global__ void assemble_arrow_kernel(ModelDims md, const DevParams* __restrict__ P, int cond,
@@ -217,12 +217,12 @@ cudaError_t launch_assemble(bta_ctx* c, int which, double* D, long long d_stride
   const int cond = which == BTA_COND;
   dim3 gx((md.b + 255) / 256, md.b, md.nt);
   if (D) {
-    assemble_blocks_kernel<<<gx, 256, 0, st>>>(md, c->P, 0, cond, c->cnt, D, d_stride);
+    assemble_blocks_kernel<<<gx, 256, 0, st>>>(md, c->P, 0, cond, c->cnt, D, d_stride, 0);
     BTA_COUNT(c);
   }
   if (B && md.nt > 1) {
     dim3 gb((md.b + 255) / 256, md.b, md.nt - 1);
-    assemble_blocks_kernel<<<gb, 256, 0, st>>>(md, c->P, 1, cond, c->cnt, B, b_stride);
+    assemble_blocks_kernel<<<gb, 256, 0, st>>>(md, c->P, 1, cond, c->cnt, B, b_stride, 0);
     BTA_COUNT(c);
   }
   if (C || rhs) {
@@ -234,6 +234,14 @@ cudaError_t launch_assemble(bta_ctx* c, int which, double* D, long long d_stride
     assemble_tip_kernel<<<1, md.a * md.a, 0, st>>>(md, c->P, cond, c->ZZ, c->zy, T, ldt, rhs_tip, rhs_tip_stride);
     BTA_COUNT(c);
   }
+  return cudaGetLastError();
+}
+
+cudaError_t launch_assemble_block(bta_ctx* c, int which, int kind, int t, double* out, cudaStream_t st) {
+  const ModelDims& md = c->md;
+  dim3 g1((md.b + 255) / 256, md.b, 1);
+  assemble_blocks_kernel<<<g1, 256, 0, st>>>(md, c->P, kind, which == BTA_COND, c->cnt, out, 0, t);
+  BTA_COUNT(c);
   return cudaGetLastError();
 }
 

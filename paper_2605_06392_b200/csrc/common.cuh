@@ -134,6 +134,7 @@ struct bta_ctx {
   void* graph_ws;                    // workspace pointer the cached graph was captured with
   long long graph_launches;          // kernels inside the cached graph
   long long grad_calls;
+  int store_mode;                    // BTA_STORE_FACTOR / BTA_STORE_CARRY
   cudaEvent_t ev[16];
   long long launches;
   long long last_pivot;
@@ -153,6 +154,8 @@ cudaError_t launch_assemble(bta_ctx* c, int which, double* D, long long d_stride
                             double* C, long long c_stride, double* T, int ldt, double* rhs, long long rhs_stride,
                             double* rhs_tip, int rhs_tip_stride, cudaStream_t st);
 cudaError_t run_setup_aggregates(bta_ctx* c, cudaStream_t st);
+// One sub-diagonal block B_t (kind 1) or diagonal block D_t (kind 0) into `out` (b x b).
+cudaError_t launch_assemble_block(bta_ctx* c, int which, int kind, int t, double* out, cudaStream_t st);
 
 // contract.cu -- layout of the small device scratch (offsets in doubles into bta_ctx::small)
 struct SmallLayout {

@@ -89,6 +89,7 @@ extern "C" int bta_create(bta_ctx** out, const bta_model_desc* desc, const bta_o
   c->graph_ws = nullptr;
   c->graph_launches = 0;
   c->grad_calls = 0;
+  c->store_mode = BTA_STORE_FACTOR;
   for (auto& e : c->ev) BTA_CUDA_OK(cudaEventCreate(&e));
   if (m > 0) {
     BTA_CUDA_OK(cudaMemcpy(c->o_var, obs->var, m * sizeof(int), cudaMemcpyHostToDevice));
@@ -134,3 +135,17 @@ extern "C" int32_t bta_num_hyper(const bta_ctx* c) { return c ? c->md.d : 0; }
 extern "C" int64_t bta_latent_size(const bta_ctx* c) { return c ? c->md.N : 0; }
 extern "C" int64_t bta_last_pivot(const bta_ctx* c) { return c ? c->last_pivot : 0; }
 extern "C" int64_t bta_kernel_launches(const bta_ctx* c) { return c ? c->launches : 0; }
+
+extern "C" int bta_set_store_mode(bta_ctx* c, int mode) {
+  if (!c || (mode != BTA_STORE_FACTOR && mode != BTA_STORE_CARRY)) {
+    bta_set_error("bta_set_store_mode: null ctx or unknown mode");
+    return BTA_ERR_ARG;
+  }
+  if (mode != c->store_mode && c->graph_exec) {  // a cached graph was captured for the other layout
+    cudaGraphExecDestroy(c->graph_exec);
+    c->graph_exec = nullptr;
+  }
+  c->store_mode = mode;
+  return BTA_OK;
+}
+extern "C" int bta_get_store_mode(const bta_ctx* c) { return c ? c->store_mode : -1; }

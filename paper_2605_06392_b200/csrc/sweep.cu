@@ -83,60 +83,78 @@ cudaError_t chain_forward_step(Chain& ch, int t, cudaStream_t st) {
   bta_ctx* c = ch.c;
   const int b = ch.b, nt = ch.nt, a = ch.a, P = ch.P(), ldt = a + ch.nr;
   const long long bb = (long long)b * b;
-  {
-    double* Dt = ch.D + t * ch.d_stride;
-    if (ch.zero_upper && ch.factor_blocks) {
-      CK(launch_zero_upper(Dt, b, b, st));
+  double* At = ch.D + t * ch.d_stride;           // D_t - S_{t-1}
+  double* Dt = ch.carry ? ch.Xs : At;            // where X_t = L_Dt^-1 is built
+  const double* LBprev = ch.carry ? ch.LBs : (t > 0 ? ch.Bout + (t - 1) * ch.b_stride : nullptr);
+  // stack rows: arrow rows (factor mode) then right-hand-side rows.
+  //   R~_t = R_t - R^_{t-1} L_B{t-1}^T  (lines 4-5), done first: in carry mode L_B{t-1} is overwritten below
+  const double* src = nullptr;
+  int ld_src = 0;
+  if (P > 0) {
+    src = ch.Rin + t * ch.rin_stride;
+    ld_src = ch.ld_rin;
+    if (t == 0 && ch.Rin == ch.Rout) {  // in-place factor: the stack product below must not alias its input
+      CK(cudaMemcpy2DAsync(ch.Rtmp, b * sizeof(double), src, ld_src * sizeof(double), b * sizeof(double), P,
+                           cudaMemcpyDeviceToDevice, st));
+      src = ch.Rtmp;
+      ld_src = b;
+    }
+    if (t > 0) {
+      double* tmp = ch.Rtmp ? ch.Rtmp : ch.Rin + t * ch.rin_stride;
+      const int ld_tmp = ch.Rtmp ? b : ch.ld_rin;
+      CK(launch_skinny_nt(P, b, b, ch.Rout + (t - 1) * ch.rout_stride, ch.ld_rout, LBprev, b, 0, -1.0, 1.0, src, ld_src,
+                          tmp, ld_tmp, st));
+      BTA_COUNT(c);
+      src = tmp;
+      ld_src = ld_tmp;
+    }
+  }
+  if (ch.factor_blocks) {
+    if (ch.zero_upper) {
+      CK(launch_zero_upper(At, b, b, st));
       BTA_COUNT(c);
     }
-    if (ch.factor_blocks)
-      CK(potrf_inv(c, Dt, b, 0, b, ch.W2, ch.W3, ch.dvec ? ch.dvec + (long long)t * b : nullptr, (long long)t * b,
-                   st));
-    if (P > 0) {
-      // stack rows: arrow rows (factor mode) then right-hand-side rows.
-      //   R~_t = R_t - R^_{t-1} L_B{t-1}^T  (lines 4-5);   R^_t = R~_t X_t^T
-      const double* src = ch.Rin + t * ch.rin_stride;
-      int ld_src = ch.ld_rin;
-      if (t == 0 && ch.Rin == ch.Rout) {  // in-place factor: the stack product below must not alias its input
-        CK(cudaMemcpy2DAsync(ch.Rtmp, b * sizeof(double), src, ld_src * sizeof(double), b * sizeof(double), P,
-                             cudaMemcpyDeviceToDevice, st));
-        src = ch.Rtmp;
-        ld_src = b;
-      }
-      if (t > 0) {
-        double* tmp = ch.Rtmp ? ch.Rtmp : ch.Rin + t * ch.rin_stride;
-        const int ld_tmp = ch.Rtmp ? b : ch.ld_rin;
-        CK(launch_skinny_nt(P, b, b, ch.Rout + (t - 1) * ch.rout_stride, ch.ld_rout, ch.Bout + (t - 1) * ch.b_stride, b,
-                            0, -1.0, 1.0, src, ld_src, tmp, ld_tmp, st));
+    if (ch.carry) {  // the carry D_t - S_{t-1} stays in its slot; factor a copy
+      CK(cudaMemcpyAsync(Dt, At, bb * sizeof(double), cudaMemcpyDeviceToDevice, st));
+      CK(potrf_inv(c, Dt, b, 0, b, ch.W1, ch.Bs, ch.dvec ? ch.dvec + (long long)t * b : nullptr, (long long)t * b, st));
+    } else {
+      CK(potrf_inv(c, Dt, b, 0, b, ch.W2, ch.W3, ch.dvec ? ch.dvec + (long long)t * b : nullptr, (long long)t * b, st));
+    }
+  }
+  if (P > 0) {
+    //   R^_t = R~_t X_t^T
+    double* Rh = ch.Rout + t * ch.rout_stride;
+    CK(launch_skinny_nt(P, b, b, src, ld_src, Dt, b, 1, 1.0, 0.0, nullptr, 0, Rh, ch.ld_rout, st));
+    BTA_COUNT(c);
+    if (a > 0) {
+      // T~ -= L_C L_C^T (line 9) and r_T - v_T, v_T += L_C z (line 5): columns [0,a) and [a, a+nr) of Tt
+      if (ch.arrow_rows) {
+        CK(launch_small_nt(a, P, b, Rh, ch.ld_rout, Rh, ch.ld_rout, -1.0, ch.Tt, ldt, st));
         BTA_COUNT(c);
-        src = tmp;
-        ld_src = ld_tmp;
-      }
-      double* Rh = ch.Rout + t * ch.rout_stride;
-      CK(launch_skinny_nt(P, b, b, src, ld_src, Dt, b, 1, 1.0, 0.0, nullptr, 0, Rh, ch.ld_rout, st));
-      BTA_COUNT(c);
-      if (a > 0) {
-        // T~ -= L_C L_C^T (line 9) and r_T - v_T, v_T += L_C z (line 5): columns [0,a) and [a, a+nr) of Tt
-        if (ch.arrow_rows) {
-          CK(launch_small_nt(a, P, b, Rh, ch.ld_rout, Rh, ch.ld_rout, -1.0, ch.Tt, ldt, st));
-          BTA_COUNT(c);
-        } else if (ch.arrow_given) {
-          CK(launch_small_nt(a, ch.nr, b, ch.LCgiven + t * ch.lc_stride, b, Rh, ch.ld_rout, -1.0, ch.Tt + a, ldt, st));
-          BTA_COUNT(c);
-        }
+      } else if (ch.arrow_given) {
+        CK(launch_small_nt(a, ch.nr, b, ch.LCgiven + t * ch.lc_stride, b, Rh, ch.ld_rout, -1.0, ch.Tt + a, ldt, st));
+        BTA_COUNT(c);
       }
     }
-    if (t < nt - 1 && ch.factor_blocks) {
-      double* Bi = ch.Bin + t * ch.b_stride;
-      double* Bo = ch.Bout + t * ch.b_stride;
-      double* dst = (Bi == Bo) ? ch.W1 : Bo;
-      CK(launch_gemm(G(GEMM_NT, b, b, b, 1.0, Bi, b, Dt, b, 0.0, dst, b, KLO_ZERO, KHI_NEND, OUT_FULL), st));
-      CK(launch_gemm(G(GEMM_NT, b, b, b, -1.0, dst, b, dst, b, 1.0, ch.D + (t + 1) * ch.d_stride, b, KLO_ZERO, KHI_K,
-                       OUT_LOWER),
-                     st));
-      c->launches += 2;
-      if (dst != Bo) CK(cudaMemcpyAsync(Bo, dst, bb * sizeof(double), cudaMemcpyDeviceToDevice, st));
+  }
+  if (t < nt - 1 && ch.factor_blocks) {
+    const double* Bi;
+    double *Bo, *dst;
+    if (ch.carry) {
+      CK(launch_assemble_block(c, ch.which, 1, t, ch.Bs, st));
+      Bi = ch.Bs;
+      Bo = dst = ch.LBs;
+    } else {
+      Bi = ch.Bin + t * ch.b_stride;
+      Bo = ch.Bout + t * ch.b_stride;
+      dst = (Bi == Bo) ? ch.W1 : Bo;
     }
+    CK(launch_gemm(G(GEMM_NT, b, b, b, 1.0, Bi, b, Dt, b, 0.0, dst, b, KLO_ZERO, KHI_NEND, OUT_FULL), st));
+    CK(launch_gemm(G(GEMM_NT, b, b, b, -1.0, dst, b, dst, b, 1.0, ch.D + (t + 1) * ch.d_stride, b, KLO_ZERO, KHI_K,
+                     OUT_LOWER),
+                   st));
+    c->launches += 2;
+    if (dst != Bo) CK(cudaMemcpyAsync(Bo, dst, bb * sizeof(double), cudaMemcpyDeviceToDevice, st));
   }
   return cudaSuccess;
 }
@@ -167,8 +185,18 @@ cudaError_t chain_backward_step(Chain& ch, int t, cudaStream_t st) {
   const bool arrow = ch.arrow();
   const int zrow0 = ch.arrow_rows ? a : 0;  // first rhs row inside the Rout stack
   {
-    const double* X = ch.D + t * ch.d_stride;
-    double* LB = (t < nt - 1) ? ch.Bout + t * ch.b_stride : nullptr;
+    if (ch.carry) {
+      // carry-based reconstruction: X_t from the stored D_t - S_{t-1}, L_Bt from the re-assembled B_t
+      CK(cudaMemcpyAsync(ch.Xs, ch.D + t * ch.d_stride, bb * sizeof(double), cudaMemcpyDeviceToDevice, st));
+      CK(potrf_inv(c, ch.Xs, b, 0, b, ch.W1, ch.Bs, nullptr, (long long)t * b, st));
+      if (t < nt - 1) {
+        CK(launch_assemble_block(c, ch.which, 1, t, ch.Bs, st));
+        CK(launch_gemm(G(GEMM_NT, b, b, b, 1.0, ch.Bs, b, ch.Xs, b, 0.0, ch.LBs, b, KLO_ZERO, KHI_NEND, OUT_FULL), st));
+        BTA_COUNT(c);
+      }
+    }
+    const double* X = ch.carry ? ch.Xs : ch.D + t * ch.d_stride;
+    double* LB = (t < nt - 1) ? (ch.carry ? ch.LBs : ch.Bout + t * ch.b_stride) : nullptr;
     const double* LC = nullptr;
     int ld_lc = b;
     if (ch.arrow_rows) {

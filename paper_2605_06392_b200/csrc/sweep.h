@@ -15,6 +15,8 @@ struct Chain {
   bool selinv = false;         // backward: selected inversion
   bool contract = false;       // backward: accumulate the Eq. 7 traces per block (fused gradient)
   bool selinv_inplace = false; // backward: copy Z_D / Z_C back over D / C (bta_selinv)
+  bool carry = false;          // carry mode (a7): D(t) keeps D_t - S_{t-1}; X_t, L_Bt live in Xs / LBs and are rebuilt
+  int which = BTA_COND;        // carry mode: which matrix B_t is re-assembled for
 
   int P() const { return (arrow_rows ? a : 0) + nr; }
   bool arrow() const { return arrow_rows || arrow_given; }
@@ -30,6 +32,7 @@ struct Chain {
   const double* rhs_tip = nullptr; int rhs_tip_stride = 0;              // rhs_tip[r * stride + p]
   // scratch
   double *W1 = nullptr, *W2 = nullptr, *W3 = nullptr;                   // b x b each
+  double *Xs = nullptr, *LBs = nullptr, *Bs = nullptr;                  // carry mode: X_t, L_Bt, assembled B_t
   double* part = nullptr;                                               // skinny_nn partial sums
   double *ubuf = nullptr, *Ebuf = nullptr, *Ybuf = nullptr;             // [nr][b], [a][b], [a][b]
   double* ZC[2] = {nullptr, nullptr};                                   // [a][b] ping-pong

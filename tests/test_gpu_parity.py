@@ -68,6 +68,30 @@ def test_value_and_grad_parity(name):
     assert st["total"] > 0
 
 
+@pytest.mark.parametrize("name", ["w0", "b81_two_tiles", "b144_h07", "nt1", "nt2", "mv_k2_b162", "mv_k3_b300", "cfg1"])
+def test_carry_mode_matches_oracle_and_factor_mode(name):
+    """Storage policy a7: carry-based reconstruction gives the same f, grad with about half the
+    block storage."""
+    model, obs, th = CASES[name]()
+    ref = O.value_and_grad(model, obs, th)
+    M = _model(model, obs)
+    ws_factor = M.workspace_bytes()
+    f0, g0 = M.inla_value_and_grad(th)
+    M.bta_set_store_mode(1)
+    assert M.bta_get_store_mode() == 1
+    ws_carry = M.workspace_bytes()
+    f1, g1 = M.inla_value_and_grad(th)
+    f2, g2 = M.inla_value_and_grad(th)          # second call: CUDA-graph replay of the carry-mode sweep
+    im = M.last_intermediates()
+    M.close()
+    assert f1 == f2 and np.array_equal(g1, g2)
+    assert abs(f1 - ref["f"]) <= TOL_F * abs(ref["f"]) and grad_ok(g1, ref["grad"])
+    assert abs(f1 - f0) <= 1e-12 * abs(f0) and np.max(np.abs(g1 - g0)) <= 1e-10 * np.max(np.abs(g0))
+    assert abs(im["ld_c"] - ref["ld_c"]) <= TOL_F * abs(ref["ld_c"])
+    if model.nt >= 8:
+        assert ws_carry < 0.62 * ws_factor       # nt carries + 6 scratch blocks vs 2 nt + 3
+
+
 def test_w0_printed_digits(golden):
     g = golden("w0.txt")
     model, obs, th = make_w0()
