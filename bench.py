@@ -253,6 +253,26 @@ def run_ours(args):
     line["roofline_step"] = {"bound": "tensor", "achieved": line["fp64"]["achieved_tflops"], "peak": peak_tf,
                              "unit": "TFLOP/s", "frac": line["fp64"]["achieved_tflops"] / peak_tf,
                              "note": "algorithmic flops of one gradient (14 nt b^3) / step time"}
+    # ---- the paper's comparison: one exact gradient against a
+    #      central finite-difference gradient = 2d+1 objective evaluations (inla_value), same kernels, same GPU
+    if not args.no_fd:
+        for _ in range(2):
+            M.inla_value(thetas[0])
+        v0, v1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        v0.record()
+        for i in range(args.steps):
+            M.inla_value(thetas[args.warmup + i])
+        v1.record()
+        torch.cuda.synchronize()
+        t_eval = v0.elapsed_time(v1) / args.steps
+        fwd = stage_acc.get("fwd_Qc", 0.0) + stage_acc.get("fwd_Qp", 0.0)
+        bwd = stage_acc.get("bwd_Qc", 0.0) + stage_acc.get("bwd_Qp", 0.0)
+        line["fd_compare"] = {"t_eval_ms": t_eval, "t_ad_ms": ms_step, "c_ad": ms_step / t_eval,
+                              "fd_gradient_ms": (2 * d + 1) * t_eval,
+                              "speedup_ad_vs_fd": (2 * d + 1) * t_eval / ms_step,
+                              "beta_bwd_over_fwd": (bwd / fwd) if fwd > 0 else None,
+                              "note": "FD gradient = (2d+1) x inla_value (Eq. 2); paper reports 4.2-7.9x per-gradient "
+                                      "speedup and c_AD 2.3-3.9 on GH200 (context only, BASELINE.md)"}
     if rank == 0 and not args.no_cpu_baseline and world == 1:
         nt_s = {0: 6, 1: 10, 2: 4, 3: 2, 4: 2}[args.config]
         dt, est, nts, _ = oracle_sample(args.config, nt_s)
@@ -275,6 +295,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=4)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-fd", action="store_true", help="skip the finite-difference comparison (NEXT-1)")
     ap.add_argument("--store", default="factor", choices=["factor", "carry"],
                     help="storage policy a7: keep the factor blocks (default) or only the Schur carries")
     ap.add_argument("--nt", type=int, default=None,

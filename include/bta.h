@@ -131,6 +131,20 @@ int bta_selinv(bta_ctx* ctx, bta_blocks inout, int which, void* ws, void* stream
 int inla_value_and_grad(bta_ctx* ctx, const double* theta, double* f, double* grad, double* stage_ms, void* ws,
                         void* stream);
 
+/* the objective alone (Eq. 1): assemble -> factor Q_c and Q_p -> solve ->
+ * scalars; no selected inversion, no contractions.  One evaluation of the finite-difference baseline. */
+int inla_value(bta_ctx* ctx, const double* theta, double* f, void* ws, void* stream);
+
+/* Central finite-difference gradient (Eq. 2; the DALIA baseline): 2d+1 calls of inla_value with
+ * step h (the paper uses 1e-3).  f (may be NULL) receives f(theta), grad HOST [d].  Truncation error O(h^2). */
+int inla_fd_grad(bta_ctx* ctx, const double* theta, double h, double* f, double* grad, void* ws, void* stream);
+
+/* posterior Hessian by central differences of the exact gradient (Eq. 13):
+ * H[:, j] = (grad f(theta + h e_j) - grad f(theta - h e_j)) / (2h), 2d+1 calls of inla_value_and_grad (the centre
+ * call returns f and grad, either may be NULL).  H HOST [d][d], as differenced (not symmetrised). */
+int inla_hessian(bta_ctx* ctx, const double* theta, double h, double* f, double* grad, double* H, void* ws,
+                 void* stream);
+
 enum {
   BTA_STAGE_ASSEMBLE = 0,
   BTA_STAGE_FWD_QC = 1,

@@ -59,6 +59,9 @@ def lib():
     L.bta_solve.argtypes = [vp, _Blocks, i32, vp, i32, vp, vp]
     L.bta_selinv.argtypes = [vp, _Blocks, i32, vp, vp]
     L.inla_value_and_grad.argtypes = [vp, dp, dp, dp, dp, vp, vp]
+    L.inla_value.argtypes = [vp, dp, dp, vp, vp]
+    L.inla_fd_grad.argtypes = [vp, dp, C.c_double, dp, dp, vp, vp]
+    L.inla_hessian.argtypes = [vp, dp, C.c_double, dp, dp, dp, vp, vp]
     L.bta_last_intermediates.argtypes = [vp, dp, dp, dp, dp, dp, dp]
     L.bta_num_hyper.argtypes = [vp]
     L.bta_num_hyper.restype = C.c_int32
@@ -215,6 +218,31 @@ class BtaModel:
         if stages:
             return f.value, grad, dict(zip(STAGES, st.tolist()))
         return f.value, grad
+
+    def inla_value(self, theta):
+        th = np.ascontiguousarray(theta, dtype=np.float64)
+        f = C.c_double()
+        _check(lib().inla_value(self._h, _dptr(th), C.byref(f), self._workspace().data_ptr(), _stream()))
+        return f.value
+
+    def inla_fd_grad(self, theta, h=1e-3):
+        """Central finite differences of inla_value (Eq. 2): 2d+1 evaluations."""
+        th = np.ascontiguousarray(theta, dtype=np.float64)
+        f = C.c_double()
+        g = np.zeros(self.d)
+        _check(lib().inla_fd_grad(self._h, _dptr(th), float(h), C.byref(f), _dptr(g), self._workspace().data_ptr(),
+                                  _stream()))
+        return f.value, g
+
+    def inla_hessian(self, theta, h=5e-3):
+        """Central differences of the exact gradient (Eq. 13): 2d+1 gradient calls."""
+        th = np.ascontiguousarray(theta, dtype=np.float64)
+        f = C.c_double()
+        g = np.zeros(self.d)
+        H = np.zeros((self.d, self.d))
+        _check(lib().inla_hessian(self._h, _dptr(th), float(h), C.byref(f), _dptr(g), _dptr(H),
+                                  self._workspace().data_ptr(), _stream()))
+        return f.value, g, H
 
     def last_intermediates(self, want_x=True):
         ld = np.zeros(2)

@@ -299,7 +299,7 @@ namespace {
 
 // Enqueue one whole gradient: theta upload -> both chains (interleaved on s0 / s1) -> scalar assembly -> result
 // download into pinned host memory.  With `timed` the stage events are recorded (not capturable in a graph).
-int enqueue_gradient(bta_ctx* c, void* ws, cudaStream_t s0, cudaStream_t s1, bool timed) {
+int enqueue_gradient(bta_ctx* c, void* ws, cudaStream_t s0, cudaStream_t s1, bool timed, bool value_only) {
   const ModelDims& md = c->md;
   const bool serial = (s0 == s1);
   Bump bp(ws);
@@ -331,7 +331,7 @@ int enqueue_gradient(bta_ctx* c, void* ws, cudaStream_t s0, cudaStream_t s1, boo
   cc.a = md.a;
   cc.nr = 1;
   cc.arrow_rows = true;
-  cc.selinv = cc.contract = true;
+  cc.selinv = cc.contract = !value_only;
   cc.D = wc.D;
   cc.d_stride = bb;
   cc.carry = carry;
@@ -379,7 +379,7 @@ int enqueue_gradient(bta_ctx* c, void* ws, cudaStream_t s0, cudaStream_t s1, boo
   cp.nt = md.nt;
   cp.a = md.a;
   cp.nr = 0;
-  cp.selinv = cp.contract = true;
+  cp.selinv = cp.contract = !value_only;
   cp.D = wp.D;
   cp.d_stride = bb;
   cp.carry = carry;
@@ -422,8 +422,8 @@ int enqueue_gradient(bta_ctx* c, void* ws, cudaStream_t s0, cudaStream_t s1, boo
   BTA_CUDA_OK(launch_logdet_partial(c, CH_PRIOR, wp.dvec, s1));
   REC(6, s1);
   for (int t = md.nt - 1; t >= 0; --t) {
-    BTA_CUDA_OK(chain_backward_step(cc, t, s0));
-    BTA_CUDA_OK(chain_backward_step(cp, t, s1));
+    BTA_CUDA_OK(chain_backward_step(cc, t, s0));                  // value only: just the upper solve (Eqs. 3-5)
+    if (!value_only) BTA_CUDA_OK(chain_backward_step(cp, t, s1));
   }
   BTA_CUDA_OK(cudaMemcpyAsync(wc.x + (long long)md.nt * md.b, cc.xT, md.a * sizeof(double), cudaMemcpyDeviceToDevice,
                               s0));
@@ -447,9 +447,10 @@ int enqueue_gradient(bta_ctx* c, void* ws, cudaStream_t s0, cudaStream_t s1, boo
 
 }  // namespace
 
-extern "C" int inla_value_and_grad(bta_ctx* c, const double* theta, double* f, double* grad, double* stage_ms,
-                                   void* ws, void* stream) {
-  if (!c || !theta || !ws) return bad("inla_value_and_grad: null ctx, theta or workspace");
+namespace {
+int value_and_grad_impl(bta_ctx* c, const double* theta, double* f, double* grad, double* stage_ms, void* ws,
+                        void* stream, bool value_only) {
+  const int gi = value_only ? 1 : 0;
   cudaStream_t s0 = (cudaStream_t)stream;
   const ModelDims& md = c->md;
   BTA_CUDA_OK(cudaSetDevice(c->device));
@@ -464,42 +465,42 @@ extern "C" int inla_value_and_grad(bta_ctx* c, const double* theta, double* f, d
   cudaStream_t sync_stream = s0;
   bool timed = true;
   if (want_graph && !serial && c->grad_calls > 0) {
-    if (!c->graph_exec || c->graph_ws != ws) {
-      if (c->graph_exec) {
-        cudaGraphExecDestroy(c->graph_exec);
-        c->graph_exec = nullptr;
+    if (!c->graph_exec[gi] || c->graph_ws[gi] != ws) {
+      if (c->graph_exec[gi]) {
+        cudaGraphExecDestroy(c->graph_exec[gi]);
+        c->graph_exec[gi] = nullptr;
       }
       const long long n0 = c->launches;
       cudaGraph_t graph = nullptr;
       BTA_CUDA_OK(cudaStreamBeginCapture(c->s_main, cudaStreamCaptureModeThreadLocal));
-      int rc = enqueue_gradient(c, ws, c->s_main, c->s_side, false);
+      int rc = enqueue_gradient(c, ws, c->s_main, c->s_side, false, value_only);
       cudaError_t ce = cudaStreamEndCapture(c->s_main, &graph);
       if (rc != BTA_OK) return rc;
       BTA_CUDA_OK(ce);
-      BTA_CUDA_OK(cudaGraphInstantiate(&c->graph_exec, graph, 0));
+      BTA_CUDA_OK(cudaGraphInstantiate(&c->graph_exec[gi], graph, 0));
       cudaGraphDestroy(graph);
-      c->graph_ws = ws;
-      c->graph_launches = c->launches - n0;
+      c->graph_ws[gi] = ws;
+      c->graph_launches[gi] = c->launches - n0;
       c->launches = n0;
     }
     BTA_CUDA_OK(cudaEventRecord(ev[11], s0));
     BTA_CUDA_OK(cudaStreamWaitEvent(c->s_main, ev[11], 0));
     BTA_CUDA_OK(cudaEventRecord(ev[0], c->s_main));
-    BTA_CUDA_OK(cudaGraphLaunch(c->graph_exec, c->s_main));
+    BTA_CUDA_OK(cudaGraphLaunch(c->graph_exec[gi], c->s_main));
     BTA_CUDA_OK(cudaEventRecord(ev[8], c->s_main));
     BTA_CUDA_OK(cudaStreamWaitEvent(s0, ev[8], 0));
-    c->launches += c->graph_launches;
+    c->launches += c->graph_launches[gi];
     sync_stream = c->s_main;
     timed = false;
   } else {
-    int rc = enqueue_gradient(c, ws, s0, serial ? s0 : c->s_side, true);
+    int rc = enqueue_gradient(c, ws, s0, serial ? s0 : c->s_side, true, value_only);
     if (rc != BTA_OK) return rc;
   }
   c->grad_calls++;
   int rc = check_pivot(c, sync_stream);  // synchronises the stream (and, through ev[7], the side stream)
   const double* o = c->host_pinned + 64;
   if (f) *f = o[0];
-  if (grad) memcpy(grad, o + 1, md.d * sizeof(double));
+  if (grad && !value_only) memcpy(grad, o + 1, md.d * sizeof(double));
   c->last_ld[0] = o[1 + md.d];
   c->last_ld[1] = o[1 + md.d + 1];
   c->last_parts.assign(o + 1 + md.d + 2, o + 1 + md.d + 2 + 3 * md.d);
@@ -525,6 +526,62 @@ extern "C" int inla_value_and_grad(bta_ctx* c, const double* theta, double* f, d
     stage_ms[BTA_STAGE_TOTAL] = el(0, 8);
   }
   return rc;
+}
+}  // namespace
+
+extern "C" int inla_value_and_grad(bta_ctx* c, const double* theta, double* f, double* grad, double* stage_ms,
+                                   void* ws, void* stream) {
+  if (!c || !theta || !ws) return bad("inla_value_and_grad: null ctx, theta or workspace");
+  return value_and_grad_impl(c, theta, f, grad, stage_ms, ws, stream, false);
+}
+
+extern "C" int inla_value(bta_ctx* c, const double* theta, double* f, void* ws, void* stream) {
+  if (!c || !theta || !ws) return bad("inla_value: null ctx, theta or workspace");
+  return value_and_grad_impl(c, theta, f, nullptr, nullptr, ws, stream, true);
+}
+
+extern "C" int inla_fd_grad(bta_ctx* c, const double* theta, double h, double* f, double* grad, void* ws,
+                            void* stream) {
+  if (!c || !theta || !ws || !grad) return bad("inla_fd_grad: null ctx, theta, grad or workspace");
+  if (!(h > 0.0)) return bad("inla_fd_grad: h must be positive");
+  const int d = c->md.d;
+  std::vector<double> th(theta, theta + d);
+  double f0 = 0.0;
+  int rc = value_and_grad_impl(c, th.data(), &f0, nullptr, nullptr, ws, stream, true);
+  if (rc != BTA_OK) return rc;
+  if (f) *f = f0;
+  for (int j = 0; j < d; ++j) {
+    double fp = 0.0, fm = 0.0;
+    th[j] = theta[j] + h;
+    if ((rc = value_and_grad_impl(c, th.data(), &fp, nullptr, nullptr, ws, stream, true)) != BTA_OK) return rc;
+    th[j] = theta[j] - h;
+    if ((rc = value_and_grad_impl(c, th.data(), &fm, nullptr, nullptr, ws, stream, true)) != BTA_OK) return rc;
+    th[j] = theta[j];
+    grad[j] = (fp - fm) / (2.0 * h);
+  }
+  return BTA_OK;
+}
+
+extern "C" int inla_hessian(bta_ctx* c, const double* theta, double h, double* f, double* grad, double* H, void* ws,
+                            void* stream) {
+  if (!c || !theta || !ws || !H) return bad("inla_hessian: null ctx, theta, H or workspace");
+  if (!(h > 0.0)) return bad("inla_hessian: h must be positive");
+  const int d = c->md.d;
+  std::vector<double> th(theta, theta + d), gp(d), gm(d), g0(d);
+  double f0 = 0.0;
+  int rc = value_and_grad_impl(c, th.data(), &f0, g0.data(), nullptr, ws, stream, false);
+  if (rc != BTA_OK) return rc;
+  if (f) *f = f0;
+  if (grad) memcpy(grad, g0.data(), d * sizeof(double));
+  for (int j = 0; j < d; ++j) {
+    th[j] = theta[j] + h;
+    if ((rc = value_and_grad_impl(c, th.data(), nullptr, gp.data(), nullptr, ws, stream, false)) != BTA_OK) return rc;
+    th[j] = theta[j] - h;
+    if ((rc = value_and_grad_impl(c, th.data(), nullptr, gm.data(), nullptr, ws, stream, false)) != BTA_OK) return rc;
+    th[j] = theta[j];
+    for (int i = 0; i < d; ++i) H[i * d + j] = (gp[i] - gm[i]) / (2.0 * h);
+  }
+  return BTA_OK;
 }
 
 extern "C" int bta_last_intermediates(bta_ctx* c, double* ld, double* x, double* parts, double* rss, double* quad,

@@ -130,9 +130,9 @@ struct bta_ctx {
   double* host_pinned;               // pinned host staging (theta in, f/grad/intermediates out)
   cudaStream_t s_side;               // second chain's stream
   cudaStream_t s_main;               // graph mode: the captured/replayed stream (the caller's may be stream 0)
-  cudaGraphExec_t graph_exec;        // cached replay of one whole gradient (small models), or nullptr
-  void* graph_ws;                    // workspace pointer the cached graph was captured with
-  long long graph_launches;          // kernels inside the cached graph
+  cudaGraphExec_t graph_exec[2];     // cached replay of one whole gradient [0] / value-only pass [1], or nullptr
+  void* graph_ws[2];                 // workspace pointer the cached graph was captured with
+  long long graph_launches[2];       // kernels inside the cached graph
   long long grad_calls;
   int store_mode;                    // BTA_STORE_FACTOR / BTA_STORE_CARRY
   cudaEvent_t ev[16];

@@ -5,6 +5,8 @@
 // L^-1 built so far (forward elimination applied to the identity) and the columns j > k hold the Schur
 // complement.  Output: X = L^-1 (lower; strict upper of the tile zeroed), diag(L) for the log-determinant
 // (PAPER.md:48), and the first non-positive pivot (Algorithm 1 line 3 needs D_i - S_{i-1} > 0).
+#include <cstdlib>
+
 #include "common.cuh"
 
 namespace {

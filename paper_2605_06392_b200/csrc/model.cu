@@ -85,9 +85,11 @@ extern "C" int bta_create(bta_ctx** out, const bta_model_desc* desc, const bta_o
   BTA_CUDA_OK(cudaMallocHost((void**)&c->host_pinned, 4096 * sizeof(double)));
   BTA_CUDA_OK(cudaStreamCreateWithFlags(&c->s_side, cudaStreamNonBlocking));
   BTA_CUDA_OK(cudaStreamCreateWithFlags(&c->s_main, cudaStreamNonBlocking));
-  c->graph_exec = nullptr;
-  c->graph_ws = nullptr;
-  c->graph_launches = 0;
+  for (int q = 0; q < 2; ++q) {
+    c->graph_exec[q] = nullptr;
+    c->graph_ws[q] = nullptr;
+    c->graph_launches[q] = 0;
+  }
   c->grad_calls = 0;
   c->store_mode = BTA_STORE_FACTOR;
   for (auto& e : c->ev) BTA_CUDA_OK(cudaEventCreate(&e));
@@ -123,7 +125,8 @@ extern "C" int bta_destroy(bta_ctx* c) {
   cudaFree(c->pivot_flag);
   cudaFree(c->small);
   cudaFreeHost(c->host_pinned);
-  if (c->graph_exec) cudaGraphExecDestroy(c->graph_exec);
+  for (int q = 0; q < 2; ++q)
+    if (c->graph_exec[q]) cudaGraphExecDestroy(c->graph_exec[q]);
   cudaStreamDestroy(c->s_side);
   cudaStreamDestroy(c->s_main);
   for (auto& e : c->ev) cudaEventDestroy(e);
@@ -141,10 +144,11 @@ extern "C" int bta_set_store_mode(bta_ctx* c, int mode) {
     bta_set_error("bta_set_store_mode: null ctx or unknown mode");
     return BTA_ERR_ARG;
   }
-  if (mode != c->store_mode && c->graph_exec) {  // a cached graph was captured for the other layout
-    cudaGraphExecDestroy(c->graph_exec);
-    c->graph_exec = nullptr;
-  }
+  for (int q = 0; q < 2; ++q)
+    if (mode != c->store_mode && c->graph_exec[q]) {  // a cached graph was captured for the other layout
+      cudaGraphExecDestroy(c->graph_exec[q]);
+      c->graph_exec[q] = nullptr;
+    }
   c->store_mode = mode;
   return BTA_OK;
 }

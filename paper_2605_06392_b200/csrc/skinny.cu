@@ -4,22 +4,23 @@
 // recurrences (R10).  P <= 16 rows; each kernel reads the b x b block exactly once (HBM roofline).
 #include "common.cuh"
 
-constexpr int NN_KCH = 128;  // rows of M per CTA of skinny_nn (one partial sum each)
+constexpr int NN_KCH = 128;
+constexpr int NT_RPW = 2;   // rows of M per warp in skinny_nt (8 warps per CTA)  // rows of M per CTA of skinny_nn (one partial sum each)
 
 namespace {
 
 // out[p][j] = beta * in[p][j] + alpha * sum_{k < kend(j)} R[p][k] * M[j][k],  kend(j) = tri ? j+1 : K.
-// One warp per 4 rows j of M (k contiguous -> coalesced); the R chunk is staged in shared memory.
+// One warp per NT_RPW rows j of M (k contiguous -> coalesced); the R chunk is staged in shared memory.
 template <int PT>
 __global__ void __launch_bounds__(256) skinny_nt_kernel(int P, int J, int K, const double* __restrict__ R, int ldr,
                                                         const double* __restrict__ M, int ldm, int tri,
                                                         double alpha, double beta, const double* __restrict__ in,
                                                         int ldin, double* __restrict__ out, int ldo) {
-  constexpr int KC = 256, RPW = 4;
+  constexpr int KC = 256, RPW = NT_RPW;
   __shared__ double Rs[PT * KC];
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const int jbase = blockIdx.x * 32 + warp * RPW;
-  const int jmax_cta = min(J, blockIdx.x * 32 + 32) - 1;
+  const int jbase = blockIdx.x * (8 * RPW) + warp * RPW;
+  const int jmax_cta = min(J, (int)(blockIdx.x + 1) * (8 * RPW)) - 1;
   const int Kcta = tri ? min(K, jmax_cta + 1) : K;
   double acc[RPW][PT];
 #pragma unroll
@@ -168,11 +169,13 @@ cudaError_t launch_skinny_nt(int P, int J, int K, const double* R, int ldr, cons
                              double alpha, double beta, const double* in, int ldin, double* out, int ldo,
                              cudaStream_t st) {
   if (P <= 0 || J <= 0) return cudaSuccess;
-  dim3 grid((J + 31) / 32);
+  dim3 grid((J + 8 * NT_RPW - 1) / (8 * NT_RPW));
   if (P <= 1)
     skinny_nt_kernel<1><<<grid, 256, 0, st>>>(P, J, K, R, ldr, M, ldm, tri, alpha, beta, in, ldin, out, ldo);
-  else if (P <= 8)
-    skinny_nt_kernel<8><<<grid, 256, 0, st>>>(P, J, K, R, ldr, M, ldm, tri, alpha, beta, in, ldin, out, ldo);
+  else if (P <= 4)
+    skinny_nt_kernel<4><<<grid, 256, 0, st>>>(P, J, K, R, ldr, M, ldm, tri, alpha, beta, in, ldin, out, ldo);
+  else if (P <= 9)
+    skinny_nt_kernel<9><<<grid, 256, 0, st>>>(P, J, K, R, ldr, M, ldm, tri, alpha, beta, in, ldin, out, ldo);
   else if (P <= 16)
     skinny_nt_kernel<16><<<grid, 256, 0, st>>>(P, J, K, R, ldr, M, ldm, tri, alpha, beta, in, ldin, out, ldo);
   else

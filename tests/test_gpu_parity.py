@@ -210,3 +210,35 @@ def test_gemm_kernel_modes():
     assert np.max(np.abs(gemm(0, t(L), t(Bm), z(), khi=2).cpu().numpy() - L @ Bm)) < 1e-11
     assert np.max(np.abs(gemm(2, t(L), t(L), z(), klo=2, out=2).cpu().numpy() - L.T @ L)) < 1e-11
     assert np.max(np.abs(gemm(1, t(Bm), t(Bm), z(), out=1).cpu().numpy() - np.tril(Bm @ Bm.T))) < 1e-11
+
+
+@pytest.mark.parametrize("name", ["w0", "b81_two_tiles", "mv_k3_tiny", "mv_k2_b162"])
+def test_value_fd_gradient_and_hessian(name):
+    """value-only pass, the finite-difference baseline (Eq. 2) and the Hessian by
+    differences of exact gradients (Eq. 13), against the same quantities formed from the oracle."""
+    model, obs, th = CASES[name]()
+    ref = O.value_and_grad(model, obs, th)
+    M = _model(model, obs)
+    assert abs(M.inla_value(th) - ref["f"]) <= TOL_F * abs(ref["f"])
+    h = 1e-3
+    f0, gfd = M.inla_fd_grad(th, h)
+    assert abs(f0 - ref["f"]) <= TOL_F * abs(ref["f"])
+    gfd_ref = np.zeros(model.d)
+    for j in range(model.d):
+        e = np.zeros(model.d)
+        e[j] = h
+        gfd_ref[j] = (O.dense_objective(model, obs, th + e)["f"] - O.dense_objective(model, obs, th - e)["f"]) / (2 * h)
+    scale = np.max(np.abs(ref["grad"]))
+    assert np.max(np.abs(gfd - gfd_ref)) <= 1e-6 * scale             # same differences, f to 1e-9 relative
+    assert np.max(np.abs(gfd - ref["grad"])) <= 2e-4 * scale          # O(h^2) truncation (PAPER.md:258)
+    hh = 5e-3
+    f1, g1, H = M.inla_hessian(th, hh)
+    M.close()
+    assert abs(f1 - ref["f"]) <= TOL_F * abs(ref["f"]) and grad_ok(g1, ref["grad"])
+    Href = np.zeros((model.d, model.d))
+    for j in range(model.d):
+        e = np.zeros(model.d)
+        e[j] = hh
+        Href[:, j] = (O.value_and_grad(model, obs, th + e)["grad"] - O.value_and_grad(model, obs, th - e)["grad"]) / (2 * hh)
+    assert np.max(np.abs(H - Href)) <= 1e-6 * np.max(np.abs(Href))
+    assert np.max(np.abs(H - H.T)) <= 1e-3 * np.max(np.abs(H))       # symmetric up to O(h^2)
