@@ -112,7 +112,6 @@ int bad(const char* msg) {
 
 }  // namespace
 
-extern "C" size_t bta_workspace_bytes(const bta_ctx* c) { return c ? grad_ws_bytes(c->md, c->store_mode) : 0; }
 extern "C" size_t bta_workspace_bytes_op(const bta_ctx* c) {
   if (!c) return 0;
   Bump bp(nullptr);
@@ -445,6 +444,258 @@ int enqueue_gradient(bta_ctx* c, void* ws, cudaStream_t s0, cudaStream_t s1, boo
   return BTA_OK;
 }
 
+// ------------------------------------------------------------------------------------------------
+// Two-way (twisted) elimination: time-domain partitioning with P = 2 inside one GPU (PAPER.md:175-183,
+// SURVEY.md §8(f) NEXT-3, first step).  Blocks 0..h-1 are eliminated upwards and blocks nt-1..h+1 downwards
+// (the same chain code on the time-reversed sub-matrix with transposed coupling blocks); both meet at the
+// separator block h, which is eliminated last together with the arrow tip.  No fill-in, the same flops, the
+// same results up to rounding order -- but four independent chains (two per matrix) instead of two, so the
+// latency-bound POTRF phases of one chain overlap the GEMMs of three others.
+struct SubWs {
+  double *B, *W1, *W2, *W3, *Xs, *LBs, *Bs, *ubuf, *Ebuf, *Ybuf, *ZC0, *ZC1, *part;
+};
+struct MatWs {
+  double *D, *dvec, *T, *Rin, *Rout, *x, *rtip, *Tt2;
+  SubWs sub[3];  // up, down, separator
+};
+
+int twist_h(const ModelDims& md) { return md.nt / 2; }
+
+MatWs carve_twist(Bump& bp, const ModelDims& md, bool cond, int store_mode) {
+  MatWs w{};
+  const size_t bb = (size_t)md.b * md.b;
+  const int P = md.a + 1, h = twist_h(md);
+  const int len[3] = {h, md.nt - 1 - h, 1};
+  w.D = bp.take(bb * md.nt);
+  w.dvec = bp.take(md.N);
+  w.T = bp.take(md.a * md.a);
+  w.Tt2 = bp.take(md.a * (md.a + 1));
+  if (cond) {
+    w.Rin = bp.take((size_t)md.nt * P * md.b);
+    w.Rout = bp.take((size_t)md.nt * P * md.b);
+    w.x = bp.take(md.N);
+    w.rtip = bp.take(md.a);
+  }
+  for (int q = 0; q < 3; ++q) {
+    SubWs& s = w.sub[q];
+    s.W1 = bp.take(bb);
+    s.W2 = bp.take(bb);
+    s.W3 = bp.take(bb);
+    if (q < 2) {
+      if (store_mode == BTA_STORE_CARRY) {
+        s.Xs = bp.take(bb);
+        s.LBs = bp.take(bb);
+        s.Bs = bp.take(bb);
+      } else {
+        s.B = bp.take(bb * (len[q] + 1));
+      }
+    }
+    if (cond) {
+      s.ubuf = bp.take(md.b);
+      s.Ebuf = bp.take((size_t)md.a * md.b);
+      s.Ybuf = bp.take((size_t)md.a * md.b);
+      s.ZC0 = bp.take((size_t)md.a * md.b);
+      s.ZC1 = bp.take((size_t)md.a * md.b);
+      s.part = bp.take(skinny_nn_part_doubles(P, md.b, md.b));
+    }
+  }
+  return w;
+}
+
+size_t twist_ws_bytes(const ModelDims& md, int store_mode) {
+  Bump bp(nullptr);
+  carve_twist(bp, md, true, store_mode);
+  carve_twist(bp, md, false, store_mode);
+  return bp.off + 256;
+}
+
+bool use_twist(const ModelDims& md) {
+  static const int env = [] {
+    const char* e = getenv("BTA_TWIST");
+    return e ? atoi(e) : 1;
+  }();
+  return env != 0 && md.nt >= 3;
+}
+
+// The three chains (up, down, separator) of one matrix.
+void make_twist_chains(bta_ctx* c, const MatWs& w, bool cond, bool value_only, Chain ch[3]) {
+  const ModelDims& md = c->md;
+  SmallLayout L = small_layout(md);
+  const long long bb = (long long)md.b * md.b;
+  const int P = md.a + 1, h = twist_h(md);
+  const int chs = cond ? CH_COND : CH_PRIOR;
+  const bool carry = c->store_mode == BTA_STORE_CARRY;
+  const long long rs = (long long)P * md.b;
+  for (int q = 0; q < 3; ++q) {
+    Chain& k = ch[q];
+    const SubWs& s = w.sub[q];
+    k = Chain();
+    k.c = c;
+    k.chain = chs;
+    k.which = cond ? BTA_COND : BTA_PRIOR;
+    k.b = md.b;
+    k.a = md.a;
+    k.nr = cond ? 1 : 0;
+    k.arrow_rows = cond;
+    k.selinv = k.contract = !value_only;
+    k.nt = q == 0 ? h : (q == 1 ? md.nt - 1 - h : 1);
+    k.t0 = q == 0 ? 0 : (q == 1 ? md.nt - 1 : h);
+    k.tdir = q == 1 ? -1 : 1;
+    k.tail_coupling = q < 2;
+    k.transposeB = q == 1;
+    k.tt_zero = q == 1;
+    k.carry = carry && q < 2;
+    k.D = w.D + (long long)k.t0 * bb;
+    k.d_stride = k.tdir * bb;
+    k.Bin = (q < 2 && !carry) ? s.B + bb : nullptr;
+    k.Bout = s.B;
+    k.b_stride = bb;
+    k.Xs = s.Xs;
+    k.LBs = s.LBs;
+    k.Bs = s.Bs;
+    if (cond) {
+      k.Rin = w.Rin + (long long)k.t0 * rs;
+      k.rin_stride = k.tdir * rs;
+      k.ld_rin = md.b;
+      k.Rout = w.Rout + (long long)k.t0 * rs;
+      k.rout_stride = k.tdir * rs;
+      k.ld_rout = md.b;
+      k.rhs_tip = w.rtip;
+      k.rhs_tip_stride = md.a;
+      k.ubuf = s.ubuf;
+      k.Ebuf = s.Ebuf;
+      k.Ybuf = s.Ybuf;
+      k.ZC[0] = s.ZC0;
+      k.ZC[1] = s.ZC1;
+      k.part = s.part;
+      k.xout = w.x;
+      k.ld_x = md.N;
+    }
+    k.T = w.T;
+    k.ldT = md.a;
+    k.W1 = s.W1;
+    k.W2 = s.W2;
+    k.W3 = s.W3;
+    k.dvec = w.dvec;
+    k.Tt = q == 1 ? w.Tt2 : c->small + L.Tt[chs];
+    k.LT = c->small + L.LT[chs];
+    k.zT = c->small + L.zT[chs];
+    k.xT = c->small + L.xT[chs];
+    k.ZT = c->small + L.ZT[chs];
+  }
+  // what the sub-chains see as their "next" block in the backward sweep: the separator
+  for (int q = 0; q < 2; ++q) {
+    ch[q].sep_x = cond ? w.x + (long long)h * md.b : nullptr;
+    ch[q].sep_ZD = ch[2].W3;      // Z_D of local block 0 of the separator chain (t & 1 == 0 -> W3)
+    ch[q].sep_ZC = ch[2].ZC[0];
+  }
+}
+
+int enqueue_gradient_twisted(bta_ctx* c, void* ws, cudaStream_t s0, bool timed, bool value_only) {
+  const ModelDims& md = c->md;
+  Bump bp(ws);
+  MatWs wc = carve_twist(bp, md, true, c->store_mode);
+  MatWs wp = carve_twist(bp, md, false, c->store_mode);
+  SmallLayout L = small_layout(md);
+  const long long bb = (long long)md.b * md.b;
+  const int P = md.a + 1, h = twist_h(md);
+  const bool carry = c->store_mode == BTA_STORE_CARRY;
+  cudaEvent_t* ev = c->ev;
+  // streams: [matrix][up, down]
+  cudaStream_t st[2][2] = {{s0, c->s_aux[0]}, {c->s_side, c->s_aux[1]}};
+#define REC(i, s)                                      \
+  do {                                                 \
+    if (timed) BTA_CUDA_OK(cudaEventRecord(ev[i], s)); \
+  } while (0)
+
+  REC(0, s0);
+  BTA_CUDA_OK(cudaMemcpyAsync(c->theta_dev, c->host_pinned, md.d * sizeof(double), cudaMemcpyHostToDevice, s0));
+  BTA_CUDA_OK(launch_theta_prep(c, s0));
+  BTA_CUDA_OK(cudaMemsetAsync(c->pivot_flag, 0xFF, sizeof(unsigned long long), s0));
+  BTA_CUDA_OK(cudaEventRecord(ev[9], s0));
+  BTA_CUDA_OK(cudaStreamWaitEvent(st[1][0], ev[9], 0));
+
+  Chain ch[2][3];  // [0] = Q_c, [1] = Q_p (Phase C)
+  make_twist_chains(c, wc, true, value_only, ch[0]);
+  make_twist_chains(c, wp, false, value_only, ch[1]);
+  const MatWs* W[2] = {&wc, &wp};
+
+  // ---- assemble: D (all blocks), arrow/rhs rows, tip on the up stream; coupling blocks per sub-chain
+  BTA_CUDA_OK(launch_assemble(c, BTA_COND, wc.D, bb, nullptr, 0, wc.Rin, (long long)P * md.b, wc.T, md.a,
+                              wc.Rin + (long long)md.a * md.b, (long long)P * md.b, wc.rtip, 1, st[0][0]));
+  REC(4, st[1][0]);
+  BTA_CUDA_OK(launch_assemble(c, BTA_PRIOR, wp.D, bb, nullptr, 0, nullptr, 0, wp.T, md.a, nullptr, 0, nullptr, 0,
+                              st[1][0]));
+  for (int m = 0; m < 2; ++m) {
+    const int which = m == 0 ? BTA_COND : BTA_PRIOR;
+    BTA_CUDA_OK(cudaEventRecord(ev[12 + m], st[m][0]));           // D, rows, tip of this matrix are assembled
+    BTA_CUDA_OK(cudaStreamWaitEvent(st[m][1], ev[12 + m], 0));
+    if (!carry) {
+      BTA_CUDA_OK(launch_assemble_seq(c, which, 1, 0, 1, ch[m][0].nt, 0, ch[m][0].Bin, bb, st[m][0]));
+      BTA_CUDA_OK(launch_assemble_seq(c, which, 1, md.nt - 2, -1, ch[m][1].nt, 1, ch[m][1].Bin, bb, st[m][1]));
+    }
+  }
+  REC(1, st[0][0]);
+  REC(5, st[1][0]);
+
+  // ---- forward: four sub-chains, launches interleaved block by block
+  for (int m = 0; m < 2; ++m)
+    for (int q = 0; q < 2; ++q) BTA_CUDA_OK(chain_forward_begin(ch[m][q], st[m][q]));
+  const int maxlen = std::max(ch[0][0].nt, ch[0][1].nt);
+  for (int s = 0; s < maxlen; ++s)
+    for (int m = 0; m < 2; ++m)
+      for (int q = 0; q < 2; ++q)
+        if (s < ch[m][q].nt) BTA_CUDA_OK(chain_forward_step(ch[m][q], s, st[m][q]));
+  for (int m = 0; m < 2; ++m) {
+    BTA_CUDA_OK(cudaEventRecord(ev[14 + m], st[m][1]));            // down chain eliminated
+    BTA_CUDA_OK(cudaStreamWaitEvent(st[m][0], ev[14 + m], 0));
+    BTA_CUDA_OK(separator_merge_forward(ch[m][0], ch[m][1], ch[m][2], st[m][0]));
+    BTA_CUDA_OK(chain_forward_step(ch[m][2], 0, st[m][0]));
+    BTA_CUDA_OK(chain_forward_end(ch[m][2], st[m][0]));
+    BTA_CUDA_OK(launch_logdet_partial(c, m == 0 ? CH_COND : CH_PRIOR, W[m]->dvec, st[m][0]));
+  }
+  REC(2, st[0][0]);
+  REC(6, st[1][0]);
+
+  // ---- backward: separator first, then the two sub-chains outwards
+  for (int m = 0; m < 2; ++m) {
+    if (value_only && m == 1) break;  // the prior needs no solve
+    BTA_CUDA_OK(chain_backward_step(ch[m][2], 0, st[m][0]));
+    BTA_CUDA_OK(cudaEventRecord(ev[16 + m], st[m][0]));
+    BTA_CUDA_OK(cudaStreamWaitEvent(st[m][1], ev[16 + m], 0));
+  }
+  for (int s = maxlen - 1; s >= 0; --s)
+    for (int m = 0; m < 2; ++m) {
+      if (value_only && m == 1) continue;
+      for (int q = 0; q < 2; ++q)
+        if (s < ch[m][q].nt) BTA_CUDA_OK(chain_backward_step(ch[m][q], s, st[m][q]));
+    }
+  // join: everything back onto s0
+  BTA_CUDA_OK(cudaEventRecord(ev[18], st[0][1]));
+  BTA_CUDA_OK(cudaStreamWaitEvent(s0, ev[18], 0));
+  BTA_CUDA_OK(cudaMemcpyAsync(wc.x + (long long)md.nt * md.b, ch[0][2].xT, md.a * sizeof(double),
+                              cudaMemcpyDeviceToDevice, s0));
+  BTA_CUDA_OK(launch_quad_stencil(c, wc.x, s0));
+  BTA_CUDA_OK(launch_residual(c, wc.x, s0));
+  REC(3, s0);
+  BTA_CUDA_OK(cudaEventRecord(ev[19], st[1][1]));
+  BTA_CUDA_OK(cudaStreamWaitEvent(st[1][0], ev[19], 0));
+  BTA_CUDA_OK(cudaEventRecord(ev[7], st[1][0]));
+  BTA_CUDA_OK(cudaStreamWaitEvent(s0, ev[7], 0));
+
+  // ---- scalar assembly (a9)
+  REC(10, s0);
+  BTA_CUDA_OK(launch_scalars(c, s0));
+  const int nout = 1 + md.d + 2 + 3 * md.d + md.k + 1;
+  BTA_CUDA_OK(cudaMemcpyAsync(c->host_pinned + 64, c->small + L.out, nout * sizeof(double), cudaMemcpyDeviceToHost,
+                              s0));
+  REC(8, s0);
+  c->last_x_dev = wc.x;
+  (void)h;
+#undef REC
+  return BTA_OK;
+}
+
 }  // namespace
 
 namespace {
@@ -473,7 +724,8 @@ int value_and_grad_impl(bta_ctx* c, const double* theta, double* f, double* grad
       const long long n0 = c->launches;
       cudaGraph_t graph = nullptr;
       BTA_CUDA_OK(cudaStreamBeginCapture(c->s_main, cudaStreamCaptureModeThreadLocal));
-      int rc = enqueue_gradient(c, ws, c->s_main, c->s_side, false, value_only);
+      int rc = use_twist(md) ? enqueue_gradient_twisted(c, ws, c->s_main, false, value_only)
+                             : enqueue_gradient(c, ws, c->s_main, c->s_side, false, value_only);
       cudaError_t ce = cudaStreamEndCapture(c->s_main, &graph);
       if (rc != BTA_OK) return rc;
       BTA_CUDA_OK(ce);
@@ -493,7 +745,8 @@ int value_and_grad_impl(bta_ctx* c, const double* theta, double* f, double* grad
     sync_stream = c->s_main;
     timed = false;
   } else {
-    int rc = enqueue_gradient(c, ws, s0, serial ? s0 : c->s_side, true, value_only);
+    int rc = (use_twist(md) && !serial) ? enqueue_gradient_twisted(c, ws, s0, true, value_only)
+                                        : enqueue_gradient(c, ws, s0, serial ? s0 : c->s_side, true, value_only);
     if (rc != BTA_OK) return rc;
   }
   c->grad_calls++;
@@ -603,4 +856,11 @@ extern "C" int bta_last_intermediates(bta_ctx* c, double* ld, double* x, double*
     BTA_CUDA_OK(cudaMemcpy(x, c->last_x_dev, c->md.N * sizeof(double), cudaMemcpyDeviceToHost));
   }
   return BTA_OK;
+}
+
+extern "C" size_t bta_workspace_bytes(const bta_ctx* c) {
+  if (!c) return 0;
+  const size_t one = grad_ws_bytes(c->md, c->store_mode);
+  const size_t two = c->md.nt >= 3 ? twist_ws_bytes(c->md, c->store_mode) : (size_t)0;
+  return one > two ? one : two;
 }

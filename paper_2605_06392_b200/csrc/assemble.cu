@@ -31,12 +31,15 @@ __global__ void theta_prep_kernel(const double* __restrict__ theta, DevParams* _
 // kind 0: D_t (lower triangle + diagonal, strict upper = 0; + tau cnt on the diagonal for Q_c);  kind 1: B_t.
 __global__ void __launch_bounds__(256) assemble_blocks_kernel(ModelDims md, const DevParams* __restrict__ P, int kind,
                                                               int cond, const double* __restrict__ cnt,
-                                                              double* __restrict__ out, long long stride, int t0) {
-  const int j = blockIdx.x * 256 + threadIdx.x, i = blockIdx.y, t = blockIdx.z + t0;
+                                                              double* __restrict__ out, long long stride, int t0,
+                                                              int tdir, int tr) {
+  // block z of the launch is global block t0 + tdir * z; tr: write the transposed block (B_t^T)
+  const int j = blockIdx.x * 256 + threadIdx.x, i = blockIdx.y, t = t0 + tdir * (int)blockIdx.z;
   if (j >= md.b) return;
   double v = 0.0;
   if (kind == 1 || j <= i) {
-    const int vi = i / md.ns, si = i % md.ns, vj = j / md.ns, sj = j % md.ns;
+    const int ii = tr ? j : i, jj = tr ? i : j;
+    const int vi = ii / md.ns, si = ii % md.ns, vj = jj / md.ns, sj = jj % md.ns;
     const int yi = si / md.g, xi = si % md.g, yj = sj / md.g, xj = sj % md.g;
     if (abs(yi - yj) + abs(xi - xj) <= 2) {
       double kv[3], mw[3];
@@ -50,7 +53,7 @@ __global__ void __launch_bounds__(256) assemble_blocks_kernel(ModelDims md, cons
     }
     if (kind == 0 && cond && i == j) v += P->tau[vi] * cnt[(long long)t * md.b + i];
   }
-  out[(long long)(t - t0) * stride + (long long)i * md.b + j] = v;
+  out[(long long)blockIdx.z * stride + (long long)i * md.b + j] = v;
 }
 
 __global__ void assemble_arrow_kernel(ModelDims md, const DevParams* __restrict__ P, int cond,
@@ -217,12 +220,12 @@ cudaError_t launch_assemble(bta_ctx* c, int which, double* D, long long d_stride
   const int cond = which == BTA_COND;
   dim3 gx((md.b + 255) / 256, md.b, md.nt);
   if (D) {
-    assemble_blocks_kernel<<<gx, 256, 0, st>>>(md, c->P, 0, cond, c->cnt, D, d_stride, 0);
+    assemble_blocks_kernel<<<gx, 256, 0, st>>>(md, c->P, 0, cond, c->cnt, D, d_stride, 0, 1, 0);
     BTA_COUNT(c);
   }
   if (B && md.nt > 1) {
     dim3 gb((md.b + 255) / 256, md.b, md.nt - 1);
-    assemble_blocks_kernel<<<gb, 256, 0, st>>>(md, c->P, 1, cond, c->cnt, B, b_stride, 0);
+    assemble_blocks_kernel<<<gb, 256, 0, st>>>(md, c->P, 1, cond, c->cnt, B, b_stride, 0, 1, 0);
     BTA_COUNT(c);
   }
   if (C || rhs) {
@@ -237,10 +240,18 @@ cudaError_t launch_assemble(bta_ctx* c, int which, double* D, long long d_stride
   return cudaGetLastError();
 }
 
-cudaError_t launch_assemble_block(bta_ctx* c, int which, int kind, int t, double* out, cudaStream_t st) {
+cudaError_t launch_assemble_block(bta_ctx* c, int which, int kind, int t, int transpose, double* out,
+                                  cudaStream_t st) {
+  return launch_assemble_seq(c, which, kind, t, 1, 1, transpose, out, 0, st);
+}
+
+cudaError_t launch_assemble_seq(bta_ctx* c, int which, int kind, int t0, int tdir, int count, int transpose,
+                                double* out, long long stride, cudaStream_t st) {
+  if (count <= 0) return cudaSuccess;
   const ModelDims& md = c->md;
-  dim3 g1((md.b + 255) / 256, md.b, 1);
-  assemble_blocks_kernel<<<g1, 256, 0, st>>>(md, c->P, kind, which == BTA_COND, c->cnt, out, 0, t);
+  dim3 g1((md.b + 255) / 256, md.b, count);
+  assemble_blocks_kernel<<<g1, 256, 0, st>>>(md, c->P, kind, which == BTA_COND, c->cnt, out, stride, t0, tdir,
+                                             transpose);
   BTA_COUNT(c);
   return cudaGetLastError();
 }

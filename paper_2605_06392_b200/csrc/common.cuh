@@ -135,7 +135,8 @@ struct bta_ctx {
   long long graph_launches[2];       // kernels inside the cached graph
   long long grad_calls;
   int store_mode;                    // BTA_STORE_FACTOR / BTA_STORE_CARRY
-  cudaEvent_t ev[16];
+  cudaStream_t s_aux[2];             // two-way elimination: the down chains of Q_c and Q_p
+  cudaEvent_t ev[32];
   long long launches;
   long long last_pivot;
   // last intermediates (host)
@@ -155,7 +156,11 @@ cudaError_t launch_assemble(bta_ctx* c, int which, double* D, long long d_stride
                             double* rhs_tip, int rhs_tip_stride, cudaStream_t st);
 cudaError_t run_setup_aggregates(bta_ctx* c, cudaStream_t st);
 // One sub-diagonal block B_t (kind 1) or diagonal block D_t (kind 0) into `out` (b x b).
-cudaError_t launch_assemble_block(bta_ctx* c, int which, int kind, int t, double* out, cudaStream_t st);
+cudaError_t launch_assemble_block(bta_ctx* c, int which, int kind, int t, int transpose, double* out,
+                                  cudaStream_t st);
+// `count` blocks t0, t0+tdir, ... of kind 0 (D) / 1 (B; transposed if `transpose`) into out + z * stride.
+cudaError_t launch_assemble_seq(bta_ctx* c, int which, int kind, int t0, int tdir, int count, int transpose,
+                                double* out, long long stride, cudaStream_t st);
 
 // contract.cu -- layout of the small device scratch (offsets in doubles into bta_ctx::small)
 struct SmallLayout {

@@ -85,6 +85,7 @@ extern "C" int bta_create(bta_ctx** out, const bta_model_desc* desc, const bta_o
   BTA_CUDA_OK(cudaMallocHost((void**)&c->host_pinned, 4096 * sizeof(double)));
   BTA_CUDA_OK(cudaStreamCreateWithFlags(&c->s_side, cudaStreamNonBlocking));
   BTA_CUDA_OK(cudaStreamCreateWithFlags(&c->s_main, cudaStreamNonBlocking));
+  for (auto& q : c->s_aux) BTA_CUDA_OK(cudaStreamCreateWithFlags(&q, cudaStreamNonBlocking));
   for (int q = 0; q < 2; ++q) {
     c->graph_exec[q] = nullptr;
     c->graph_ws[q] = nullptr;
@@ -129,6 +130,7 @@ extern "C" int bta_destroy(bta_ctx* c) {
     if (c->graph_exec[q]) cudaGraphExecDestroy(c->graph_exec[q]);
   cudaStreamDestroy(c->s_side);
   cudaStreamDestroy(c->s_main);
+  for (auto& q : c->s_aux) cudaStreamDestroy(q);
   for (auto& e : c->ev) cudaEventDestroy(e);
   delete c;
   return BTA_OK;

@@ -58,10 +58,15 @@ cudaError_t potrf_inv(bta_ctx* c, double* A, int ld, int lo, int hi, double* T1,
 
 namespace {
 __global__ void tip_init_kernel(int a, int nr, const double* __restrict__ T, int ldt_in,
-                                const double* __restrict__ rhs_tip, int tip_stride, double* __restrict__ Tt) {
+                                const double* __restrict__ rhs_tip, int tip_stride, double* __restrict__ Tt, int zero) {
   const int p = threadIdx.x / (a + nr), q = threadIdx.x % (a + nr);
   if (p >= a) return;
-  Tt[p * (a + nr) + q] = (q < a) ? T[p * ldt_in + q] : rhs_tip[(long long)(q - a) * tip_stride + p];
+  double v = 0.0;
+  if (!zero) v = (q < a) ? T[p * ldt_in + q] : rhs_tip[(long long)(q - a) * tip_stride + p];
+  Tt[p * (a + nr) + q] = v;
+}
+__global__ void tip_add_kernel(int n, const double* __restrict__ src, double* __restrict__ dst) {
+  if (threadIdx.x < n) dst[threadIdx.x] += src[threadIdx.x];
 }
 __global__ void scale_copy_kernel(long long n, double alpha, const double* __restrict__ in, double* __restrict__ out) {
   long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x;
@@ -73,7 +78,8 @@ cudaError_t chain_forward_begin(Chain& ch, cudaStream_t st) {
   bta_ctx* c = ch.c;
   const int a = ch.a, ldt = a + ch.nr;
   if (a > 0) {
-    tip_init_kernel<<<1, a * ldt, 0, st>>>(a, ch.nr, ch.T, ch.ldT, ch.rhs_tip, ch.rhs_tip_stride, ch.Tt);
+    tip_init_kernel<<<1, a * ldt, 0, st>>>(a, ch.nr, ch.T, ch.ldT, ch.rhs_tip, ch.rhs_tip_stride, ch.Tt,
+                                           ch.tt_zero ? 1 : 0);
     BTA_COUNT(c);
   }
   return cudaGetLastError();
@@ -83,6 +89,7 @@ cudaError_t chain_forward_step(Chain& ch, int t, cudaStream_t st) {
   bta_ctx* c = ch.c;
   const int b = ch.b, nt = ch.nt, a = ch.a, P = ch.P(), ldt = a + ch.nr;
   const long long bb = (long long)b * b;
+  const long long tg = ch.tg(t);                  // global time block (diag(L) position, pivot row)
   double* At = ch.D + t * ch.d_stride;           // D_t - S_{t-1}
   double* Dt = ch.carry ? ch.Xs : At;            // where X_t = L_Dt^-1 is built
   const double* LBprev = ch.carry ? ch.LBs : (t > 0 ? ch.Bout + (t - 1) * ch.b_stride : nullptr);
@@ -116,9 +123,9 @@ cudaError_t chain_forward_step(Chain& ch, int t, cudaStream_t st) {
     }
     if (ch.carry) {  // the carry D_t - S_{t-1} stays in its slot; factor a copy
       CK(cudaMemcpyAsync(Dt, At, bb * sizeof(double), cudaMemcpyDeviceToDevice, st));
-      CK(potrf_inv(c, Dt, b, 0, b, ch.W1, ch.Bs, ch.dvec ? ch.dvec + (long long)t * b : nullptr, (long long)t * b, st));
+      CK(potrf_inv(c, Dt, b, 0, b, ch.W1, ch.Bs, ch.dvec ? ch.dvec + tg * b : nullptr, tg * b, st));
     } else {
-      CK(potrf_inv(c, Dt, b, 0, b, ch.W2, ch.W3, ch.dvec ? ch.dvec + (long long)t * b : nullptr, (long long)t * b, st));
+      CK(potrf_inv(c, Dt, b, 0, b, ch.W2, ch.W3, ch.dvec ? ch.dvec + tg * b : nullptr, tg * b, st));
     }
   }
   if (P > 0) {
@@ -137,11 +144,11 @@ cudaError_t chain_forward_step(Chain& ch, int t, cudaStream_t st) {
       }
     }
   }
-  if (t < nt - 1 && ch.factor_blocks) {
+  if ((t < nt - 1 || ch.tail_coupling) && ch.factor_blocks) {
     const double* Bi;
     double *Bo, *dst;
     if (ch.carry) {
-      CK(launch_assemble_block(c, ch.which, 1, t, ch.Bs, st));
+      CK(launch_assemble_block(c, ch.which, 1, ch.tB(t), ch.transposeB ? 1 : 0, ch.Bs, st));
       Bi = ch.Bs;
       Bo = dst = ch.LBs;
     } else {
@@ -150,10 +157,13 @@ cudaError_t chain_forward_step(Chain& ch, int t, cudaStream_t st) {
       dst = (Bi == Bo) ? ch.W1 : Bo;
     }
     CK(launch_gemm(G(GEMM_NT, b, b, b, 1.0, Bi, b, Dt, b, 0.0, dst, b, KLO_ZERO, KHI_NEND, OUT_FULL), st));
-    CK(launch_gemm(G(GEMM_NT, b, b, b, -1.0, dst, b, dst, b, 1.0, ch.D + (t + 1) * ch.d_stride, b, KLO_ZERO, KHI_K,
-                     OUT_LOWER),
-                   st));
-    c->launches += 2;
+    BTA_COUNT(c);
+    if (t < nt - 1) {  // the Schur update of a separator is applied by the separator stage (two chains meet there)
+      CK(launch_gemm(G(GEMM_NT, b, b, b, -1.0, dst, b, dst, b, 1.0, ch.D + (t + 1) * ch.d_stride, b, KLO_ZERO, KHI_K,
+                       OUT_LOWER),
+                     st));
+      BTA_COUNT(c);
+    }
     if (dst != Bo) CK(cudaMemcpyAsync(Bo, dst, bb * sizeof(double), cudaMemcpyDeviceToDevice, st));
   }
   return cudaSuccess;
@@ -161,10 +171,36 @@ cudaError_t chain_forward_step(Chain& ch, int t, cudaStream_t st) {
 
 cudaError_t chain_forward_end(Chain& ch, cudaStream_t st) {
   bta_ctx* c = ch.c;
-  const int b = ch.b, nt = ch.nt, a = ch.a;
+  const int b = ch.b, nt = c->md.nt, a = ch.a;  // the tip sits after all nt blocks, whatever this chain's length
   if (a > 0) {
     CK(launch_tip(ch.Tt, a, ch.nr, ch.tip_chol ? 1 : 0, ch.LT, ch.zT, ch.xT, ch.ZT,
                   ch.dvec ? ch.dvec + (long long)nt * b : nullptr, (long long)nt * b, c->pivot_flag, st));
+    BTA_COUNT(c);
+  }
+  return cudaSuccess;
+}
+
+// Two-way elimination: the up chain (blocks 0..h-1) and the down chain (blocks nt-1..h+1, time-reversed, with
+// transposed coupling blocks) have been eliminated independently; both couple to the separator block h through
+// their last L_B.  Apply their Schur updates, arrow/rhs updates and tip contributions to the separator chain `cs`
+// (one block, its Rin rows and D already assembled), which is then factored like a last block.
+cudaError_t separator_merge_forward(Chain& up, Chain& dn, Chain& cs, cudaStream_t st) {
+  bta_ctx* c = cs.c;
+  const int b = cs.b, a = cs.a, P = cs.P();
+  Chain* sub[2] = {&up, &dn};
+  if (a > 0) {
+    tip_add_kernel<<<1, 32 * ((a * (a + cs.nr) + 31) / 32), 0, st>>>(a * (a + cs.nr), dn.Tt, up.Tt);
+    BTA_COUNT(c);
+  }
+  for (Chain* q : sub) {
+    const int last = q->nt - 1;
+    const double* LB = q->carry ? q->LBs : q->Bout + last * q->b_stride;
+    if (P > 0) {
+      CK(launch_skinny_nt(P, b, b, q->Rout + last * q->rout_stride, q->ld_rout, LB, b, 0, -1.0, 1.0, cs.Rin, cs.ld_rin,
+                          cs.Rin, cs.ld_rin, st));
+      BTA_COUNT(c);
+    }
+    CK(launch_gemm(G(GEMM_NT, b, b, b, -1.0, LB, b, LB, b, 1.0, cs.D, b, KLO_ZERO, KHI_K, OUT_LOWER), st));
     BTA_COUNT(c);
   }
   return cudaSuccess;
@@ -184,19 +220,21 @@ cudaError_t chain_backward_step(Chain& ch, int t, cudaStream_t st) {
   const long long bb = (long long)b * b;
   const bool arrow = ch.arrow();
   const int zrow0 = ch.arrow_rows ? a : 0;  // first rhs row inside the Rout stack
+  const bool has_next = (t < nt - 1) || ch.tail_coupling;   // a block eliminated after this one couples to it
+  const long long tg = ch.tg(t);
   {
     if (ch.carry) {
       // carry-based reconstruction: X_t from the stored D_t - S_{t-1}, L_Bt from the re-assembled B_t
       CK(cudaMemcpyAsync(ch.Xs, ch.D + t * ch.d_stride, bb * sizeof(double), cudaMemcpyDeviceToDevice, st));
-      CK(potrf_inv(c, ch.Xs, b, 0, b, ch.W1, ch.Bs, nullptr, (long long)t * b, st));
-      if (t < nt - 1) {
-        CK(launch_assemble_block(c, ch.which, 1, t, ch.Bs, st));
+      CK(potrf_inv(c, ch.Xs, b, 0, b, ch.W1, ch.Bs, nullptr, (long long)ch.tg(t) * b, st));
+      if (has_next) {
+        CK(launch_assemble_block(c, ch.which, 1, ch.tB(t), ch.transposeB ? 1 : 0, ch.Bs, st));
         CK(launch_gemm(G(GEMM_NT, b, b, b, 1.0, ch.Bs, b, ch.Xs, b, 0.0, ch.LBs, b, KLO_ZERO, KHI_NEND, OUT_FULL), st));
         BTA_COUNT(c);
       }
     }
     const double* X = ch.carry ? ch.Xs : ch.D + t * ch.d_stride;
-    double* LB = (t < nt - 1) ? (ch.carry ? ch.LBs : ch.Bout + t * ch.b_stride) : nullptr;
+    double* LB = has_next ? (ch.carry ? ch.LBs : ch.Bout + t * ch.b_stride) : nullptr;
     const double* LC = nullptr;
     int ld_lc = b;
     if (ch.arrow_rows) {
@@ -216,14 +254,15 @@ cudaError_t chain_backward_step(Chain& ch, int t, cudaStream_t st) {
         u = ch.ubuf;
         ld_u = b;
       }
-      if (t < nt - 1) {
-        CK(launch_skinny_nn(nr, b, b, ch.xout + (long long)(t + 1) * b, (int)ch.ld_x, LB, b, 0, -1.0, 1.0, u, ld_u,
+      if (has_next) {
+        const double* xnext = (t < nt - 1) ? ch.xout + (long long)ch.tg(t + 1) * b : ch.sep_x;
+        CK(launch_skinny_nn(nr, b, b, xnext, (int)ch.ld_x, LB, b, 0, -1.0, 1.0, u, ld_u,
                             ch.ubuf, b, ch.part, st));
         c->launches += 2;
         u = ch.ubuf;
         ld_u = b;
       }
-      CK(launch_skinny_nn(nr, b, b, u, ld_u, X, b, 1, 1.0, 0.0, nullptr, 0, ch.xout + (long long)t * b, (int)ch.ld_x,
+      CK(launch_skinny_nn(nr, b, b, u, ld_u, X, b, 1, 1.0, 0.0, nullptr, 0, ch.xout + tg * b, (int)ch.ld_x,
                           ch.part, st));
       c->launches += 2;
     }
@@ -231,15 +270,15 @@ cudaError_t chain_backward_step(Chain& ch, int t, cudaStream_t st) {
     // ---- selected inversion (R10), tensor-friendly form:  G = L_B X,  E = L_C X,
     //      Z_B = -Z_D{t+1} G - Z_C{t+1}^T E,  Z_C = -Z_C{t+1} G - Z_T E,  Z_D = X^T X - Z_B^T G - Z_C^T E
     double* ZDcur = (t & 1) ? ch.W2 : ch.W3;
-    double* ZDnext = (t & 1) ? ch.W3 : ch.W2;
+    const double* ZDnext = (t < nt - 1) ? ((t & 1) ? ch.W3 : ch.W2) : ch.sep_ZD;
     double* ZCcur = ch.ZC[t & 1];
-    double* ZCnext = ch.ZC[(t & 1) ^ 1];
+    const double* ZCnext = (t < nt - 1) ? ch.ZC[(t & 1) ^ 1] : ch.sep_ZC;
     if (arrow) {
       CK(launch_skinny_nn(a, b, b, LC, ld_lc, X, b, 1, 1.0, 0.0, nullptr, 0, ch.Ebuf, b, ch.part, st));  // E
       CK(launch_small_left_mul(a, a, b, ch.ZT, a, ch.Ebuf, b, 1.0, 0.0, nullptr, 0, ch.Ybuf, b, st));   // Z_T E
       c->launches += 3;
     }
-    if (t < nt - 1) {
+    if (has_next) {
       double* Gm = ch.W1;
       CK(launch_gemm(G(GEMM_NN, b, b, b, 1.0, LB, b, X, b, 0.0, Gm, b, KLO_N0, KHI_K, OUT_FULL), st));
       BTA_COUNT(c);
@@ -276,9 +315,9 @@ cudaError_t chain_backward_step(Chain& ch, int t, cudaStream_t st) {
       BTA_COUNT(c);
     }
     if (ch.contract) {
-      CK(launch_trace_stencil(c, ch.chain, t, 0, ZDcur, b, st));
-      if (t < nt - 1) CK(launch_trace_stencil(c, ch.chain, t, 1, LB, b, st));
-      if (arrow) CK(launch_noise_trace(c, t, ZDcur, b, ZCcur, b, st));
+      CK(launch_trace_stencil(c, ch.chain, (int)tg, 0, ZDcur, b, st));
+      if (has_next) CK(launch_trace_stencil(c, ch.chain, ch.tB(t), 1, LB, b, st));
+      if (arrow) CK(launch_noise_trace(c, (int)tg, ZDcur, b, ZCcur, b, st));
     }
     if (ch.selinv_inplace) {
       CK(cudaMemcpyAsync(ch.D + t * ch.d_stride, ZDcur, bb * sizeof(double), cudaMemcpyDeviceToDevice, st));

@@ -17,6 +17,17 @@ struct Chain {
   bool selinv_inplace = false; // backward: copy Z_D / Z_C back over D / C (bta_selinv)
   bool carry = false;          // carry mode (a7): D(t) keeps D_t - S_{t-1}; X_t, L_Bt live in Xs / LBs and are rebuilt
   int which = BTA_COND;        // carry mode: which matrix B_t is re-assembled for
+  // Sub-chain of a two-way (twisted) elimination: local block s is global time block t0 + tdir * s; with
+  // tail_coupling the last local block also couples (through B(nt-1)) to a separator block eliminated later.
+  int t0 = 0, tdir = 1;
+  bool tail_coupling = false;
+  bool transposeB = false;     // the coupling blocks of this chain are B^T (down chain); carry mode re-assembly
+  bool tt_zero = false;        // forward_begin: start the tip accumulator from zero (the up chain carries T)
+  const double* sep_x = nullptr;   // backward: x, Z_D, Z_C of the separator (the "next" block of local block nt-1)
+  const double* sep_ZD = nullptr;
+  const double* sep_ZC = nullptr;
+  int tg(int s) const { return t0 + tdir * s; }
+  int tB(int s) const { return tdir > 0 ? tg(s) : tg(s) - 1; }   // index of the sub-diagonal block between s, s+1
 
   int P() const { return (arrow_rows ? a : 0) + nr; }
   bool arrow() const { return arrow_rows || arrow_given; }
@@ -50,4 +61,5 @@ cudaError_t chain_forward_begin(Chain& ch, cudaStream_t st);
 cudaError_t chain_forward_step(Chain& ch, int t, cudaStream_t st);
 cudaError_t chain_forward_end(Chain& ch, cudaStream_t st);
 cudaError_t chain_backward_step(Chain& ch, int t, cudaStream_t st);
+cudaError_t separator_merge_forward(Chain& up, Chain& dn, Chain& cs, cudaStream_t st);
 cudaError_t chain_backward(Chain& ch, cudaStream_t st);
