@@ -745,9 +745,20 @@ int value_and_grad_impl(bta_ctx* c, const double* theta, double* f, double* grad
     sync_stream = c->s_main;
     timed = false;
   } else {
-    int rc = (use_twist(md) && !serial) ? enqueue_gradient_twisted(c, ws, s0, true, value_only)
-                                        : enqueue_gradient(c, ws, s0, serial ? s0 : c->s_side, true, value_only);
-    if (rc != BTA_OK) return rc;
+    int rc;
+    if (use_twist(md) && !serial) {
+      // run on the library's own prioritised streams; the caller's stream only orders the call
+      BTA_CUDA_OK(cudaEventRecord(ev[11], s0));
+      BTA_CUDA_OK(cudaStreamWaitEvent(c->s_main, ev[11], 0));
+      rc = enqueue_gradient_twisted(c, ws, c->s_main, true, value_only);
+      if (rc != BTA_OK) return rc;
+      BTA_CUDA_OK(cudaEventRecord(ev[20], c->s_main));
+      BTA_CUDA_OK(cudaStreamWaitEvent(s0, ev[20], 0));
+      sync_stream = c->s_main;
+    } else {
+      rc = enqueue_gradient(c, ws, s0, serial ? s0 : c->s_side, true, value_only);
+      if (rc != BTA_OK) return rc;
+    }
   }
   c->grad_calls++;
   int rc = check_pivot(c, sync_stream);  // synchronises the stream (and, through ev[7], the side stream)

@@ -305,7 +305,11 @@ cudaError_t launch_gemm(const GemmArgs& g0, cudaStream_t st) {
     const char* e = getenv("BTA_GEMM_CFG");
     return e ? atoi(e) : 0;
   }();
-  if (tiles128 >= 120) {
+  static const long long thresh = [] {
+    const char* e = getenv("BTA_TILE_THRESH");
+    return e ? atoll(e) : 120LL;
+  }();
+  if (tiles128 >= thresh) {
     switch (big) {
       case 1: return launch_mode<128, 128, 32, 64, 1, 32>(g, st);
       case 2: return launch_mode<128, 128, 32, 32, 1, 16>(g, st);
