@@ -135,7 +135,20 @@ __global__ void __launch_bounds__(Cfg<BM, BN, WM, WN, A_KM, B_KM, BK>::NT, MINB)
     N = s.N;
     K = s.K;
   }
-  const int m0 = blockIdx.y * BM, n0 = blockIdx.x * BN;
+  // Tile order: CTAs are dispatched x-fastest.  With a restricted k-range the work per tile varies by up to 32x;
+  // the tiles are enumerated heaviest-first (the heavy tile column / row is the slow grid dimension), so the last,
+  // partially filled wave consists of the lightest tiles.
+  int tm = blockIdx.y, tn = blockIdx.x;
+  if (g.klo == KLO_N0) {
+    tm = blockIdx.x;
+    tn = blockIdx.y;
+  } else if (g.khi == KHI_NEND) {
+    tm = blockIdx.x;
+    tn = (int)gridDim.y - 1 - (int)blockIdx.y;
+  } else if (g.khi == KHI_MEND) {
+    tm = (int)gridDim.y - 1 - (int)blockIdx.y;
+  }
+  const int m0 = tm * BM, n0 = tn * BN;
   if (m0 >= M || n0 >= N) return;
   if (g.out != OUT_FULL && n0 > m0 + BM - 1) return;  // tile entirely above the diagonal
 
@@ -272,7 +285,9 @@ cudaError_t launch_cfg(const GemmArgs& g, cudaStream_t st) {
     if (e != cudaSuccess) return e;
     attr_done = true;
   }
-  dim3 grid((g.N + BN - 1) / BN, (g.M + BM - 1) / BM, g.subs ? g.nsub : 1);
+  const int tilesM = (g.M + BM - 1) / BM, tilesN = (g.N + BN - 1) / BN;
+  const bool swap = g.klo == KLO_N0 || g.khi == KHI_NEND;  // heavy-first enumeration (see the kernel)
+  dim3 grid(swap ? tilesM : tilesN, swap ? tilesN : tilesM, g.subs ? g.nsub : 1);
   kern<<<grid, C_::NT, C_::SMEM, st>>>(g);
   return cudaGetLastError();
 }
