@@ -145,6 +145,13 @@ int inla_fd_grad(bta_ctx* ctx, const double* theta, double h, double* f, double*
 int inla_hessian(bta_ctx* ctx, const double* theta, double h, double* f, double* grad, double* H, void* ws,
                  void* stream);
 
+/* the INLA mode search: maximise f(theta) (reading R1: Eq. 1 is a
+ * log-posterior) by L-BFGS on -f with exact gradients from inla_value_and_grad and an Armijo backtracking line search;
+ * host driver, no new kernels.  Stops when ||grad||_inf <= gtol or after max_iter iterations.  Outputs (HOST, any may
+ * be NULL): theta_opt[d], f_opt, grad_opt[d], iters, evals (number of inla_value_and_grad calls). */
+int inla_optimize(bta_ctx* ctx, const double* theta0, int max_iter, double gtol, double* theta_opt, double* f_opt,
+                  double* grad_opt, int* iters, int* evals, void* ws, void* stream);
+
 enum {
   BTA_STAGE_ASSEMBLE = 0,
   BTA_STAGE_FWD_QC = 1,

@@ -62,6 +62,7 @@ def lib():
     L.inla_value.argtypes = [vp, dp, dp, vp, vp]
     L.inla_fd_grad.argtypes = [vp, dp, C.c_double, dp, dp, vp, vp]
     L.inla_hessian.argtypes = [vp, dp, C.c_double, dp, dp, dp, vp, vp]
+    L.inla_optimize.argtypes = [vp, dp, i32, C.c_double, dp, dp, dp, C.POINTER(C.c_int), C.POINTER(C.c_int), vp, vp]
     L.bta_last_intermediates.argtypes = [vp, dp, dp, dp, dp, dp, dp]
     L.bta_num_hyper.argtypes = [vp]
     L.bta_num_hyper.restype = C.c_int32
@@ -243,6 +244,17 @@ class BtaModel:
         _check(lib().inla_hessian(self._h, _dptr(th), float(h), C.byref(f), _dptr(g), _dptr(H),
                                   self._workspace().data_ptr(), _stream()))
         return f.value, g, H
+
+    def inla_optimize(self, theta0, max_iter=100, gtol=1e-6):
+        """L-BFGS mode search on f (maximisation); returns (theta*, f*, grad*, iterations, gradient evaluations)."""
+        th0 = np.ascontiguousarray(theta0, dtype=np.float64)
+        th = np.zeros(self.d)
+        g = np.zeros(self.d)
+        f = C.c_double()
+        it, ev = C.c_int(), C.c_int()
+        _check(lib().inla_optimize(self._h, _dptr(th0), int(max_iter), float(gtol), _dptr(th), C.byref(f), _dptr(g),
+                                   C.byref(it), C.byref(ev), self._workspace().data_ptr(), _stream()))
+        return th, f.value, g, it.value, ev.value
 
     def last_intermediates(self, want_x=True):
         ld = np.zeros(2)

@@ -1,5 +1,6 @@
 // The C-ABI entry points of include/bta.h: argument checks, workspace carving, stream/event plumbing.
 #include <algorithm>
+#include <cmath>
 #include <cstdlib>
 #include <cstring>
 
@@ -845,6 +846,103 @@ extern "C" int inla_hessian(bta_ctx* c, const double* theta, double h, double* f
     th[j] = theta[j];
     for (int i = 0; i < d; ++i) H[i * d + j] = (gp[i] - gm[i]) / (2.0 * h);
   }
+  return BTA_OK;
+}
+
+extern "C" int inla_optimize(bta_ctx* c, const double* theta0, int max_iter, double gtol, double* theta_opt,
+                             double* f_opt, double* grad_opt, int* iters, int* evals, void* ws, void* stream) {
+  if (!c || !theta0 || !ws) return bad("inla_optimize: null ctx, theta0 or workspace");
+  if (max_iter < 0 || !(gtol >= 0.0)) return bad("inla_optimize: max_iter >= 0 and gtol >= 0 required");
+  const int d = c->md.d, mem = 10;
+  // minimise phi = -f;  g = -grad f
+  std::vector<double> x(theta0, theta0 + d), g(d), xn(d), gn(d), dir(d), q(d);
+  std::vector<std::vector<double>> S, Y;
+  std::vector<double> rho;
+  double phi = 0.0;
+  int nev = 0, it = 0;
+  auto eval = [&](const std::vector<double>& th, double& ph, std::vector<double>& gr) -> int {
+    double fv = 0.0;
+    int rc = value_and_grad_impl(c, th.data(), &fv, gr.data(), nullptr, ws, stream, false);
+    ++nev;
+    ph = -fv;
+    for (int i = 0; i < d; ++i) gr[i] = -gr[i];
+    return rc;
+  };
+  auto dot = [&](const std::vector<double>& a_, const std::vector<double>& b_) {
+    double s_ = 0.0;
+    for (int i = 0; i < d; ++i) s_ += a_[i] * b_[i];
+    return s_;
+  };
+  int rc = eval(x, phi, g);
+  if (rc != BTA_OK) return rc;
+  for (; it < max_iter; ++it) {
+    double gmax = 0.0;
+    for (int i = 0; i < d; ++i) gmax = std::max(gmax, std::fabs(g[i]));
+    if (gmax <= gtol) break;
+    // two-loop recursion
+    q = g;
+    const int mcur = (int)S.size();
+    std::vector<double> al(mcur);
+    for (int i = mcur - 1; i >= 0; --i) {
+      al[i] = rho[i] * dot(S[i], q);
+      for (int j = 0; j < d; ++j) q[j] -= al[i] * Y[i][j];
+    }
+    double gamma = 1.0;
+    if (mcur > 0) gamma = dot(S[mcur - 1], Y[mcur - 1]) / dot(Y[mcur - 1], Y[mcur - 1]);
+    for (int j = 0; j < d; ++j) q[j] *= gamma;
+    for (int i = 0; i < mcur; ++i) {
+      const double be = rho[i] * dot(Y[i], q);
+      for (int j = 0; j < d; ++j) q[j] += (al[i] - be) * S[i][j];
+    }
+    for (int j = 0; j < d; ++j) dir[j] = -q[j];
+    double slope = dot(g, dir);
+    if (!(slope < 0.0)) {  // not a descent direction: restart from steepest descent
+      S.clear();
+      Y.clear();
+      rho.clear();
+      for (int j = 0; j < d; ++j) dir[j] = -g[j];
+      slope = dot(g, dir);
+    }
+    double step = (mcur == 0) ? std::min(1.0, 1.0 / std::max(gmax, 1e-300)) : 1.0;
+    double phin = 0.0;
+    bool ok = false;
+    for (int ls = 0; ls < 30; ++ls) {
+      for (int j = 0; j < d; ++j) xn[j] = x[j] + step * dir[j];
+      rc = eval(xn, phin, gn);
+      if (rc == BTA_OK && std::isfinite(phin) && phin <= phi + 1e-4 * step * slope) {
+        ok = true;
+        break;
+      }
+      if (rc != BTA_OK && rc != BTA_ERR_NOTSPD) return rc;
+      step *= 0.5;
+    }
+    if (!ok) break;  // no progress possible at this precision
+    std::vector<double> sv(d), yv(d);
+    for (int j = 0; j < d; ++j) {
+      sv[j] = xn[j] - x[j];
+      yv[j] = gn[j] - g[j];
+    }
+    const double sy = dot(sv, yv);
+    if (sy > 1e-12 * std::sqrt(dot(sv, sv) * dot(yv, yv))) {
+      S.push_back(sv);
+      Y.push_back(yv);
+      rho.push_back(1.0 / sy);
+      if ((int)S.size() > mem) {
+        S.erase(S.begin());
+        Y.erase(Y.begin());
+        rho.erase(rho.begin());
+      }
+    }
+    x = xn;
+    g = gn;
+    phi = phin;
+  }
+  if (theta_opt) memcpy(theta_opt, x.data(), d * sizeof(double));
+  if (f_opt) *f_opt = -phi;
+  if (grad_opt)
+    for (int i = 0; i < d; ++i) grad_opt[i] = -g[i];
+  if (iters) *iters = it;
+  if (evals) *evals = nev;
   return BTA_OK;
 }
 

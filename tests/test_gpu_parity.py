@@ -242,3 +242,21 @@ def test_value_fd_gradient_and_hessian(name):
         Href[:, j] = (O.value_and_grad(model, obs, th + e)["grad"] - O.value_and_grad(model, obs, th - e)["grad"]) / (2 * hh)
     assert np.max(np.abs(H - Href)) <= 1e-6 * np.max(np.abs(Href))
     assert np.max(np.abs(H - H.T)) <= 1e-3 * np.max(np.abs(H))       # symmetric up to O(h^2)
+
+
+@pytest.mark.parametrize("name", ["w0", "mv_k3_tiny"])
+def test_mode_search_matches_scipy_on_the_oracle(name):
+    """L-BFGS over theta with exact GPU gradients reaches the optimum that scipy's
+    L-BFGS-B finds on the oracle's objective."""
+    from scipy.optimize import minimize
+    model, obs, th0 = CASES[name]()
+    M = _model(model, obs)
+    th, f, g, iters, evals = M.inla_optimize(th0, max_iter=200, gtol=1e-7)
+    M.close()
+    assert np.max(np.abs(g)) <= 1e-5 and iters > 0 and evals >= iters
+    fun = lambda t: tuple(-np.asarray(v) for v in (lambda r: (r["f"], r["grad"]))(O.value_and_grad(model, obs, t)))
+    ref = minimize(fun, th0, jac=True, method="L-BFGS-B", options=dict(maxiter=500, ftol=1e-15, gtol=1e-9))
+    assert abs(f - (-ref.fun)) <= 1e-8 * abs(ref.fun)
+    assert np.max(np.abs(th - ref.x)) <= 1e-4
+    r = O.value_and_grad(model, obs, th)            # the oracle agrees at the GPU optimum
+    assert abs(r["f"] - f) <= TOL_F * abs(f) and np.max(np.abs(r["grad"])) <= 1e-4
