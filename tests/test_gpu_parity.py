@@ -38,6 +38,10 @@ CASES = {
     "a8": lambda: (lambda m: (m, draw_obs(m, 800, 36), draw_theta(m, 36)))(make_model(8, 1, 6, 8)),
     "no_obs": lambda: (lambda m: (m, draw_obs(m, 0, 37), draw_theta(m, 37)))(make_model(5, 1, 4, 2)),
     "uniform_design": lambda: (lambda m: (m, uniform_design(m, 2), draw_theta(m, 38)))(make_model(6, 1, 5, 2)),
+    "nt3_twist_min": lambda: (lambda m: (m, draw_obs(m, 200, 41), draw_theta(m, 41)))(make_model(7, 1, 3, 2)),
+    "nt4_twist": lambda: (lambda m: (m, draw_obs(m, 200, 42), draw_theta(m, 42)))(make_model(6, 1, 4, 3)),
+    "mv_k4": lambda: (lambda m: (m, draw_obs(m, 60, 43), draw_theta(m, 43)))(make_model(3, 4, 5, 8)),
+    "mv_k2_a8": lambda: (lambda m: (m, draw_obs(m, 300, 44), draw_theta(m, 44)))(make_model(8, 2, 7, 8)),
     "cfg1": lambda: make_config(1),
 }
 
@@ -68,7 +72,8 @@ def test_value_and_grad_parity(name):
     assert st["total"] > 0
 
 
-@pytest.mark.parametrize("name", ["w0", "b81_two_tiles", "b144_h07", "nt1", "nt2", "mv_k2_b162", "mv_k3_b300", "cfg1"])
+@pytest.mark.parametrize("name", ["w0", "b81_two_tiles", "b144_h07", "nt1", "nt2", "nt3_twist_min", "nt4_twist",
+                                  "mv_k2_b162", "mv_k3_b300", "cfg1"])
 def test_carry_mode_matches_oracle_and_factor_mode(name):
     """Storage policy a7: carry-based reconstruction gives the same f, grad with about half the
     block storage."""
