@@ -620,6 +620,20 @@ int enqueue_gradient_twisted(bta_ctx* c, void* ws, cudaStream_t s0, bool timed, 
   make_twist_chains(c, wc, true, value_only, ch[0]);
   make_twist_chains(c, wp, false, value_only, ch[1]);
   const MatWs* W[2] = {&wc, &wp};
+  {
+    static const int lanes = [] {
+      const char* e = getenv("BTA_LANES");
+      return e ? atoi(e) : 1;
+    }();
+    if (lanes)
+      for (int m = 0; m < 2; ++m) {
+        ch[m][0].hi = c->s_hi[2 * m];
+        ch[m][1].hi = c->s_hi[2 * m + 1];
+        ch[m][2].hi = c->s_hi[2 * m];  // the separator runs on the up chain's streams
+        for (int q = 0; q < 3; ++q) ch[m][q].lanes_bwd = lanes != 2;
+      }
+  }
+  auto join_lanes = [&](int m, int q) { return chain_to_big(ch[m][q], st[m][q == 2 ? 0 : q]); };
 
   // ---- assemble: D (all blocks), arrow/rhs rows, tip on the up stream; coupling blocks per sub-chain
   BTA_CUDA_OK(launch_assemble(c, BTA_COND, wc.D, bb, nullptr, 0, wc.Rin, (long long)P * md.b, wc.T, md.a,
@@ -648,11 +662,14 @@ int enqueue_gradient_twisted(bta_ctx* c, void* ws, cudaStream_t s0, bool timed, 
       for (int q = 0; q < 2; ++q)
         if (s < ch[m][q].nt) BTA_CUDA_OK(chain_forward_step(ch[m][q], s, st[m][q]));
   for (int m = 0; m < 2; ++m) {
+    BTA_CUDA_OK(join_lanes(m, 0));
+    BTA_CUDA_OK(join_lanes(m, 1));
     BTA_CUDA_OK(cudaEventRecord(ev[14 + m], st[m][1]));            // down chain eliminated
     BTA_CUDA_OK(cudaStreamWaitEvent(st[m][0], ev[14 + m], 0));
     BTA_CUDA_OK(separator_merge_forward(ch[m][0], ch[m][1], ch[m][2], st[m][0]));
     BTA_CUDA_OK(chain_forward_step(ch[m][2], 0, st[m][0]));
     BTA_CUDA_OK(chain_forward_end(ch[m][2], st[m][0]));
+    BTA_CUDA_OK(join_lanes(m, 2));
     BTA_CUDA_OK(launch_logdet_partial(c, m == 0 ? CH_COND : CH_PRIOR, W[m]->dvec, st[m][0]));
   }
   REC(2, st[0][0]);
@@ -662,6 +679,7 @@ int enqueue_gradient_twisted(bta_ctx* c, void* ws, cudaStream_t s0, bool timed, 
   for (int m = 0; m < 2; ++m) {
     if (value_only && m == 1) break;  // the prior needs no solve
     BTA_CUDA_OK(chain_backward_step(ch[m][2], 0, st[m][0]));
+    BTA_CUDA_OK(join_lanes(m, 2));
     BTA_CUDA_OK(cudaEventRecord(ev[16 + m], st[m][0]));
     BTA_CUDA_OK(cudaStreamWaitEvent(st[m][1], ev[16 + m], 0));
   }
@@ -672,6 +690,8 @@ int enqueue_gradient_twisted(bta_ctx* c, void* ws, cudaStream_t s0, bool timed, 
         if (s < ch[m][q].nt) BTA_CUDA_OK(chain_backward_step(ch[m][q], s, st[m][q]));
     }
   // join: everything back onto s0
+  for (int m = 0; m < 2; ++m)
+    for (int q = 0; q < 2; ++q) BTA_CUDA_OK(join_lanes(m, q));
   BTA_CUDA_OK(cudaEventRecord(ev[18], st[0][1]));
   BTA_CUDA_OK(cudaStreamWaitEvent(s0, ev[18], 0));
   BTA_CUDA_OK(cudaMemcpyAsync(wc.x + (long long)md.nt * md.b, ch[0][2].xT, md.a * sizeof(double),

@@ -64,6 +64,7 @@ struct GemmArgs {
 };
 
 cudaError_t launch_gemm(const GemmArgs& g, cudaStream_t st);
+bool gemm_uses_small_tiles(const GemmArgs& g);  // the 64x64-tile configuration (few CTAs)
 
 // ------------------------------------------------------------------------------------------------
 // Leaf / tip kernels (diag.cu)
@@ -113,6 +114,8 @@ struct ModelDims {
   double h, fixed_prec;
 };
 
+constexpr int BTA_NSW = 256;
+
 struct bta_ctx {
   ModelDims md;
   int device;
@@ -137,6 +140,9 @@ struct bta_ctx {
   int store_mode;                    // BTA_STORE_FACTOR / BTA_STORE_CARRY
   cudaStream_t s_aux[2];             // two-way elimination: the down chains of Q_c and Q_p
   cudaEvent_t ev[32];
+  cudaStream_t s_hi[4];              // high-priority companions of the four chains (small kernels)
+  cudaEvent_t ev_sw[256];            // lane-switch events, used round-robin
+  unsigned ev_sw_next;
   long long launches;
   long long last_pivot;
   // last intermediates (host)

@@ -306,6 +306,23 @@ cudaError_t launch_mode(const GemmArgs& g, cudaStream_t st) {
 
 // Tile choice: 128x128 (8 warps, 32x64 per warp) once the problem fills the chip with big tiles,
 // else 64x64 (4 warps, 32x32 per warp) for more CTAs on small problems.
+namespace {
+long long big_tiles(const GemmArgs& g) {
+  long long tiles128 = (long long)((g.M + 127) / 128) * ((g.N + 127) / 128) * (g.subs ? g.nsub : 1);
+  if (g.out != OUT_FULL) tiles128 = tiles128 / 2 + 1;
+  return tiles128;
+}
+long long tile_threshold() {
+  static const long long thresh = [] {
+    const char* e = getenv("BTA_TILE_THRESH");
+    return e ? atoll(e) : 120LL;
+  }();
+  return thresh;
+}
+}  // namespace
+
+bool gemm_uses_small_tiles(const GemmArgs& g) { return big_tiles(g) < tile_threshold(); }
+
 cudaError_t launch_gemm(const GemmArgs& g0, cudaStream_t st) {
   if (g0.M <= 0 || g0.N <= 0) return cudaSuccess;
   static const int dbg = [] {
@@ -314,17 +331,11 @@ cudaError_t launch_gemm(const GemmArgs& g0, cudaStream_t st) {
   }();
   GemmArgs g = g0;
   g.dbg = dbg;
-  long long tiles128 = (long long)((g.M + 127) / 128) * ((g.N + 127) / 128) * (g.subs ? g.nsub : 1);
-  if (g.out != OUT_FULL) tiles128 = tiles128 / 2 + 1;
   static const int big = [] {
     const char* e = getenv("BTA_GEMM_CFG");
     return e ? atoi(e) : 0;
   }();
-  static const long long thresh = [] {
-    const char* e = getenv("BTA_TILE_THRESH");
-    return e ? atoll(e) : 120LL;
-  }();
-  if (tiles128 >= thresh) {
+  if (!gemm_uses_small_tiles(g)) {
     switch (big) {
       case 1: return launch_mode<128, 128, 32, 64, 1, 32>(g, st);
       case 2: return launch_mode<128, 128, 32, 32, 1, 16>(g, st);

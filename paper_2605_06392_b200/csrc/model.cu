@@ -105,6 +105,13 @@ extern "C" int bta_create(bta_ctx** out, const bta_model_desc* desc, const bta_o
   c->grad_calls = 0;
   c->store_mode = BTA_STORE_FACTOR;
   for (auto& e : c->ev) BTA_CUDA_OK(cudaEventCreate(&e));
+  {
+    int plo = 0, phi = 0;
+    BTA_CUDA_OK(cudaDeviceGetStreamPriorityRange(&plo, &phi));
+    for (auto& q : c->s_hi) BTA_CUDA_OK(cudaStreamCreateWithPriority(&q, cudaStreamNonBlocking, phi));
+    for (auto& e : c->ev_sw) BTA_CUDA_OK(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+    c->ev_sw_next = 0;
+  }
   if (m > 0) {
     BTA_CUDA_OK(cudaMemcpy(c->o_var, obs->var, m * sizeof(int), cudaMemcpyHostToDevice));
     BTA_CUDA_OK(cudaMemcpy(c->o_node, obs->node, m * sizeof(int), cudaMemcpyHostToDevice));
@@ -143,6 +150,8 @@ extern "C" int bta_destroy(bta_ctx* c) {
   cudaStreamDestroy(c->s_main);
   for (auto& q : c->s_aux) cudaStreamDestroy(q);
   for (auto& e : c->ev) cudaEventDestroy(e);
+  for (auto& q : c->s_hi) cudaStreamDestroy(q);
+  for (auto& e : c->ev_sw) cudaEventDestroy(e);
   delete c;
   return BTA_OK;
 }

@@ -14,6 +14,29 @@
     if (e_ != cudaSuccess) return e_; \
   } while (0)
 
+// Two lanes per chain: its normal stream for the full-chip kernels and (optionally) a high-priority companion stream
+// for the small latency-bound ones (POTRF leaves, small GEMMs of the recursion, skinny / tip / contraction kernels).
+// The block scheduler serves pending CTAs of higher-priority streams first, so a one-CTA leaf of this chain is not
+// queued behind the hundreds of pending CTAs of another chain's GEMM.  Switching lanes costs one event.
+cudaStream_t lane(Chain* ch, cudaStream_t big, bool small) {
+  if (!ch || !ch->hi) return big;
+  if (ch->on_small != small) {
+    bta_ctx* c = ch->c;
+    cudaEvent_t e = c->ev_sw[(c->ev_sw_next++) % BTA_NSW];
+    cudaStream_t from = ch->on_small ? ch->hi : big, to = small ? ch->hi : big;
+    cudaEventRecord(e, from);
+    cudaStreamWaitEvent(to, e, 0);
+    ch->on_small = small;
+  }
+  return small ? ch->hi : big;
+}
+cudaError_t chain_to_big(Chain& ch, cudaStream_t big) {
+  lane(&ch, big, false);
+  return cudaGetLastError();
+}
+#define SS lane(lch, st, true)
+#define SB lane(lch, st, false)
+
 namespace {
 inline GemmArgs G(int mode, int M, int N, int K, double alpha, const double* A, int lda, const double* B, int ldb,
                   double beta, double* C, int ldc, int klo, int khi, int out) {
@@ -21,10 +44,17 @@ inline GemmArgs G(int mode, int M, int N, int K, double alpha, const double* A, 
 }
 }  // namespace
 
+namespace {
+// a GEMM of the recursion goes to the small lane when it runs with the small-tile configuration
+cudaError_t gemm_lane(Chain* lch, cudaStream_t st, const GemmArgs& g) {
+  return launch_gemm(g, gemm_uses_small_tiles(g) ? SS : SB);
+}
+}  // namespace
+
 // A[lo:hi, lo:hi] (lower, SPD) -> X = L^-1 in place; T1, T2: scratch with the same leading dimension.
 // Recursive on 64-wide tiles:  chol/inv(A11);  L21 = A21 X11^T;  A22 -= L21 L21^T;  chol/inv(A22);
 // X21 = -X22 (L21 X11).  b^3/3 (POTRF) + b^3/3 (TRTRI) flops, all but the 64x64 leaves in DMMA GEMMs.
-cudaError_t potrf_inv(bta_ctx* c, double* A, int ld, int lo, int hi, double* T1, double* T2, double* diagL,
+cudaError_t potrf_inv(bta_ctx* c, Chain* lch, double* A, int ld, int lo, int hi, double* T1, double* T2, double* diagL,
                       long long grow0, cudaStream_t st) {
   const int n = hi - lo;
   if (n <= 0) return cudaSuccess;
@@ -35,23 +65,23 @@ cudaError_t potrf_inv(bta_ctx* c, double* A, int ld, int lo, int hi, double* T1,
   if (n <= LEAF) {
     BTA_COUNT(c);
     return launch_potrf_inv_tile(A + (long long)lo * ld + lo, ld, n, diagL ? diagL + lo : nullptr, grow0 + lo,
-                                 c->pivot_flag, st);
+                                 c->pivot_flag, SS);
   }
   const int ntile = (n + LEAF - 1) / LEAF;
   const int mid = lo + LEAF * ((ntile + 1) / 2);
   const int s1 = mid - lo, s2 = hi - mid;
-  CK(potrf_inv(c, A, ld, lo, mid, T1, T2, diagL, grow0, st));
+  CK(potrf_inv(c, lch, A, ld, lo, mid, T1, T2, diagL, grow0, st));
   double* A11 = A + (long long)lo * ld + lo;
   double* A21 = A + (long long)mid * ld + lo;
   double* A22 = A + (long long)mid * ld + mid;
   double* L21 = T1 + (long long)mid * ld + lo;
   double* LX = T2 + (long long)mid * ld + lo;
-  CK(launch_gemm(G(GEMM_NT, s2, s1, s1, 1.0, A21, ld, A11, ld, 0.0, L21, ld, KLO_ZERO, KHI_NEND, OUT_FULL), st));
-  CK(launch_gemm(G(GEMM_NT, s2, s2, s1, -1.0, L21, ld, L21, ld, 1.0, A22, ld, KLO_ZERO, KHI_K, OUT_LOWER), st));
+  CK(gemm_lane(lch, st, G(GEMM_NT, s2, s1, s1, 1.0, A21, ld, A11, ld, 0.0, L21, ld, KLO_ZERO, KHI_NEND, OUT_FULL)));
+  CK(gemm_lane(lch, st, G(GEMM_NT, s2, s2, s1, -1.0, L21, ld, L21, ld, 1.0, A22, ld, KLO_ZERO, KHI_K, OUT_LOWER)));
   c->launches += 2;
-  CK(potrf_inv(c, A, ld, mid, hi, T1, T2, diagL, grow0, st));
-  CK(launch_gemm(G(GEMM_NN, s2, s1, s1, 1.0, L21, ld, A11, ld, 0.0, LX, ld, KLO_N0, KHI_K, OUT_FULL), st));
-  CK(launch_gemm(G(GEMM_NN, s2, s1, s2, -1.0, A22, ld, LX, ld, 0.0, A21, ld, KLO_ZERO, KHI_MEND, OUT_FULL), st));
+  CK(potrf_inv(c, lch, A, ld, mid, hi, T1, T2, diagL, grow0, st));
+  CK(gemm_lane(lch, st, G(GEMM_NN, s2, s1, s1, 1.0, L21, ld, A11, ld, 0.0, LX, ld, KLO_N0, KHI_K, OUT_FULL)));
+  CK(gemm_lane(lch, st, G(GEMM_NN, s2, s1, s2, -1.0, A22, ld, LX, ld, 0.0, A21, ld, KLO_ZERO, KHI_MEND, OUT_FULL)));
   c->launches += 2;
   return cudaSuccess;
 }
@@ -75,10 +105,11 @@ __global__ void scale_copy_kernel(long long n, double alpha, const double* __res
 }  // namespace
 
 cudaError_t chain_forward_begin(Chain& ch, cudaStream_t st) {
+  Chain* lch = &ch;
   bta_ctx* c = ch.c;
   const int a = ch.a, ldt = a + ch.nr;
   if (a > 0) {
-    tip_init_kernel<<<1, a * ldt, 0, st>>>(a, ch.nr, ch.T, ch.ldT, ch.rhs_tip, ch.rhs_tip_stride, ch.Tt,
+    tip_init_kernel<<<1, a * ldt, 0, SS>>>(a, ch.nr, ch.T, ch.ldT, ch.rhs_tip, ch.rhs_tip_stride, ch.Tt,
                                            ch.tt_zero ? 1 : 0);
     BTA_COUNT(c);
   }
@@ -86,6 +117,7 @@ cudaError_t chain_forward_begin(Chain& ch, cudaStream_t st) {
 }
 
 cudaError_t chain_forward_step(Chain& ch, int t, cudaStream_t st) {
+  Chain* lch = &ch;
   bta_ctx* c = ch.c;
   const int b = ch.b, nt = ch.nt, a = ch.a, P = ch.P(), ldt = a + ch.nr;
   const long long bb = (long long)b * b;
@@ -102,7 +134,7 @@ cudaError_t chain_forward_step(Chain& ch, int t, cudaStream_t st) {
     ld_src = ch.ld_rin;
     if (t == 0 && ch.Rin == ch.Rout) {  // in-place factor: the stack product below must not alias its input
       CK(cudaMemcpy2DAsync(ch.Rtmp, b * sizeof(double), src, ld_src * sizeof(double), b * sizeof(double), P,
-                           cudaMemcpyDeviceToDevice, st));
+                           cudaMemcpyDeviceToDevice, SS));
       src = ch.Rtmp;
       ld_src = b;
     }
@@ -110,7 +142,7 @@ cudaError_t chain_forward_step(Chain& ch, int t, cudaStream_t st) {
       double* tmp = ch.Rtmp ? ch.Rtmp : ch.Rin + t * ch.rin_stride;
       const int ld_tmp = ch.Rtmp ? b : ch.ld_rin;
       CK(launch_skinny_nt(P, b, b, ch.Rout + (t - 1) * ch.rout_stride, ch.ld_rout, LBprev, b, 0, -1.0, 1.0, src, ld_src,
-                          tmp, ld_tmp, st));
+                          tmp, ld_tmp, SS));
       BTA_COUNT(c);
       src = tmp;
       ld_src = ld_tmp;
@@ -118,28 +150,28 @@ cudaError_t chain_forward_step(Chain& ch, int t, cudaStream_t st) {
   }
   if (ch.factor_blocks) {
     if (ch.zero_upper) {
-      CK(launch_zero_upper(At, b, b, st));
+      CK(launch_zero_upper(At, b, b, SB));
       BTA_COUNT(c);
     }
     if (ch.carry) {  // the carry D_t - S_{t-1} stays in its slot; factor a copy
-      CK(cudaMemcpyAsync(Dt, At, bb * sizeof(double), cudaMemcpyDeviceToDevice, st));
-      CK(potrf_inv(c, Dt, b, 0, b, ch.W1, ch.Bs, ch.dvec ? ch.dvec + tg * b : nullptr, tg * b, st));
+      CK(cudaMemcpyAsync(Dt, At, bb * sizeof(double), cudaMemcpyDeviceToDevice, SB));
+      CK(potrf_inv(c, lch, Dt, b, 0, b, ch.W1, ch.Bs, ch.dvec ? ch.dvec + tg * b : nullptr, tg * b, st));
     } else {
-      CK(potrf_inv(c, Dt, b, 0, b, ch.W2, ch.W3, ch.dvec ? ch.dvec + tg * b : nullptr, tg * b, st));
+      CK(potrf_inv(c, lch, Dt, b, 0, b, ch.W2, ch.W3, ch.dvec ? ch.dvec + tg * b : nullptr, tg * b, st));
     }
   }
   if (P > 0) {
     //   R^_t = R~_t X_t^T
     double* Rh = ch.Rout + t * ch.rout_stride;
-    CK(launch_skinny_nt(P, b, b, src, ld_src, Dt, b, 1, 1.0, 0.0, nullptr, 0, Rh, ch.ld_rout, st));
+    CK(launch_skinny_nt(P, b, b, src, ld_src, Dt, b, 1, 1.0, 0.0, nullptr, 0, Rh, ch.ld_rout, SS));
     BTA_COUNT(c);
     if (a > 0) {
       // T~ -= L_C L_C^T (line 9) and r_T - v_T, v_T += L_C z (line 5): columns [0,a) and [a, a+nr) of Tt
       if (ch.arrow_rows) {
-        CK(launch_small_nt(a, P, b, Rh, ch.ld_rout, Rh, ch.ld_rout, -1.0, ch.Tt, ldt, st));
+        CK(launch_small_nt(a, P, b, Rh, ch.ld_rout, Rh, ch.ld_rout, -1.0, ch.Tt, ldt, SS));
         BTA_COUNT(c);
       } else if (ch.arrow_given) {
-        CK(launch_small_nt(a, ch.nr, b, ch.LCgiven + t * ch.lc_stride, b, Rh, ch.ld_rout, -1.0, ch.Tt + a, ldt, st));
+        CK(launch_small_nt(a, ch.nr, b, ch.LCgiven + t * ch.lc_stride, b, Rh, ch.ld_rout, -1.0, ch.Tt + a, ldt, SS));
         BTA_COUNT(c);
       }
     }
@@ -148,7 +180,7 @@ cudaError_t chain_forward_step(Chain& ch, int t, cudaStream_t st) {
     const double* Bi;
     double *Bo, *dst;
     if (ch.carry) {
-      CK(launch_assemble_block(c, ch.which, 1, ch.tB(t), ch.transposeB ? 1 : 0, ch.Bs, st));
+      CK(launch_assemble_block(c, ch.which, 1, ch.tB(t), ch.transposeB ? 1 : 0, ch.Bs, SB));
       Bi = ch.Bs;
       Bo = dst = ch.LBs;
     } else {
@@ -156,25 +188,26 @@ cudaError_t chain_forward_step(Chain& ch, int t, cudaStream_t st) {
       Bo = ch.Bout + t * ch.b_stride;
       dst = (Bi == Bo) ? ch.W1 : Bo;
     }
-    CK(launch_gemm(G(GEMM_NT, b, b, b, 1.0, Bi, b, Dt, b, 0.0, dst, b, KLO_ZERO, KHI_NEND, OUT_FULL), st));
+    CK(launch_gemm(G(GEMM_NT, b, b, b, 1.0, Bi, b, Dt, b, 0.0, dst, b, KLO_ZERO, KHI_NEND, OUT_FULL), SB));
     BTA_COUNT(c);
     if (t < nt - 1) {  // the Schur update of a separator is applied by the separator stage (two chains meet there)
       CK(launch_gemm(G(GEMM_NT, b, b, b, -1.0, dst, b, dst, b, 1.0, ch.D + (t + 1) * ch.d_stride, b, KLO_ZERO, KHI_K,
                        OUT_LOWER),
-                     st));
+                     SB));
       BTA_COUNT(c);
     }
-    if (dst != Bo) CK(cudaMemcpyAsync(Bo, dst, bb * sizeof(double), cudaMemcpyDeviceToDevice, st));
+    if (dst != Bo) CK(cudaMemcpyAsync(Bo, dst, bb * sizeof(double), cudaMemcpyDeviceToDevice, SB));
   }
   return cudaSuccess;
 }
 
 cudaError_t chain_forward_end(Chain& ch, cudaStream_t st) {
+  Chain* lch = &ch;
   bta_ctx* c = ch.c;
   const int b = ch.b, nt = c->md.nt, a = ch.a;  // the tip sits after all nt blocks, whatever this chain's length
   if (a > 0) {
     CK(launch_tip(ch.Tt, a, ch.nr, ch.tip_chol ? 1 : 0, ch.LT, ch.zT, ch.xT, ch.ZT,
-                  ch.dvec ? ch.dvec + (long long)nt * b : nullptr, (long long)nt * b, c->pivot_flag, st));
+                  ch.dvec ? ch.dvec + (long long)nt * b : nullptr, (long long)nt * b, c->pivot_flag, SS));
     BTA_COUNT(c);
   }
   return cudaSuccess;
@@ -185,11 +218,12 @@ cudaError_t chain_forward_end(Chain& ch, cudaStream_t st) {
 // their last L_B.  Apply their Schur updates, arrow/rhs updates and tip contributions to the separator chain `cs`
 // (one block, its Rin rows and D already assembled), which is then factored like a last block.
 cudaError_t separator_merge_forward(Chain& up, Chain& dn, Chain& cs, cudaStream_t st) {
+  Chain* lch = &cs;
   bta_ctx* c = cs.c;
   const int b = cs.b, a = cs.a, P = cs.P();
   Chain* sub[2] = {&up, &dn};
   if (a > 0) {
-    tip_add_kernel<<<1, 32 * ((a * (a + cs.nr) + 31) / 32), 0, st>>>(a * (a + cs.nr), dn.Tt, up.Tt);
+    tip_add_kernel<<<1, 32 * ((a * (a + cs.nr) + 31) / 32), 0, SS>>>(a * (a + cs.nr), dn.Tt, up.Tt);
     BTA_COUNT(c);
   }
   for (Chain* q : sub) {
@@ -197,10 +231,10 @@ cudaError_t separator_merge_forward(Chain& up, Chain& dn, Chain& cs, cudaStream_
     const double* LB = q->carry ? q->LBs : q->Bout + last * q->b_stride;
     if (P > 0) {
       CK(launch_skinny_nt(P, b, b, q->Rout + last * q->rout_stride, q->ld_rout, LB, b, 0, -1.0, 1.0, cs.Rin, cs.ld_rin,
-                          cs.Rin, cs.ld_rin, st));
+                          cs.Rin, cs.ld_rin, SS));
       BTA_COUNT(c);
     }
-    CK(launch_gemm(G(GEMM_NT, b, b, b, -1.0, LB, b, LB, b, 1.0, cs.D, b, KLO_ZERO, KHI_K, OUT_LOWER), st));
+    CK(launch_gemm(G(GEMM_NT, b, b, b, -1.0, LB, b, LB, b, 1.0, cs.D, b, KLO_ZERO, KHI_K, OUT_LOWER), SB));
     BTA_COUNT(c);
   }
   return cudaSuccess;
@@ -215,6 +249,7 @@ cudaError_t chain_forward(Chain& ch, cudaStream_t st) {
 // Backward sweep t = nt-1 .. 0.  Needs from the forward sweep: X_t in D(t), L_Bt in Bout(t), the arrow factor
 // rows L_Ct, z_t (rows a.. of Rout(t) when arrow_rows, else rows 0..), and the tip outputs x_T, Z_T.
 cudaError_t chain_backward_step(Chain& ch, int t, cudaStream_t st) {
+  Chain* lch = ch.lanes_bwd ? &ch : nullptr;
   bta_ctx* c = ch.c;
   const int b = ch.b, nt = ch.nt, a = ch.a, nr = ch.nr;
   const long long bb = (long long)b * b;
@@ -225,11 +260,11 @@ cudaError_t chain_backward_step(Chain& ch, int t, cudaStream_t st) {
   {
     if (ch.carry) {
       // carry-based reconstruction: X_t from the stored D_t - S_{t-1}, L_Bt from the re-assembled B_t
-      CK(cudaMemcpyAsync(ch.Xs, ch.D + t * ch.d_stride, bb * sizeof(double), cudaMemcpyDeviceToDevice, st));
-      CK(potrf_inv(c, ch.Xs, b, 0, b, ch.W1, ch.Bs, nullptr, (long long)ch.tg(t) * b, st));
+      CK(cudaMemcpyAsync(ch.Xs, ch.D + t * ch.d_stride, bb * sizeof(double), cudaMemcpyDeviceToDevice, SB));
+      CK(potrf_inv(c, lch, ch.Xs, b, 0, b, ch.W1, ch.Bs, nullptr, (long long)ch.tg(t) * b, st));
       if (has_next) {
-        CK(launch_assemble_block(c, ch.which, 1, ch.tB(t), ch.transposeB ? 1 : 0, ch.Bs, st));
-        CK(launch_gemm(G(GEMM_NT, b, b, b, 1.0, ch.Bs, b, ch.Xs, b, 0.0, ch.LBs, b, KLO_ZERO, KHI_NEND, OUT_FULL), st));
+        CK(launch_assemble_block(c, ch.which, 1, ch.tB(t), ch.transposeB ? 1 : 0, ch.Bs, SB));
+        CK(launch_gemm(G(GEMM_NT, b, b, b, 1.0, ch.Bs, b, ch.Xs, b, 0.0, ch.LBs, b, KLO_ZERO, KHI_NEND, OUT_FULL), SB));
         BTA_COUNT(c);
       }
     }
@@ -249,7 +284,7 @@ cudaError_t chain_backward_step(Chain& ch, int t, cudaStream_t st) {
       const double* u = z;
       int ld_u = ch.ld_rout;
       if (arrow) {
-        CK(launch_small_left_mul(nr, a, b, ch.xT, a, LC, ld_lc, -1.0, 1.0, u, ld_u, ch.ubuf, b, st));
+        CK(launch_small_left_mul(nr, a, b, ch.xT, a, LC, ld_lc, -1.0, 1.0, u, ld_u, ch.ubuf, b, SS));
         BTA_COUNT(c);
         u = ch.ubuf;
         ld_u = b;
@@ -257,13 +292,13 @@ cudaError_t chain_backward_step(Chain& ch, int t, cudaStream_t st) {
       if (has_next) {
         const double* xnext = (t < nt - 1) ? ch.xout + (long long)ch.tg(t + 1) * b : ch.sep_x;
         CK(launch_skinny_nn(nr, b, b, xnext, (int)ch.ld_x, LB, b, 0, -1.0, 1.0, u, ld_u,
-                            ch.ubuf, b, ch.part, st));
+                            ch.ubuf, b, ch.part, SS));
         c->launches += 2;
         u = ch.ubuf;
         ld_u = b;
       }
       CK(launch_skinny_nn(nr, b, b, u, ld_u, X, b, 1, 1.0, 0.0, nullptr, 0, ch.xout + tg * b, (int)ch.ld_x,
-                          ch.part, st));
+                          ch.part, SS));
       c->launches += 2;
     }
     if (!ch.selinv) return cudaSuccess;
@@ -274,56 +309,56 @@ cudaError_t chain_backward_step(Chain& ch, int t, cudaStream_t st) {
     double* ZCcur = ch.ZC[t & 1];
     const double* ZCnext = (t < nt - 1) ? ch.ZC[(t & 1) ^ 1] : ch.sep_ZC;
     if (arrow) {
-      CK(launch_skinny_nn(a, b, b, LC, ld_lc, X, b, 1, 1.0, 0.0, nullptr, 0, ch.Ebuf, b, ch.part, st));  // E
-      CK(launch_small_left_mul(a, a, b, ch.ZT, a, ch.Ebuf, b, 1.0, 0.0, nullptr, 0, ch.Ybuf, b, st));   // Z_T E
+      CK(launch_skinny_nn(a, b, b, LC, ld_lc, X, b, 1, 1.0, 0.0, nullptr, 0, ch.Ebuf, b, ch.part, SS));  // E
+      CK(launch_small_left_mul(a, a, b, ch.ZT, a, ch.Ebuf, b, 1.0, 0.0, nullptr, 0, ch.Ybuf, b, SS));   // Z_T E
       c->launches += 3;
     }
     if (has_next) {
       double* Gm = ch.W1;
-      CK(launch_gemm(G(GEMM_NN, b, b, b, 1.0, LB, b, X, b, 0.0, Gm, b, KLO_N0, KHI_K, OUT_FULL), st));
+      CK(launch_gemm(G(GEMM_NN, b, b, b, 1.0, LB, b, X, b, 0.0, Gm, b, KLO_N0, KHI_K, OUT_FULL), SB));
       BTA_COUNT(c);
       if (arrow) {
-        CK(launch_skinny_nn(a, b, b, ZCnext, b, Gm, b, 0, -1.0, -1.0, ch.Ybuf, b, ZCcur, b, ch.part, st));
+        CK(launch_skinny_nn(a, b, b, ZCnext, b, Gm, b, 0, -1.0, -1.0, ch.Ybuf, b, ZCcur, b, ch.part, SS));
         c->launches += 2;
       }
       double* ZB = LB;  // L_Bt is dead from here on: Z_Bt takes its slot
-      CK(launch_gemm(G(GEMM_NN, b, b, b, -1.0, ZDnext, b, Gm, b, 0.0, ZB, b, KLO_ZERO, KHI_K, OUT_FULL), st));
+      CK(launch_gemm(G(GEMM_NN, b, b, b, -1.0, ZDnext, b, Gm, b, 0.0, ZB, b, KLO_ZERO, KHI_K, OUT_FULL), SB));
       BTA_COUNT(c);
       if (arrow) {
-        CK(launch_gemm(G(GEMM_TN, b, b, a, -1.0, ZCnext, b, ch.Ebuf, b, 1.0, ZB, b, KLO_ZERO, KHI_K, OUT_FULL), st));
+        CK(launch_gemm(G(GEMM_TN, b, b, a, -1.0, ZCnext, b, ch.Ebuf, b, 1.0, ZB, b, KLO_ZERO, KHI_K, OUT_FULL), SB));
         BTA_COUNT(c);
       }
-      CK(launch_gemm(G(GEMM_TN, b, b, b, 1.0, X, b, X, b, 0.0, ZDcur, b, KLO_M0, KHI_K, OUT_LOWER), st));
+      CK(launch_gemm(G(GEMM_TN, b, b, b, 1.0, X, b, X, b, 0.0, ZDcur, b, KLO_M0, KHI_K, OUT_LOWER), SB));
       CK(launch_gemm(G(GEMM_TN, b, b, b, -1.0, ZB, b, Gm, b, 1.0, ZDcur, b, KLO_ZERO, KHI_K,
                        arrow ? OUT_LOWER : OUT_LOWER_MIRROR),
-                     st));
+                     SB));
       c->launches += 2;
     } else {
       if (arrow) {
-        scale_copy_kernel<<<(unsigned)(((long long)a * b + 255) / 256), 256, 0, st>>>((long long)a * b, -1.0, ch.Ybuf,
+        scale_copy_kernel<<<(unsigned)(((long long)a * b + 255) / 256), 256, 0, SS>>>((long long)a * b, -1.0, ch.Ybuf,
                                                                                       ZCcur);
         BTA_COUNT(c);
       }
       CK(launch_gemm(G(GEMM_TN, b, b, b, 1.0, X, b, X, b, 0.0, ZDcur, b, KLO_M0, KHI_K,
                        arrow ? OUT_LOWER : OUT_LOWER_MIRROR),
-                     st));
+                     SB));
       BTA_COUNT(c);
     }
     if (arrow) {
       CK(launch_gemm(G(GEMM_TN, b, b, a, -1.0, ZCcur, b, ch.Ebuf, b, 1.0, ZDcur, b, KLO_ZERO, KHI_K, OUT_LOWER_MIRROR),
-                     st));
+                     SB));
       BTA_COUNT(c);
     }
     if (ch.contract) {
-      CK(launch_trace_stencil(c, ch.chain, (int)tg, 0, ZDcur, b, st));
-      if (has_next) CK(launch_trace_stencil(c, ch.chain, ch.tB(t), 1, LB, b, st));
-      if (arrow) CK(launch_noise_trace(c, (int)tg, ZDcur, b, ZCcur, b, st));
+      CK(launch_trace_stencil(c, ch.chain, (int)tg, 0, ZDcur, b, SS));
+      if (has_next) CK(launch_trace_stencil(c, ch.chain, ch.tB(t), 1, LB, b, SS));
+      if (arrow) CK(launch_noise_trace(c, (int)tg, ZDcur, b, ZCcur, b, SS));
     }
     if (ch.selinv_inplace) {
-      CK(cudaMemcpyAsync(ch.D + t * ch.d_stride, ZDcur, bb * sizeof(double), cudaMemcpyDeviceToDevice, st));
+      CK(cudaMemcpyAsync(ch.D + t * ch.d_stride, ZDcur, bb * sizeof(double), cudaMemcpyDeviceToDevice, SB));
       if (arrow && ch.Cout)
         CK(cudaMemcpyAsync(ch.Cout + t * ch.cout_stride, ZCcur, (size_t)a * b * sizeof(double),
-                           cudaMemcpyDeviceToDevice, st));
+                           cudaMemcpyDeviceToDevice, SB));
     }
   }
   return cudaSuccess;

@@ -26,6 +26,9 @@ struct Chain {
   const double* sep_x = nullptr;   // backward: x, Z_D, Z_C of the separator (the "next" block of local block nt-1)
   const double* sep_ZD = nullptr;
   const double* sep_ZC = nullptr;
+  cudaStream_t hi = nullptr;   // optional high-priority companion stream for the small kernels of this chain
+  bool on_small = false;       // which lane the chain's work currently ends on
+  bool lanes_bwd = true;       // use the small lane in the backward sweep too
   int tg(int s) const { return t0 + tdir * s; }
   int tB(int s) const { return tdir > 0 ? tg(s) : tg(s) - 1; }   // index of the sub-diagonal block between s, s+1
 
@@ -54,8 +57,9 @@ struct Chain {
   double* Cout = nullptr; long long cout_stride = 0;                    // selinv_inplace: Z_Ct destination
 };
 
-cudaError_t potrf_inv(bta_ctx* c, double* A, int ld, int lo, int hi, double* T1, double* T2, double* diagL,
-                      long long grow0, cudaStream_t st);
+cudaError_t potrf_inv(bta_ctx* c, Chain* lanes, double* A, int ld, int lo, int hi, double* T1, double* T2,
+                      double* diagL, long long grow0, cudaStream_t st);
+cudaError_t chain_to_big(Chain& ch, cudaStream_t big);  // join the small lane back into the chain's main stream
 cudaError_t chain_forward(Chain& ch, cudaStream_t st);
 cudaError_t chain_forward_begin(Chain& ch, cudaStream_t st);
 cudaError_t chain_forward_step(Chain& ch, int t, cudaStream_t st);
