@@ -636,11 +636,24 @@ int enqueue_gradient_twisted(bta_ctx* c, void* ws, cudaStream_t s0, bool timed, 
   auto join_lanes = [&](int m, int q) { return chain_to_big(ch[m][q], st[m][q == 2 ? 0 : q]); };
 
   // ---- assemble: D (all blocks), arrow/rhs rows, tip on the up stream; coupling blocks per sub-chain
-  BTA_CUDA_OK(launch_assemble(c, BTA_COND, wc.D, bb, nullptr, 0, wc.Rin, (long long)P * md.b, wc.T, md.a,
+  // The diagonal blocks are assembled lazily, a few blocks ahead of each sub-chain (assemble_ahead below): the 2 nt
+  // blocks are 69 GB of writes that would otherwise sit in front of the first POTRF.
+  BTA_CUDA_OK(launch_assemble(c, BTA_COND, nullptr, bb, nullptr, 0, wc.Rin, (long long)P * md.b, wc.T, md.a,
                               wc.Rin + (long long)md.a * md.b, (long long)P * md.b, wc.rtip, 1, st[0][0]));
   REC(4, st[1][0]);
-  BTA_CUDA_OK(launch_assemble(c, BTA_PRIOR, wp.D, bb, nullptr, 0, nullptr, 0, wp.T, md.a, nullptr, 0, nullptr, 0,
+  BTA_CUDA_OK(launch_assemble(c, BTA_PRIOR, nullptr, bb, nullptr, 0, nullptr, 0, wp.T, md.a, nullptr, 0, nullptr, 0,
                               st[1][0]));
+  constexpr int AHEAD = 8;
+  // local blocks [lo, hi) of sub-chain (m, q); the up chain also owns the separator (local index nt_up)
+  auto assemble_range = [&](int m, int q, int lo, int hi) -> int {
+    const Chain& k = ch[m][q];
+    const int top = k.nt + (q == 0 ? 1 : 0);
+    hi = std::min(hi, top);
+    if (lo >= hi) return BTA_OK;
+    BTA_CUDA_OK(launch_assemble_seq(c, m == 0 ? BTA_COND : BTA_PRIOR, 0, k.tg(lo), k.tdir, hi - lo, 0,
+                                    k.D + (long long)lo * k.d_stride, k.d_stride, st[m][q]));
+    return BTA_OK;
+  };
   for (int m = 0; m < 2; ++m) {
     const int which = m == 0 ? BTA_COND : BTA_PRIOR;
     BTA_CUDA_OK(cudaEventRecord(ev[12 + m], st[m][0]));           // D, rows, tip of this matrix are assembled
@@ -657,10 +670,22 @@ int enqueue_gradient_twisted(bta_ctx* c, void* ws, cudaStream_t s0, bool timed, 
   for (int m = 0; m < 2; ++m)
     for (int q = 0; q < 2; ++q) BTA_CUDA_OK(chain_forward_begin(ch[m][q], st[m][q]));
   const int maxlen = std::max(ch[0][0].nt, ch[0][1].nt);
+  for (int m = 0; m < 2; ++m)
+    for (int q = 0; q < 2; ++q) {
+      int rc = assemble_range(m, q, 0, 2);
+      if (rc != BTA_OK) return rc;
+    }
   for (int s = 0; s < maxlen; ++s)
     for (int m = 0; m < 2; ++m)
       for (int q = 0; q < 2; ++q)
-        if (s < ch[m][q].nt) BTA_CUDA_OK(chain_forward_step(ch[m][q], s, st[m][q]));
+        if (s < ch[m][q].nt) {
+          if (s % AHEAD == 0) {  // blocks s+2 .. s+AHEAD+1 (block s+1 receives this step's Schur update)
+            BTA_CUDA_OK(chain_to_big(ch[m][q], st[m][q]));
+            int rc = assemble_range(m, q, s + 2, s + 2 + AHEAD);
+            if (rc != BTA_OK) return rc;
+          }
+          BTA_CUDA_OK(chain_forward_step(ch[m][q], s, st[m][q]));
+        }
   for (int m = 0; m < 2; ++m) {
     BTA_CUDA_OK(join_lanes(m, 0));
     BTA_CUDA_OK(join_lanes(m, 1));

@@ -52,8 +52,8 @@ cudaError_t gemm_lane(Chain* lch, cudaStream_t st, const GemmArgs& g) {
 }  // namespace
 
 // A[lo:hi, lo:hi] (lower, SPD) -> X = L^-1 in place; T1, T2: scratch with the same leading dimension.
-// Recursive on 64-wide tiles:  chol/inv(A11);  L21 = A21 X11^T;  A22 -= L21 L21^T;  chol/inv(A22);
-// X21 = -X22 (L21 X11).  b^3/3 (POTRF) + b^3/3 (TRTRI) flops, all but the 64x64 leaves in DMMA GEMMs.
+// Recursive on 128-wide tiles (leaf: diag.cu):  chol/inv(A11);  L21 = A21 X11^T;  A22 -= L21 L21^T;  chol/inv(A22);
+// X21 = -X22 (L21 X11).  b^3/3 (POTRF) + b^3/3 (TRTRI) flops, all but the 128x128 leaves in DMMA GEMMs.
 cudaError_t potrf_inv(bta_ctx* c, Chain* lch, double* A, int ld, int lo, int hi, double* T1, double* T2, double* diagL,
                       long long grow0, cudaStream_t st) {
   const int n = hi - lo;
