@@ -30,6 +30,23 @@ __device__ __forceinline__ void cp_async_wait() {
   asm volatile("cp.async.wait_group %0;\n" ::"n"(N));
 }
 
+// Split barrier (mbarrier in shared memory): arrive early, wait late, so the barrier latency hides behind DMMAs.
+__device__ __forceinline__ void mbar_init(unsigned long long* bar, int count) {
+  unsigned a = (unsigned)__cvta_generic_to_shared(bar);
+  asm volatile("mbarrier.init.shared.b64 [%0], %1;\n" ::"r"(a), "r"(count));
+}
+__device__ __forceinline__ void mbar_arrive(unsigned long long* bar) {
+  unsigned a = (unsigned)__cvta_generic_to_shared(bar);
+  asm volatile("{\n.reg .b64 st;\nmbarrier.arrive.shared.b64 st, [%0];\n}\n" ::"r"(a) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long* bar, unsigned parity) {
+  unsigned a = (unsigned)__cvta_generic_to_shared(bar);
+  asm volatile(
+      "{\n.reg .pred p;\nWAIT_LOOP:\nmbarrier.try_wait.parity.shared.b64 p, [%0], %1;\n@!p bra WAIT_LOOP;\n}\n" ::"r"(a),
+      "r"(parity)
+      : "memory");
+}
+
 __device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double b) {
   asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
                : "+d"(c0), "+d"(c1)
@@ -111,7 +128,7 @@ struct Cfg {
   static constexpr int NT = NWM * NWN * 32;
   static constexpr int A_ST = A_KM ? BK * (BM + KPAD) : BM * (BK + KPAD);
   static constexpr int B_ST = B_KM ? BK * (BN + KPAD) : BN * (BK + KPAD);
-  static constexpr int SMEM = STAGES * (A_ST + B_ST) * (int)sizeof(double);
+  static constexpr int SMEM = (2 + STAGES * (A_ST + B_ST)) * (int)sizeof(double);
 };
 
 template <int BM, int BN, int WM, int WN, bool A_KM, bool B_KM, int MINB, int BK>
@@ -119,8 +136,9 @@ __global__ void __launch_bounds__(Cfg<BM, BN, WM, WN, A_KM, B_KM, BK>::NT, MINB)
   using C_ = Cfg<BM, BN, WM, WN, A_KM, B_KM, BK>;
   constexpr int NT = C_::NT;
   extern __shared__ __align__(16) double smem[];
-  double* As = smem;
-  double* Bs = smem + STAGES * C_::A_ST;
+  unsigned long long* bar = reinterpret_cast<unsigned long long*>(smem);  // 16 bytes reserved
+  double* As = smem + 2;
+  double* Bs = As + STAGES * C_::A_ST;
 
   const double* __restrict__ A = g.A;
   const double* __restrict__ B = g.B;
@@ -216,15 +234,16 @@ __global__ void __launch_bounds__(Cfg<BM, BN, WM, WN, A_KM, B_KM, BK>::NT, MINB)
 
 #pragma unroll
   for (int s = 0; s < STAGES - 1; ++s) issue(s);
+  if (tid == 0) mbar_init(bar, NT);
+  cp_async_wait<STAGES - 2>();
+  __syncthreads();  // stage 0 is visible, the mbarrier is initialised
 
+  // Per k-tile: [k-step 0: DMMAs, then the refill of the stage consumed one iteration ago] ... [last k-step: this
+  // thread's last reads of the stage, wait for its own copies of the next stage, ARRIVE, DMMAs, then WAIT].  When all
+  // NT threads have arrived, the next stage is visible and the current one is free -- one split barrier per k-tile
+  // whose latency is covered by the last k-step's DMMAs.  (The refill is issued after the first k-step, not right
+  // after the barrier: address arithmetic there would idle the tensor pipe of every scheduler at once.)
   for (int it = 0; it < nk; ++it) {
-    if (!(g.dbg & 2)) {
-      cp_async_wait<STAGES - 2>();
-      __syncthreads();
-    }
-    // The refill of the stage consumed in iteration it-1 is issued after the first k-step's DMMAs, not right
-    // after the barrier: all warps leave the barrier together, and address arithmetic there would idle the
-    // tensor pipe of every scheduler at once.
     const double* as = As + (it % STAGES) * C_::A_ST;
     const double* bs = Bs + (it % STAGES) * C_::B_ST;
 #pragma unroll
@@ -240,11 +259,16 @@ __global__ void __launch_bounds__(Cfg<BM, BN, WM, WN, A_KM, B_KM, BK>::NT, MINB)
         int n = wn0 + j * 8 + gid, k = kk + tig;
         bf[j] = B_KM ? bs[k * (BN + KPAD) + n] : bs[n * (BK + KPAD) + k];
       }
+      if (kk == BK - 4) {
+        cp_async_wait<STAGES - 2>();
+        mbar_arrive(bar);
+      }
 #pragma unroll
       for (int i = 0; i < WM / 8; ++i)
 #pragma unroll
         for (int j = 0; j < WN / 8; ++j) dmma884(acc[i][j][0], acc[i][j][1], af[i], bf[j]);
-      if (kk == 0 && !(g.dbg & 1)) issue(it + STAGES - 1);
+      if (kk == 0) issue(it + STAGES - 1);
+      if (kk == BK - 4) mbar_wait(bar, (unsigned)(it & 1));
     }
   }
   cp_async_wait<0>();
