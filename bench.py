@@ -184,9 +184,11 @@ def run_ours(args):
     n0 = M.kernel_launches()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     stage_acc = {}
+    step_ms = []
     e0.record()
     for i in range(args.steps):
         f, g, st = M.inla_value_and_grad(thetas[args.warmup + i], stages=True)
+        step_ms.append(st.get("total", float("nan")))
         for k_, v in st.items():
             stage_acc[k_] = stage_acc.get(k_, 0.0) + v / args.steps
     e1.record()
@@ -212,16 +214,17 @@ def run_ours(args):
             "dtype": "f64", "data": "synthetic",
             "config": {"workload": workload_name(args.config, model), "parallelism": f"replicas x{world}",
                        "l2": "inputs larger than L2 (blocks of both matrices: %.1f GB per replica)" % (ws_bytes / 1e9),
-                       "workspace_bytes": ws_bytes, "chains": "Q_c and Q_p sweeps on two streams", "store_mode": args.store},
+                       "workspace_bytes": ws_bytes, "chains": "two-way elimination: up and down chains of Q_c and Q_p on four streams (+ priority lanes)", "store_mode": args.store},
             "clocks": clocks,
             "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": 8 * d,
                     "d2h_bytes_per_step": 8 * (1 + d + 2 + 3 * d + model.k + 1) + 8},
             "gpu_launches": int(launches),
             "stage_ms": stage_acc,
+            "step_ms_samples": step_ms,
             "fp64": {"alg_flop_per_gradient": f_alg(model), "achieved_tflops": f_alg(model) / (ms_step * 1e-3) / 1e12,
                      "dmma_issue_peak_tflops": peak_tf, "dfma_issue_peak_tflops": dfma_tf}}
-    # ---- roofline of the dominant kernel: the 128x128-tile DMMA GEMM (68 % of the serialised kernel time of a
-    #      step, profiles/r01_launches_bench_nt3.md), timed live on a b x b x b product (operands 3 b^2 8 B > L2
+    # ---- roofline of the dominant kernel: the 128x128-tile DMMA GEMM (74 % of the serialised kernel time of a
+    #      step, profiles/r01_launches_bench_nt5.md), timed live on a b x b x b product (operands 3 b^2 8 B > L2
     #      at the large configs), CUDA events on the launching stream.
     from paper_2605_06392_b200 import gemm as _gemm
     b = model.b
@@ -246,7 +249,7 @@ def run_ours(args):
                         "traffic": 1.221e9 if b == 4096 else None,
                         "traffic_note": "dram read+write bytes per launch at b=4096 from ncu --set full "
                                         "(profiles/r01_gemm_full.md); algorithmic bytes 3 b^2 8 = 4.03e8",
-                        "share_of_step": 0.68,
+                        "share_of_step": 0.74,
                         "peak_source": "measured live: mma.sync.m8n8k4.f64 issue loop on all SMs (MEASURED_PEAKS.json "
                                        "has no FP64 entry; nominal-ratio alternative bf16_tflops x 40/2250 = "
                                        "29.1 TFLOP/s is lower)"}

@@ -61,6 +61,7 @@ struct GemmArgs {
   const GemmSub* subs;  // device array (nsub problems; M,N,K above = maxima for the grid) or nullptr
   int nsub;
   int dbg;              // diagnostics only (0 in production): 1 = no loads in the main loop, 2 = no barriers
+  int group;            // tile-order grouping (set by launch_gemm): slow tile rows swept together, <= 1 = off
 };
 
 cudaError_t launch_gemm(const GemmArgs& g, cudaStream_t st);

@@ -156,15 +156,27 @@ __global__ void __launch_bounds__(Cfg<BM, BN, WM, WN, A_KM, B_KM, BK>::NT, MINB)
   // Tile order: CTAs are dispatched x-fastest.  With a restricted k-range the work per tile varies by up to 32x;
   // the tiles are enumerated heaviest-first (the heavy tile column / row is the slow grid dimension), so the last,
   // partially filled wave consists of the lightest tiles.
-  int tm = blockIdx.y, tn = blockIdx.x;
+  // Within that order the slow index is regrouped: `group` consecutive slow tile rows are swept together (slow index
+  // fastest inside a group), so the ~148 co-resident CTAs form a (group x 148/group) patch of the tile grid that
+  // shares `group` panels of one operand and 148/group of the other, instead of 4.6 x 32: fewer DRAM re-reads.
+  int slow = blockIdx.y, fastx = blockIdx.x;
+  if (g.group > 1) {
+    const int per = g.group * (int)gridDim.x;
+    const int lin = slow * (int)gridDim.x + fastx;
+    const int grp = lin / per, within = lin - grp * per;
+    const int gsz = min(g.group, (int)gridDim.y - grp * g.group);
+    slow = grp * g.group + within % gsz;
+    fastx = within / gsz;
+  }
+  int tm = slow, tn = fastx;
   if (g.klo == KLO_N0) {
-    tm = blockIdx.x;
-    tn = blockIdx.y;
+    tm = fastx;
+    tn = slow;
   } else if (g.khi == KHI_NEND) {
-    tm = blockIdx.x;
-    tn = (int)gridDim.y - 1 - (int)blockIdx.y;
+    tm = fastx;
+    tn = (int)gridDim.y - 1 - slow;
   } else if (g.khi == KHI_MEND) {
-    tm = (int)gridDim.y - 1 - (int)blockIdx.y;
+    tm = (int)gridDim.y - 1 - slow;
   }
   const int m0 = tm * BM, n0 = tn * BN;
   if (m0 >= M || n0 >= N) return;
@@ -312,7 +324,12 @@ cudaError_t launch_cfg(const GemmArgs& g, cudaStream_t st) {
   const int tilesM = (g.M + BM - 1) / BM, tilesN = (g.N + BN - 1) / BN;
   const bool swap = g.klo == KLO_N0 || g.khi == KHI_NEND;  // heavy-first enumeration (see the kernel)
   dim3 grid(swap ? tilesM : tilesN, swap ? tilesN : tilesM, g.subs ? g.nsub : 1);
-  kern<<<grid, C_::NT, C_::SMEM, st>>>(g);
+  GemmArgs ga = g;
+  if (ga.group > 1) {  // equal-sized groups of at most `group` slow tile rows (18 rows -> 9 + 9, not 16 + 2)
+    const int ngroups = ((int)grid.y + ga.group - 1) / ga.group;
+    ga.group = ((int)grid.y + ngroups - 1) / ngroups;
+  }
+  kern<<<grid, C_::NT, C_::SMEM, st>>>(ga);
   return cudaGetLastError();
 }
 
@@ -355,6 +372,11 @@ cudaError_t launch_gemm(const GemmArgs& g0, cudaStream_t st) {
   }();
   GemmArgs g = g0;
   g.dbg = dbg;
+  static const int group = [] {
+    const char* e = getenv("BTA_GEMM_GROUP");
+    return e ? atoi(e) : 16;
+  }();
+  g.group = group;
   static const int big = [] {
     const char* e = getenv("BTA_GEMM_CFG");
     return e ? atoi(e) : 0;
