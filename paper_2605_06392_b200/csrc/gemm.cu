@@ -356,7 +356,7 @@ long long big_tiles(const GemmArgs& g) {
 long long tile_threshold() {
   static const long long thresh = [] {
     const char* e = getenv("BTA_TILE_THRESH");
-    return e ? atoll(e) : 120LL;
+    return e ? atoll(e) : 180LL;
   }();
   return thresh;
 }
