@@ -33,6 +33,10 @@ def f_alg(model):
 
 
 def workload_name(idx, model):
+    if idx >= 5:
+        from workloads import EXTREME_NAMES
+        return (f"extreme[{idx}] {EXTREME_NAMES[idx]} (SURVEY.md 8(f) NEXT-4, not a BASELINE config): g={model.g} "
+                f"ns={model.ns} k={model.k} b={model.b} nt={model.nt} a={model.a} d={model.d} N={model.N}")
     return (f"configs[{idx}]: g={model.g} ns={model.ns} k={model.k} b={model.b} nt={model.nt} a={model.a} "
             f"d={model.d} N={model.N}")
 
@@ -115,7 +119,7 @@ def run_reference(args):
         return 0
     from workloads import CONFIGS
     full_model = CONFIGS[args.config][0]
-    nt_s = {0: 6, 1: 10, 2: 4, 3: 2, 4: 2}[args.config]
+    nt_s = {0: 6, 1: 10, 2: 4, 3: 2, 4: 2, 5: 2, 6: 1}[args.config]
     for _ in range(args.warmup if args.config < 2 else min(args.warmup, 1)):
         oracle_sample(args.config, nt_s)
     ts = []
@@ -221,7 +225,9 @@ def run_ours(args):
             "gpu_launches": int(launches),
             "stage_ms": stage_acc,
             "step_ms_samples": step_ms,
-            "fp64": {"alg_flop_per_gradient": f_alg(model), "achieved_tflops": f_alg(model) / (ms_step * 1e-3) / 1e12,
+            "fp64": {"alg_flop_per_gradient": f_alg(model),
+                     "carry_rebuild_flop_per_gradient": (10.0 / 3.0) * model.nt * float(model.b) ** 3
+                     if args.store == "carry" else 0.0, "achieved_tflops": f_alg(model) / (ms_step * 1e-3) / 1e12,
                      "dmma_issue_peak_tflops": peak_tf, "dfma_issue_peak_tflops": dfma_tf}}
     # ---- roofline of the dominant kernel: the 128x128-tile DMMA GEMM (74 % of the serialised kernel time of a
     #      step, profiles/r01_launches_bench_nt5.md), timed live on a b x b x b product (operands 3 b^2 8 B > L2
@@ -276,7 +282,7 @@ def run_ours(args):
                               "beta_bwd_over_fwd": (bwd / fwd) if fwd > 0 else None,
                               "note": "FD gradient = (2d+1) x inla_value (Eq. 2); paper reports 4.2-7.9x per-gradient "
                                       "speedup and c_AD 2.3-3.9 on GH200 (context only, BASELINE.md)"}
-    if rank == 0 and not args.no_cpu_baseline and world == 1:
+    if rank == 0 and not args.no_cpu_baseline and world == 1 and args.config <= 4:
         nt_s = {0: 6, 1: 10, 2: 4, 3: 2, 4: 2}[args.config]
         dt, est, nts, _ = oracle_sample(args.config, nt_s)
         line["cpu_baseline"] = {"value": 1.0 / est, "unit": UNIT, "cores": threads_used(), "kind": "oracle",

@@ -3,6 +3,8 @@ configs 2-4 in seconds, so these tests use (i) the oracle on an nt-truncated mod
 (ii) properties that hold at any size: the DCT closed form for log det Q_p and the Phase-C traces (pin P9), the
 sum rules P7/P8, the value identity P6, the residual Q_c x* = r on every row, the uniform-design closed form for
 log det Q_c and Phase A (pin P12), and the scalar assembly of f recomputed from the returned intermediates."""
+import os
+
 import numpy as np
 import pytest
 
@@ -17,9 +19,11 @@ from closed_form import closed_form
 TOL_F, TOL_G = 1e-9, 1e-6
 
 
-def _run(model, obs, th):
+def _run(model, obs, th, store=0):
     from paper_2605_06392_b200 import BtaModel
     M = BtaModel.from_workload(model, obs, device=0)
+    if store:
+        M.bta_set_store_mode(store)
     f, g = M.inla_value_and_grad(th)
     im = M.last_intermediates()
     M.close()
@@ -59,9 +63,21 @@ def _closed_form_prior(model, th):
 
 @pytest.mark.parametrize("idx", [2, 3, 4])
 def test_full_size_properties(idx):
+    _check_properties(idx, 0)
+
+
+@pytest.mark.skipif(os.environ.get("BTA_EXTREME") != "1",
+                    reason="minutes of GPU time and > 150 GB of HBM each: set BTA_EXTREME=1")
+@pytest.mark.parametrize("idx,store", [(5, 0), (6, 1)])
+def test_extreme_workload_properties(idx, store):
+    """WA1-like (nt = 512, factor mode) and WA2-like (b = 12288, carry mode) stand-ins."""
+    _check_properties(idx, store)
+
+
+def _check_properties(idx, store):
     model, obs, th = make_config(idx)
     k, nt, b, ns, a, N = model.k, model.nt, model.b, model.ns, model.a, model.N
-    f, g, im = _run(model, obs, th)
+    f, g, im = _run(model, obs, th, store)
     E, Lam, tau = O.unpack_theta(model, th)
     nprior = model.d - k
     # P9 / P10: prior log-determinant and Phase-C traces

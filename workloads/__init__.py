@@ -9,6 +9,7 @@ produced here; neither imports the other.
 """
 from .generate import (  # noqa: F401
     CONFIGS,
+    EXTREME_NAMES,
     Model,
     Obs,
     make_config,

@@ -108,7 +108,13 @@ CONFIGS = {
     2: (Model(g=48, k=1, nt=100, a=6), 200_000, 1002, None),
     3: (Model(g=32, k=3, nt=64, a=6), 50_000, 1003, None),
     4: (Model(g=64, k=1, nt=128, a=8), 1_000_000, 1004, None),
+    # two stand-ins shaped like the extremes of the paper's model zoo (
+    # not BASELINE.json configs): "WA1-like" = many time steps (b = 3072, nt = 512), "WA2-like" = very large
+    # blocks (b = 12288, nt = 48; needs the carry store mode to fit 180 GB).  Both multivariate (k = 3, d = 15).
+    5: (Model(g=32, k=3, nt=512, a=6), 400_000, 1005, None),
+    6: (Model(g=64, k=3, nt=48, a=6), 300_000, 1006, None),
 }
+EXTREME_NAMES = {5: "WA1-like (long time axis)", 6: "WA2-like (large blocks)"}
 
 
 def make_model(g: int, k: int, nt: int, a: int, h: float = 1.0, fixed_prec: float = 1e-3) -> Model:
