@@ -6,7 +6,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libbta_b200.so")
-SOURCES = ["gemm.cu", "diag.cu", "skinny.cu", "assemble.cu", "contract.cu", "sweep.cu", "model.cu", "api.cu",
+SOURCES = ["gemm.cu", "diag.cu", "leaf.cu", "skinny.cu", "assemble.cu", "contract.cu", "sweep.cu", "model.cu", "api.cu",
            "api_misc.cu", "peak.cu"]
 
 

@@ -72,6 +72,9 @@ bool gemm_uses_small_tiles(const GemmArgs& g);  // the 64x64-tile configuration 
 // ------------------------------------------------------------------------------------------------
 cudaError_t launch_potrf_inv_tile(double* A, int ld, int n, double* diagL, long long grow0,
                                   unsigned long long* pivot_flag, cudaStream_t st);
+// leaf.cu: the blocked (16-wide panels) version of the same leaf
+cudaError_t launch_potrf_inv_blocked(double* A, int ld, int n, double* diagL, long long grow0,
+                                     unsigned long long* pivot_flag, cudaStream_t st);
 cudaError_t launch_tip(const double* Tt, int a, int nr, int do_chol, double* LT, double* zT, double* xT, double* ZT,
                        double* diagL, long long grow0, unsigned long long* pivot_flag, cudaStream_t st);
 cudaError_t launch_zero_upper(double* A, int ld, int n, cudaStream_t st);

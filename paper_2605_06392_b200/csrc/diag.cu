@@ -251,6 +251,11 @@ __global__ void tip_inverse_kernel(const double* __restrict__ LT, int a, double*
 
 cudaError_t launch_potrf_inv_tile(double* A, int ld, int n, double* diagL, long long grow0,
                                   unsigned long long* pivot_flag, cudaStream_t st) {
+  static const int blocked = [] {
+    const char* e = getenv("BTA_LEAF");
+    return e ? atoi(e) : 1;
+  }();
+  if (blocked) return launch_potrf_inv_blocked(A, ld, n, diagL, grow0, pivot_flag, st);
   if (n <= 64)
     potrf_inv_tile_kernel<64, 8><<<1, 256, 0, st>>>(A, ld, n, diagL, grow0, pivot_flag);
   else if (n <= 128)
