@@ -252,7 +252,7 @@ __global__ void tip_inverse_kernel(const double* __restrict__ LT, int a, double*
 cudaError_t launch_potrf_inv_tile(double* A, int ld, int n, double* diagL, long long grow0,
                                   unsigned long long* pivot_flag, cudaStream_t st) {
   static const int blocked = [] {
-    const char* e = getenv("BTA_LEAF");
+    const char* e = getenv("BTA_LEAF_BLOCKED");
     return e ? atoi(e) : 1;
   }();
   if (blocked) return launch_potrf_inv_blocked(A, ld, n, diagL, grow0, pivot_flag, st);
