@@ -634,6 +634,22 @@ int enqueue_gradient_twisted(bta_ctx* c, void* ws, cudaStream_t s0, bool timed, 
       }
   }
   auto join_lanes = [&](int m, int q) { return chain_to_big(ch[m][q], st[m][q == 2 ? 0 : q]); };
+  for (int m = 0; m < 2; ++m)
+    for (int q = 0; q < 3; ++q) ch[m][q].trace_id = 3 * m + q;
+  {
+    // phase stagger: chain i starts its first POTRF when chain i-1 has finished its own (order Q_c up, Q_c down,
+    // Q_p up, Q_p down), so that the four chains do not run their latency-bound recursions in lock-step
+    static const int stagger = [] {
+      const char* e = getenv("BTA_STAGGER");
+      return e ? atoi(e) : 1;
+    }();
+    if (stagger && !value_only)
+      for (int i = 0; i < 3; ++i) {
+        if (ch[i / 2][i % 2].nt < 1 || ch[(i + 1) / 2][(i + 1) % 2].nt < 1) continue;
+        ch[i / 2][i % 2].stagger_rec = ev[24 + i];
+        ch[(i + 1) / 2][(i + 1) % 2].stagger_wait = ev[24 + i];
+      }
+  }
 
   // ---- assemble: D (all blocks), arrow/rhs rows, tip on the up stream; coupling blocks per sub-chain
   // The diagonal blocks are assembled lazily, a few blocks ahead of each sub-chain (assemble_ahead below): the 2 nt
@@ -807,7 +823,20 @@ int value_and_grad_impl(bta_ctx* c, const double* theta, double* f, double* grad
     }
   }
   c->grad_calls++;
-  int rc = check_pivot(c, sync_stream);  // synchronises the stream (and, through ev[7], the side stream)
+  int rc = check_pivot(c, sync_stream);
+  if (c->trace_on && !c->trace.empty()) {  // diagnostic timeline: "<chain> <t> <tag> <ms since the call started>"
+    if (FILE* fp = fopen(getenv("BTA_TRACE"), "w")) {
+      for (auto& r : c->trace) {
+        float ms = 0.f;
+        cudaEventSynchronize(r.e);
+        cudaEventElapsedTime(&ms, ev[0], r.e);
+        fprintf(fp, "%d %d %d %.4f\n", r.chain, r.t, r.tag, ms);
+      }
+      fclose(fp);
+    }
+    for (auto& r : c->trace) cudaEventDestroy(r.e);
+    c->trace.clear();
+  }  // synchronises the stream (and, through ev[7], the side stream)
   const double* o = c->host_pinned + 64;
   if (f) *f = o[0];
   if (grad && !value_only) memcpy(grad, o + 1, md.d * sizeof(double));

@@ -153,7 +153,18 @@ struct bta_ctx {
   double last_ld[2], last_quad;
   std::vector<double> last_parts, last_rss;
   double* last_x_dev;                // device pointer into the caller's workspace (valid until it is reused)
+  // BTA_TRACE=<file>: phase marks of the sweeps (diagnostic timeline; events are created on demand)
+  struct TraceRec { cudaEvent_t e; int chain, t, tag; };
+  std::vector<TraceRec> trace;
+  bool trace_on;
 };
+inline void trace_mark(bta_ctx* c, cudaStream_t st, int chain, int t, int tag) {
+  if (!c->trace_on) return;
+  cudaEvent_t e;
+  cudaEventCreate(&e);
+  cudaEventRecord(e, st);
+  c->trace.push_back({e, chain, t, tag});
+}
 
 #define BTA_COUNT(ctx) ((ctx)->launches++)
 

@@ -364,6 +364,21 @@ long long tile_threshold() {
 
 bool gemm_uses_small_tiles(const GemmArgs& g) { return big_tiles(g) < tile_threshold(); }
 
+namespace {
+// Latency-bound launches (the deep levels of the POTRF+TRTRI recursion: a few dozen 64x64 tiles, one dependent kernel
+// after the other): 32x32 tiles (4 warps, 16x16 per warp) shorten each CTA's k-loop fourfold (4 DMMAs per k-step and
+// warp instead of 16) and spread the product over four times as many CTAs.
+bool gemm_uses_tiny_tiles(const GemmArgs& g) {
+  static const long long thresh = [] {
+    const char* e = getenv("BTA_TINY_THRESH");
+    return e ? atoll(e) : 148LL;
+  }();
+  long long t64 = (long long)((g.M + 63) / 64) * ((g.N + 63) / 64) * (g.subs ? g.nsub : 1);
+  if (g.out != OUT_FULL) t64 = t64 / 2 + 1;
+  return t64 <= thresh;
+}
+}  // namespace
+
 cudaError_t launch_gemm(const GemmArgs& g0, cudaStream_t st) {
   if (g0.M <= 0 || g0.N <= 0) return cudaSuccess;
   static const int dbg = [] {
@@ -389,5 +404,6 @@ cudaError_t launch_gemm(const GemmArgs& g0, cudaStream_t st) {
       default: return launch_mode<128, 128, 32, 64, 1, 16>(g, st);
     }
   }
+  if (gemm_uses_tiny_tiles(g)) return launch_mode<32, 32, 16, 16, 4, 16>(g, st);
   return launch_mode<64, 64, 32, 32, 2, 16>(g, st);
 }

@@ -103,6 +103,7 @@ extern "C" int bta_create(bta_ctx** out, const bta_model_desc* desc, const bta_o
     c->graph_launches[q] = 0;
   }
   c->grad_calls = 0;
+  c->trace_on = getenv("BTA_TRACE") != nullptr;
   c->store_mode = BTA_STORE_FACTOR;
   for (auto& e : c->ev) BTA_CUDA_OK(cudaEventCreate(&e));
   {

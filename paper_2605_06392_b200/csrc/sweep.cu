@@ -70,7 +70,11 @@ cudaError_t potrf_inv(bta_ctx* c, Chain* lch, double* A, int ld, int lo, int hi,
   const int ntile = (n + LEAF - 1) / LEAF;
   const int mid = lo + LEAF * ((ntile + 1) / 2);
   const int s1 = mid - lo, s2 = hi - mid;
+  const bool top = lch && n == ld && c->trace_on;
+#define PM(tag) \
+  if (top) trace_mark(c, lane(lch, st, lch->on_small), lch->trace_id, (int)(grow0 / ld), tag)
   CK(potrf_inv(c, lch, A, ld, lo, mid, T1, T2, diagL, grow0, st));
+  PM(10);
   double* A11 = A + (long long)lo * ld + lo;
   double* A21 = A + (long long)mid * ld + lo;
   double* A22 = A + (long long)mid * ld + mid;
@@ -79,7 +83,9 @@ cudaError_t potrf_inv(bta_ctx* c, Chain* lch, double* A, int ld, int lo, int hi,
   CK(gemm_lane(lch, st, G(GEMM_NT, s2, s1, s1, 1.0, A21, ld, A11, ld, 0.0, L21, ld, KLO_ZERO, KHI_NEND, OUT_FULL)));
   CK(gemm_lane(lch, st, G(GEMM_NT, s2, s2, s1, -1.0, L21, ld, L21, ld, 1.0, A22, ld, KLO_ZERO, KHI_K, OUT_LOWER)));
   c->launches += 2;
+  PM(11);
   CK(potrf_inv(c, lch, A, ld, mid, hi, T1, T2, diagL, grow0, st));
+  PM(12);
   CK(gemm_lane(lch, st, G(GEMM_NN, s2, s1, s1, 1.0, L21, ld, A11, ld, 0.0, LX, ld, KLO_N0, KHI_K, OUT_FULL)));
   CK(gemm_lane(lch, st, G(GEMM_NN, s2, s1, s2, -1.0, A22, ld, LX, ld, 0.0, A21, ld, KLO_ZERO, KHI_MEND, OUT_FULL)));
   c->launches += 2;
@@ -148,7 +154,10 @@ cudaError_t chain_forward_step(Chain& ch, int t, cudaStream_t st) {
       ld_src = ld_tmp;
     }
   }
+#define TM(tag) trace_mark(c, lane(lch, st, ch.on_small), ch.trace_id, t, tag)
+  TM(0);
   if (ch.factor_blocks) {
+    if (t == 0 && ch.stagger_wait) CK(cudaStreamWaitEvent(SB, ch.stagger_wait, 0));
     if (ch.zero_upper) {
       CK(launch_zero_upper(At, b, b, SB));
       BTA_COUNT(c);
@@ -159,7 +168,9 @@ cudaError_t chain_forward_step(Chain& ch, int t, cudaStream_t st) {
     } else {
       CK(potrf_inv(c, lch, Dt, b, 0, b, ch.W2, ch.W3, ch.dvec ? ch.dvec + tg * b : nullptr, tg * b, st));
     }
+    if (t == 0 && ch.stagger_rec) CK(cudaEventRecord(ch.stagger_rec, SB));
   }
+  TM(1);
   if (P > 0) {
     //   R^_t = R~_t X_t^T
     double* Rh = ch.Rout + t * ch.rout_stride;
@@ -188,8 +199,10 @@ cudaError_t chain_forward_step(Chain& ch, int t, cudaStream_t st) {
       Bo = ch.Bout + t * ch.b_stride;
       dst = (Bi == Bo) ? ch.W1 : Bo;
     }
+    TM(2);
     CK(launch_gemm(G(GEMM_NT, b, b, b, 1.0, Bi, b, Dt, b, 0.0, dst, b, KLO_ZERO, KHI_NEND, OUT_FULL), SB));
     BTA_COUNT(c);
+    TM(3);
     if (t < nt - 1) {  // the Schur update of a separator is applied by the separator stage (two chains meet there)
       CK(launch_gemm(G(GEMM_NT, b, b, b, -1.0, dst, b, dst, b, 1.0, ch.D + (t + 1) * ch.d_stride, b, KLO_ZERO, KHI_K,
                        OUT_LOWER),
@@ -197,6 +210,7 @@ cudaError_t chain_forward_step(Chain& ch, int t, cudaStream_t st) {
       BTA_COUNT(c);
     }
     if (dst != Bo) CK(cudaMemcpyAsync(Bo, dst, bb * sizeof(double), cudaMemcpyDeviceToDevice, SB));
+    TM(4);
   }
   return cudaSuccess;
 }
