@@ -637,18 +637,13 @@ int enqueue_gradient_twisted(bta_ctx* c, void* ws, cudaStream_t s0, bool timed, 
   for (int m = 0; m < 2; ++m)
     for (int q = 0; q < 3; ++q) ch[m][q].trace_id = 3 * m + q;
   {
-    // phase stagger: chain i starts its first POTRF when chain i-1 has finished its own (order Q_c up, Q_c down,
-    // Q_p up, Q_p down), so that the four chains do not run their latency-bound recursions in lock-step
-    static const int stagger = [] {
-      const char* e = getenv("BTA_STAGGER");
+    static const int split = [] {
+      const char* e = getenv("BTA_SPLIT");
       return e ? atoi(e) : 1;
     }();
-    if (stagger && !value_only)
-      for (int i = 0; i < 3; ++i) {
-        if (ch[i / 2][i % 2].nt < 1 || ch[(i + 1) / 2][(i + 1) % 2].nt < 1) continue;
-        ch[i / 2][i % 2].stagger_rec = ev[24 + i];
-        ch[(i + 1) / 2][(i + 1) % 2].stagger_wait = ev[24 + i];
-      }
+    if (split)
+      for (int m = 0; m < 2; ++m)
+        for (int q = 0; q < 2; ++q) ch[m][q].xs = c->s_x[2 * m + q];
   }
 
   // ---- assemble: D (all blocks), arrow/rhs rows, tip on the up stream; coupling blocks per sub-chain

@@ -145,6 +145,7 @@ struct bta_ctx {
   cudaStream_t s_aux[2];             // two-way elimination: the down chains of Q_c and Q_p
   cudaEvent_t ev[32];
   cudaStream_t s_hi[4];              // high-priority companions of the four chains (small kernels)
+  cudaStream_t s_x[4];               // side streams of the four chains (off-chain work of the forward steps)
   cudaEvent_t ev_sw[256];            // lane-switch events, used round-robin
   unsigned ev_sw_next;
   long long launches;

@@ -7,6 +7,7 @@
 // 64-bit fragment loads are bank-conflict-free (leading dimension = 4 mod 16 doubles); accumulators live
 // in registers.  Triangular operands are exploited by restricting the k-range per output tile
 // (KLO_*/KHI_*), symmetric outputs by computing the lower tiles only (OUT_LOWER*).
+#include <algorithm>
 #include <cstdlib>
 
 #include "common.cuh"
@@ -362,7 +363,28 @@ long long tile_threshold() {
 }
 }  // namespace
 
-bool gemm_uses_small_tiles(const GemmArgs& g) { return big_tiles(g) < tile_threshold(); }
+// Small tiles (64x64, two CTAs per SM) for launches of fewer than ~1.2 waves of big tiles, and wherever the last,
+// partially filled wave of big tiles would cost more than the small tiles' lower rate (0.97 of the big tile's):
+// e.g. the lower-only products at b = 3072 are 300 big tiles = 2.03 waves (3 waves: 68 %) but 1176 small ones =
+// 3.97 waves of 296.
+bool gemm_uses_small_tiles(const GemmArgs& g) {
+  const long long t128 = big_tiles(g);
+  if (t128 < tile_threshold()) return true;
+  static const int wave_rule = [] {
+    const char* e = getenv("BTA_TILE_WAVES");
+    return e ? atoi(e) : 1;
+  }();
+  if (!wave_rule) return false;
+  const long long nb = g.subs ? g.nsub : 1;
+  const long long m64 = (g.M + 63) / 64, n64 = (g.N + 63) / 64;
+  const long long t64 = (g.out != OUT_FULL ? std::min(m64, n64) * (std::min(m64, n64) + 1) / 2 : m64 * n64) * nb;
+  const long long m128 = (g.M + 127) / 128, n128 = (g.N + 127) / 128;
+  const long long x128 =
+      (g.out != OUT_FULL ? std::min(m128, n128) * (std::min(m128, n128) + 1) / 2 : m128 * n128) * nb;
+  const double e128 = (double)x128 / (double)(((x128 + 147) / 148) * 148);
+  const double e64 = 0.97 * (double)t64 / (double)(((t64 + 295) / 296) * 296);
+  return e64 > e128 + 0.03;
+}
 
 namespace {
 // Latency-bound launches (the deep levels of the POTRF+TRTRI recursion: a few dozen 64x64 tiles, one dependent kernel

@@ -110,6 +110,7 @@ extern "C" int bta_create(bta_ctx** out, const bta_model_desc* desc, const bta_o
     int plo = 0, phi = 0;
     BTA_CUDA_OK(cudaDeviceGetStreamPriorityRange(&plo, &phi));
     for (auto& q : c->s_hi) BTA_CUDA_OK(cudaStreamCreateWithPriority(&q, cudaStreamNonBlocking, phi));
+    for (auto& q : c->s_x) BTA_CUDA_OK(cudaStreamCreateWithPriority(&q, cudaStreamNonBlocking, plo));
     for (auto& e : c->ev_sw) BTA_CUDA_OK(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
     c->ev_sw_next = 0;
   }
@@ -152,6 +153,7 @@ extern "C" int bta_destroy(bta_ctx* c) {
   for (auto& q : c->s_aux) cudaStreamDestroy(q);
   for (auto& e : c->ev) cudaEventDestroy(e);
   for (auto& q : c->s_hi) cudaStreamDestroy(q);
+  for (auto& q : c->s_x) cudaStreamDestroy(q);
   for (auto& e : c->ev_sw) cudaEventDestroy(e);
   delete c;
   return BTA_OK;

@@ -92,6 +92,74 @@ cudaError_t potrf_inv(bta_ctx* c, Chain* lch, double* A, int ld, int lo, int hi,
   return cudaSuccess;
 }
 
+// Forward step with the coupling block folded into the top level of the POTRF+TRTRI recursion (factor mode).
+// With A = [[A11, .], [A21, A22]], X = L^-1 = [[X11, 0], [X21, X22]] and B = [B1 | B2]:
+//   L_B = B X^T = [ B1 X11^T | (B2 - L_B1 L21^T) X22^T ],   S = L_B1 L_B1^T + L_B2 L_B2^T,   X21 = -X22 (L21 X11).
+// L_B1 and its half of the Schur update need only X11, and X21 is not needed by the factorisation at all, so they
+// run on the chain's side stream `xs` next to the second half of the recursion; the dependent chain of a step is
+// potrf_inv(A11) -> L21, A22 -> potrf_inv(A22) -> L_B2 -> second half of S instead of ... -> X21 -> L_B -> S.  Same
+// flops.  B (its right half) is updated in place; L_B goes to `dst`.
+cudaError_t potrf_inv_coupled(bta_ctx* c, Chain* lch, double* A, int b, double* Bi, double* dst, double* Dnext,
+                              double* T1, double* T2, double* diagL, long long grow0, cudaStream_t st,
+                              cudaStream_t xs) {
+  Chain& ch = *lch;
+  const int t = (int)(grow0 / b);
+  const int LEAF = 128;
+  const int ntile = (b + LEAF - 1) / LEAF;
+  const int mid = LEAF * ((ntile + 1) / 2);
+  const int s1 = mid, s2 = b - mid, ld = b;
+  auto ev_next = [&]() { return c->ev_sw[(c->ev_sw_next++) % BTA_NSW]; };
+  auto cur = [&]() { return lane(lch, st, ch.on_small); };
+#define XM(tag) trace_mark(c, cur(), ch.trace_id, t, tag)
+  CK(potrf_inv(c, lch, A, ld, 0, mid, T1, T2, diagL, grow0, st));
+  XM(10);
+  cudaEvent_t e1 = ev_next(), e2 = ev_next(), e3 = ev_next(), e4 = ev_next(), e5 = ev_next();
+  CK(cudaEventRecord(e1, cur()));
+  CK(cudaStreamWaitEvent(xs, e1, 0));
+  //   side: L_B1 = B1 X11^T, S += L_B1 L_B1^T
+  CK(launch_gemm(G(GEMM_NT, b, s1, s1, 1.0, Bi, b, A, ld, 0.0, dst, b, KLO_ZERO, KHI_NEND, OUT_FULL), xs));
+  CK(cudaEventRecord(e2, xs));
+  if (Dnext)
+    CK(launch_gemm(G(GEMM_NT, b, b, s1, -1.0, dst, b, dst, b, 1.0, Dnext, b, KLO_ZERO, KHI_K, OUT_LOWER), xs));
+  CK(cudaEventRecord(e3, xs));
+  c->launches += Dnext ? 2 : 1;
+  //   main: second half of the recursion
+  double* A21 = A + (long long)mid * ld;
+  double* A22 = A + (long long)mid * ld + mid;
+  double* L21 = T1 + (long long)mid * ld;
+  double* LX = T2 + (long long)mid * ld;
+  CK(gemm_lane(lch, st, G(GEMM_NT, s2, s1, s1, 1.0, A21, ld, A, ld, 0.0, L21, ld, KLO_ZERO, KHI_NEND, OUT_FULL)));
+  CK(gemm_lane(lch, st, G(GEMM_NT, s2, s2, s1, -1.0, L21, ld, L21, ld, 1.0, A22, ld, KLO_ZERO, KHI_K, OUT_LOWER)));
+  c->launches += 2;
+  XM(11);
+  CK(potrf_inv(c, lch, A, ld, mid, b, T1, T2, diagL, grow0, st));
+  XM(12);
+  //   side: X21 = -X22 (L21 X11), off the dependent chain
+  CK(cudaEventRecord(e4, cur()));
+  CK(cudaStreamWaitEvent(xs, e4, 0));
+  CK(launch_gemm(G(GEMM_NN, s2, s1, s1, 1.0, L21, ld, A, ld, 0.0, LX, ld, KLO_N0, KHI_K, OUT_FULL), xs));
+  CK(launch_gemm(G(GEMM_NN, s2, s1, s2, -1.0, A22, ld, LX, ld, 0.0, A21, ld, KLO_ZERO, KHI_MEND, OUT_FULL), xs));
+  CK(cudaEventRecord(e5, xs));
+  c->launches += 2;
+  //   main: L_B2 = (B2 - L_B1 L21^T) X22^T, S += L_B2 L_B2^T
+  CK(cudaStreamWaitEvent(SB, e2, 0));
+  CK(launch_gemm(G(GEMM_NT, b, s2, s1, -1.0, dst, b, L21, ld, 1.0, Bi + mid, b, KLO_ZERO, KHI_K, OUT_FULL), SB));
+  CK(launch_gemm(G(GEMM_NT, b, s2, s2, 1.0, Bi + mid, b, A22, ld, 0.0, dst + mid, b, KLO_ZERO, KHI_NEND, OUT_FULL),
+                 SB));
+  c->launches += 2;
+  XM(3);
+  CK(cudaStreamWaitEvent(SB, e3, 0));
+  if (Dnext) {
+    CK(launch_gemm(G(GEMM_NT, b, b, s2, -1.0, dst + mid, b, dst + mid, b, 1.0, Dnext, b, KLO_ZERO, KHI_K, OUT_LOWER),
+                   SB));
+    BTA_COUNT(c);
+  }
+  CK(cudaStreamWaitEvent(SB, e5, 0));
+  XM(4);
+#undef XM
+  return cudaSuccess;
+}
+
 namespace {
 __global__ void tip_init_kernel(int a, int nr, const double* __restrict__ T, int ldt_in,
                                 const double* __restrict__ rhs_tip, int tip_stride, double* __restrict__ Tt, int zero) {
@@ -156,8 +224,8 @@ cudaError_t chain_forward_step(Chain& ch, int t, cudaStream_t st) {
   }
 #define TM(tag) trace_mark(c, lane(lch, st, ch.on_small), ch.trace_id, t, tag)
   TM(0);
+  bool coupled = false;  // L_B and the Schur update were folded into the recursion (potrf_inv_coupled)
   if (ch.factor_blocks) {
-    if (t == 0 && ch.stagger_wait) CK(cudaStreamWaitEvent(SB, ch.stagger_wait, 0));
     if (ch.zero_upper) {
       CK(launch_zero_upper(At, b, b, SB));
       BTA_COUNT(c);
@@ -166,9 +234,23 @@ cudaError_t chain_forward_step(Chain& ch, int t, cudaStream_t st) {
       CK(cudaMemcpyAsync(Dt, At, bb * sizeof(double), cudaMemcpyDeviceToDevice, SB));
       CK(potrf_inv(c, lch, Dt, b, 0, b, ch.W1, ch.Bs, ch.dvec ? ch.dvec + tg * b : nullptr, tg * b, st));
     } else {
-      CK(potrf_inv(c, lch, Dt, b, 0, b, ch.W2, ch.W3, ch.dvec ? ch.dvec + tg * b : nullptr, tg * b, st));
+      static const int split_maxb = [] {
+        const char* e = getenv("BTA_SPLIT_MAXB");
+        return e ? atoi(e) : 1024;
+      }();
+      const bool has_coupling = t < nt - 1 || ch.tail_coupling;
+      coupled = has_coupling && ch.xs && b > 128 && b <= split_maxb;
+      if (coupled) {
+        double* Bi = ch.Bin + t * ch.b_stride;
+        double* Bo = ch.Bout + t * ch.b_stride;
+        double* dst = (Bi == Bo) ? ch.W1 : Bo;
+        CK(potrf_inv_coupled(c, lch, Dt, b, Bi, dst, t < nt - 1 ? ch.D + (t + 1) * ch.d_stride : nullptr, ch.W2, ch.W3,
+                             ch.dvec ? ch.dvec + tg * b : nullptr, tg * b, st, ch.xs));
+        if (dst != Bo) CK(cudaMemcpyAsync(Bo, dst, bb * sizeof(double), cudaMemcpyDeviceToDevice, SB));
+      } else {
+        CK(potrf_inv(c, lch, Dt, b, 0, b, ch.W2, ch.W3, ch.dvec ? ch.dvec + tg * b : nullptr, tg * b, st));
+      }
     }
-    if (t == 0 && ch.stagger_rec) CK(cudaEventRecord(ch.stagger_rec, SB));
   }
   TM(1);
   if (P > 0) {
@@ -187,7 +269,7 @@ cudaError_t chain_forward_step(Chain& ch, int t, cudaStream_t st) {
       }
     }
   }
-  if ((t < nt - 1 || ch.tail_coupling) && ch.factor_blocks) {
+  if ((t < nt - 1 || ch.tail_coupling) && ch.factor_blocks && !coupled) {
     const double* Bi;
     double *Bo, *dst;
     if (ch.carry) {

@@ -29,10 +29,8 @@ struct Chain {
   cudaStream_t hi = nullptr;   // optional high-priority companion stream for the small kernels of this chain
   bool on_small = false;       // which lane the chain's work currently ends on
   bool lanes_bwd = true;       // use the small lane in the backward sweep too
-  // phase stagger between concurrent chains: at local block 0 the forward step waits for stagger_wait before its
-  // POTRF and records stagger_rec after it, so the chains' latency-bound and GEMM-bound phases interleave
-  cudaEvent_t stagger_wait = nullptr, stagger_rec = nullptr;
   int trace_id = -1;           // BTA_TRACE label of this chain
+  cudaStream_t xs = nullptr;   // optional side stream: work of a forward step that is off its dependent chain
   int tg(int s) const { return t0 + tdir * s; }
   int tB(int s) const { return tdir > 0 ? tg(s) : tg(s) - 1; }   // index of the sub-diagonal block between s, s+1
 
