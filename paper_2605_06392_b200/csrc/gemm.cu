@@ -346,8 +346,8 @@ cudaError_t launch_mode(const GemmArgs& g, cudaStream_t st) {
 
 }  // namespace
 
-// Tile choice: 128x128 (8 warps, 32x64 per warp) once the problem fills the chip with big tiles,
-// else 64x64 (4 warps, 32x32 per warp) for more CTAs on small problems.
+// Tile choice: 128x128 (16 warps, 32x32 per warp) once the problem fills the chip with big tiles,
+// else 64x64 (4 warps, 32x32 per warp, three CTAs per SM), and 32x32 for the latency-bound launches.
 namespace {
 long long big_tiles(const GemmArgs& g) {
   long long tiles128 = (long long)((g.M + 127) / 128) * ((g.N + 127) / 128) * (g.subs ? g.nsub : 1);
@@ -363,10 +363,10 @@ long long tile_threshold() {
 }
 }  // namespace
 
-// Small tiles (64x64, two CTAs per SM) for launches of fewer than ~1.2 waves of big tiles, and wherever the last,
+// Small tiles (64x64, three CTAs per SM) for launches of fewer than ~1.2 waves of big tiles, and wherever the last,
 // partially filled wave of big tiles would cost more than the small tiles' lower rate (0.97 of the big tile's):
 // e.g. the lower-only products at b = 3072 are 300 big tiles = 2.03 waves (3 waves: 68 %) but 1176 small ones =
-// 3.97 waves of 296.
+// 2.65 waves of 444.
 bool gemm_uses_small_tiles(const GemmArgs& g) {
   const long long t128 = big_tiles(g);
   if (t128 < tile_threshold()) return true;
@@ -382,7 +382,7 @@ bool gemm_uses_small_tiles(const GemmArgs& g) {
   const long long x128 =
       (g.out != OUT_FULL ? std::min(m128, n128) * (std::min(m128, n128) + 1) / 2 : m128 * n128) * nb;
   const double e128 = (double)x128 / (double)(((x128 + 147) / 148) * 148);
-  const double e64 = 0.97 * (double)t64 / (double)(((t64 + 295) / 296) * 296);
+  const double e64 = 0.97 * (double)t64 / (double)(((t64 + 443) / 444) * 444);
   return e64 > e128 + 0.03;
 }
 
@@ -421,11 +421,20 @@ cudaError_t launch_gemm(const GemmArgs& g0, cudaStream_t st) {
   if (!gemm_uses_small_tiles(g)) {
     switch (big) {
       case 1: return launch_mode<128, 128, 32, 64, 1, 32>(g, st);
-      case 2: return launch_mode<128, 128, 32, 32, 1, 16>(g, st);
+      case 2: return launch_mode<128, 128, 32, 64, 1, 16>(g, st);
       case 3: return launch_mode<128, 128, 32, 32, 1, 32>(g, st);
-      default: return launch_mode<128, 128, 32, 64, 1, 16>(g, st);
+      default: return launch_mode<128, 128, 32, 32, 1, 16>(g, st);  // 16 warps, 32x32 per warp
     }
   }
   if (gemm_uses_tiny_tiles(g)) return launch_mode<32, 32, 16, 16, 4, 16>(g, st);
-  return launch_mode<64, 64, 32, 32, 2, 16>(g, st);
+  static const int small = [] {
+    const char* e = getenv("BTA_GEMM_SMALL");
+    return e ? atoi(e) : 3;
+  }();
+  switch (small) {
+    case 1: return launch_mode<64, 64, 32, 16, 2, 16>(g, st);
+    case 2: return launch_mode<64, 64, 32, 16, 3, 16>(g, st);
+    case 0: return launch_mode<64, 64, 32, 32, 2, 16>(g, st);
+    default: return launch_mode<64, 64, 32, 32, 3, 16>(g, st);  // three CTAs per SM
+  }
 }
