@@ -229,7 +229,7 @@ def run_ours(args):
                      "carry_rebuild_flop_per_gradient": (10.0 / 3.0) * model.nt * float(model.b) ** 3
                      if args.store == "carry" else 0.0, "achieved_tflops": f_alg(model) / (ms_step * 1e-3) / 1e12,
                      "dmma_issue_peak_tflops": peak_tf, "dfma_issue_peak_tflops": dfma_tf}}
-    # ---- roofline of the dominant kernel: the 128x128-tile DMMA GEMM (74 % of the serialised kernel time of a
+    # ---- roofline of the dominant kernel: the 128x128-tile DMMA GEMM (79 % of the serialised kernel time of a
     #      step, profiles/r01_launches_bench_nt5.md), timed live on a b x b x b product (operands 3 b^2 8 B > L2
     #      at the large configs), CUDA events on the launching stream.
     from paper_2605_06392_b200 import gemm as _gemm
@@ -252,10 +252,10 @@ def run_ours(args):
     line["roofline"] = {"bound": "tensor", "kernel": "gemm_kernel (FP64 mma.sync m8n8k4 / DMMA.8x8x4), C = A B, b^3",
                         "achieved": gemm_tf, "peak": peak_tf, "unit": "TFLOP/s", "frac": gemm_tf / peak_tf,
                         "launch_ms": gemm_ms, "alg_flop_per_launch": 2.0 * float(b) ** 3,
-                        "traffic": 1.221e9 if b == 4096 else None,
+                        "traffic": 0.940e9 if b == 4096 else None,
                         "traffic_note": "dram read+write bytes per launch at b=4096 from ncu --set full "
                                         "(profiles/r01_gemm_full.md); algorithmic bytes 3 b^2 8 = 4.03e8",
-                        "share_of_step": 0.74,
+                        "share_of_step": 0.786,
                         "peak_source": "measured live: mma.sync.m8n8k4.f64 issue loop on all SMs (MEASURED_PEAKS.json "
                                        "has no FP64 entry; nominal-ratio alternative bf16_tflops x 40/2250 = "
                                        "29.1 TFLOP/s is lower)"}
