@@ -3,7 +3,7 @@
 // The dense b x b block products of the BTA sweeps (Algorithm 1's TRSM/SYRK steps, and
 // the selected-inversion products) all run through this kernel.  sm_100a has no
 // tcgen05 f64 kind; the FP64 tensor path is warp-level `mma.sync.m8n8k4.f64` (SASS DMMA.8x8x4).
-// Operands are staged in shared memory by a 3-stage cp.async (LDGSTS) pipeline in layouts chosen so the
+// Operands are staged in shared memory by a 3-stage (template parameter) cp.async (LDGSTS) pipeline in layouts chosen so the
 // 64-bit fragment loads are bank-conflict-free (leading dimension = 4 mod 16 doubles); accumulators live
 // in registers.  Triangular operands are exploited by restricting the k-range per output tile
 // (KLO_*/KHI_*), symmetric outputs by computing the lower tiles only (OUT_LOWER*).
@@ -14,7 +14,6 @@
 
 namespace {
 
-constexpr int STAGES = 3;
 constexpr int KPAD = 4;  // leading dimensions are == 4 (mod 16) doubles
 
 __device__ __forceinline__ void cp_async16(void* smem, const void* gmem, int src_bytes) {
@@ -123,7 +122,7 @@ __device__ __forceinline__ void load_tile_fast(double* sm_thread, const double* 
   }
 }
 
-template <int BM, int BN, int WM, int WN, bool A_KM, bool B_KM, int BK>
+template <int BM, int BN, int WM, int WN, bool A_KM, bool B_KM, int BK, int STAGES>
 struct Cfg {
   static constexpr int NWM = BM / WM, NWN = BN / WN;
   static constexpr int NT = NWM * NWN * 32;
@@ -132,9 +131,9 @@ struct Cfg {
   static constexpr int SMEM = (2 + STAGES * (A_ST + B_ST)) * (int)sizeof(double);
 };
 
-template <int BM, int BN, int WM, int WN, bool A_KM, bool B_KM, int MINB, int BK>
-__global__ void __launch_bounds__(Cfg<BM, BN, WM, WN, A_KM, B_KM, BK>::NT, MINB) gemm_kernel(GemmArgs g) {
-  using C_ = Cfg<BM, BN, WM, WN, A_KM, B_KM, BK>;
+template <int BM, int BN, int WM, int WN, bool A_KM, bool B_KM, int MINB, int BK, int STAGES>
+__global__ void __launch_bounds__(Cfg<BM, BN, WM, WN, A_KM, B_KM, BK, STAGES>::NT, MINB) gemm_kernel(GemmArgs g) {
+  using C_ = Cfg<BM, BN, WM, WN, A_KM, B_KM, BK, STAGES>;
   constexpr int NT = C_::NT;
   extern __shared__ __align__(16) double smem[];
   unsigned long long* bar = reinterpret_cast<unsigned long long*>(smem);  // 16 bytes reserved
@@ -312,10 +311,10 @@ __global__ void __launch_bounds__(Cfg<BM, BN, WM, WN, A_KM, B_KM, BK>::NT, MINB)
   }
 }
 
-template <int BM, int BN, int WM, int WN, bool A_KM, bool B_KM, int MINB, int BK>
+template <int BM, int BN, int WM, int WN, bool A_KM, bool B_KM, int MINB, int BK, int STAGES>
 cudaError_t launch_cfg(const GemmArgs& g, cudaStream_t st) {
-  using C_ = Cfg<BM, BN, WM, WN, A_KM, B_KM, BK>;
-  auto kern = gemm_kernel<BM, BN, WM, WN, A_KM, B_KM, MINB, BK>;
+  using C_ = Cfg<BM, BN, WM, WN, A_KM, B_KM, BK, STAGES>;
+  auto kern = gemm_kernel<BM, BN, WM, WN, A_KM, B_KM, MINB, BK, STAGES>;
   static bool attr_done = false;  // per instantiation
   if (!attr_done) {
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C_::SMEM);
@@ -334,12 +333,12 @@ cudaError_t launch_cfg(const GemmArgs& g, cudaStream_t st) {
   return cudaGetLastError();
 }
 
-template <int BM, int BN, int WM, int WN, int MINB, int BK>
+template <int BM, int BN, int WM, int WN, int MINB, int BK, int STAGES = 3>
 cudaError_t launch_mode(const GemmArgs& g, cudaStream_t st) {
   switch (g.mode) {
-    case GEMM_NN: return launch_cfg<BM, BN, WM, WN, false, true, MINB, BK>(g, st);
-    case GEMM_NT: return launch_cfg<BM, BN, WM, WN, false, false, MINB, BK>(g, st);
-    case GEMM_TN: return launch_cfg<BM, BN, WM, WN, true, true, MINB, BK>(g, st);
+    case GEMM_NN: return launch_cfg<BM, BN, WM, WN, false, true, MINB, BK, STAGES>(g, st);
+    case GEMM_NT: return launch_cfg<BM, BN, WM, WN, false, false, MINB, BK, STAGES>(g, st);
+    case GEMM_TN: return launch_cfg<BM, BN, WM, WN, true, true, MINB, BK, STAGES>(g, st);
   }
   return cudaErrorInvalidValue;
 }
