@@ -217,6 +217,36 @@ def test_gemm_kernel_modes():
     assert np.max(np.abs(gemm(1, t(Bm), t(Bm), z(), out=1).cpu().numpy() - np.tril(Bm @ Bm.T))) < 1e-11
 
 
+def test_gemm_tile_classes_and_ragged_edges():
+    """The three tile classes of launch_gemm (32x32 / 64x64 / 128x128), ragged tails in M, N and K,
+    and the triangular k-ranges / lower-only outputs at sizes that reach the 64x64 and 128x128 tiles."""
+    import torch
+    from paper_2605_06392_b200 import gemm
+    rng = np.random.default_rng(1)
+    t = lambda x: torch.tensor(x, device="cuda")
+    for (Mm, Nn, Kk) in [(1000, 900, 520),      # 16 x 15 small tiles -> 64x64 class
+                         (1990, 2000, 301),     # 16 x 16 big tiles -> 128x128 class, ragged in M and K
+                         (2304, 2304, 130)]:    # 324 big tiles = 2.19 waves -> 64x64 class by the wave rule
+        for mode in (0, 1, 2):
+            A = rng.standard_normal((Mm, Kk) if mode != 2 else (Kk, Mm))
+            B = rng.standard_normal((Kk, Nn) if mode != 1 else (Nn, Kk))
+            C0 = rng.standard_normal((Mm, Nn))
+            ref = 0.75 * (A if mode != 2 else A.T) @ (B if mode != 1 else B.T) - 2.0 * C0
+            Cd = t(C0)
+            gemm(mode, t(A), t(B), Cd, alpha=0.75, beta=-2.0)
+            assert np.max(np.abs(Cd.cpu().numpy() - ref)) <= 1e-12 * Kk, (Mm, Nn, Kk, mode)
+    for n in (1100, 1930):                      # 64x64 class; 128x128 class with a ragged last tile
+        L = np.tril(rng.standard_normal((n, n)))
+        Bm = rng.standard_normal((n, n))
+        z = lambda: torch.zeros(n, n, dtype=torch.float64, device="cuda")
+        tol = 1e-12 * n
+        assert np.max(np.abs(gemm(1, t(Bm), t(L), z(), khi=1).cpu().numpy() - Bm @ L.T)) < tol
+        assert np.max(np.abs(gemm(0, t(Bm), t(L), z(), klo=1).cpu().numpy() - Bm @ L)) < tol
+        assert np.max(np.abs(gemm(0, t(L), t(Bm), z(), khi=2).cpu().numpy() - L @ Bm)) < tol
+        assert np.max(np.abs(gemm(2, t(L), t(L), z(), klo=2, out=2).cpu().numpy() - L.T @ L)) < tol
+        assert np.max(np.abs(gemm(1, t(Bm), t(Bm), z(), out=1).cpu().numpy() - np.tril(Bm @ Bm.T))) < tol
+
+
 @pytest.mark.parametrize("name", ["w0", "b81_two_tiles", "mv_k3_tiny", "mv_k2_b162"])
 def test_value_fd_gradient_and_hessian(name):
     """value-only pass, the finite-difference baseline (Eq. 2) and the Hessian by
