@@ -184,6 +184,12 @@ int bta_fp64_peak(int kind, int iters, double* tflops, double* ms, void* stream)
 int bta_gemm(int mode, int M, int N, int K, double alpha, const double* A, int lda, const double* B, int ldb,
              double beta, double* C, int ldc, int klo, int khi, int out, void* stream);
 
+/* Diagnostic (not on the hot path): one record {start ns, end ns, smid | tile << 16 | mode << 28, k-range | M << 32}
+ * per GEMM CTA into buf[cap][4] (DEVICE memory, caller-owned, must outlive the tracing); buf = NULL switches it off.
+ * Both calls synchronise the device.  bta_debug_cta_trace_count returns the number of CTAs seen since it was armed. */
+int bta_debug_cta_trace(unsigned long long* buf, unsigned int cap);
+int bta_debug_cta_trace_count(unsigned int* n);
+
 #ifdef __cplusplus
 }
 #endif

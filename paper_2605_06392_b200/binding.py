@@ -77,6 +77,8 @@ def lib():
     L.bta_get_store_mode.argtypes = [vp]
     L.bta_fp64_peak.argtypes = [i32, i32, dp, dp, vp]
     L.bta_gemm.argtypes = [i32, i32, i32, i32, C.c_double, vp, i32, vp, i32, C.c_double, vp, i32, i32, i32, i32, vp]
+    L.bta_debug_cta_trace.argtypes = [vp, C.c_uint]
+    L.bta_debug_cta_trace_count.argtypes = [C.POINTER(C.c_uint)]
     _lib = L
     return L
 
@@ -304,3 +306,17 @@ def gemm(mode, A, B, Cm, alpha=1.0, beta=0.0, klo=0, khi=0, out=0):
     _check(lib().bta_gemm(mode, M, N, K, alpha, A.data_ptr(), A.stride(0), B.data_ptr(), B.stride(0), beta,
                           Cm.data_ptr(), Cm.stride(0), klo, khi, out, _stream()))
     return Cm
+
+
+def cta_trace_start(buf):
+    """Diagnostic: arm the per-CTA GEMM timeline; `buf` is a CUDA int64 tensor of shape [cap, 4] (None: off)."""
+    if buf is None:
+        _check(lib().bta_debug_cta_trace(None, 0))
+    else:
+        _check(lib().bta_debug_cta_trace(buf.data_ptr(), buf.shape[0]))
+
+
+def cta_trace_count():
+    n = C.c_uint(0)
+    _check(lib().bta_debug_cta_trace_count(C.byref(n)))
+    return n.value

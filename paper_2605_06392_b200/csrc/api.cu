@@ -604,6 +604,17 @@ int enqueue_gradient_twisted(bta_ctx* c, void* ws, cudaStream_t s0, bool timed, 
   cudaEvent_t* ev = c->ev;
   // streams: [matrix][up, down]
   cudaStream_t st[2][2] = {{s0, c->s_aux[0]}, {c->s_side, c->s_aux[1]}};
+  // forward sweeps: the same streams, or (BTA_FWD_RESERVE) streams of the green context that leaves some SMs to the
+  // latency-bound kernels of the other chains' recursions (model.cu: make_forward_partition)
+  cudaStream_t fs[2][2];
+  for (int m = 0; m < 2; ++m)
+    for (int q = 0; q < 2; ++q) fs[m][q] = c->s_fwd[2 * m + q] ? c->s_fwd[2 * m + q] : st[m][q];
+  auto hand_over = [&](cudaStream_t from, cudaStream_t to) -> cudaError_t {
+    if (from == to) return cudaSuccess;
+    cudaEvent_t e = c->ev_sw[(c->ev_sw_next++) % BTA_NSW];
+    cudaError_t ce = cudaEventRecord(e, from);
+    return ce != cudaSuccess ? ce : cudaStreamWaitEvent(to, e, 0);
+  };
 #define REC(i, s)                                      \
   do {                                                 \
     if (timed) BTA_CUDA_OK(cudaEventRecord(ev[i], s)); \
@@ -662,7 +673,7 @@ int enqueue_gradient_twisted(bta_ctx* c, void* ws, cudaStream_t s0, bool timed, 
     hi = std::min(hi, top);
     if (lo >= hi) return BTA_OK;
     BTA_CUDA_OK(launch_assemble_seq(c, m == 0 ? BTA_COND : BTA_PRIOR, 0, k.tg(lo), k.tdir, hi - lo, 0,
-                                    k.D + (long long)lo * k.d_stride, k.d_stride, st[m][q]));
+                                    k.D + (long long)lo * k.d_stride, k.d_stride, fs[m][q]));
     return BTA_OK;
   };
   for (int m = 0; m < 2; ++m) {
@@ -679,7 +690,10 @@ int enqueue_gradient_twisted(bta_ctx* c, void* ws, cudaStream_t s0, bool timed, 
 
   // ---- forward: four sub-chains, launches interleaved block by block
   for (int m = 0; m < 2; ++m)
-    for (int q = 0; q < 2; ++q) BTA_CUDA_OK(chain_forward_begin(ch[m][q], st[m][q]));
+    for (int q = 0; q < 2; ++q) {
+      BTA_CUDA_OK(hand_over(st[m][q], fs[m][q]));
+      BTA_CUDA_OK(chain_forward_begin(ch[m][q], fs[m][q]));
+    }
   const int maxlen = std::max(ch[0][0].nt, ch[0][1].nt);
   for (int m = 0; m < 2; ++m)
     for (int q = 0; q < 2; ++q) {
@@ -691,12 +705,17 @@ int enqueue_gradient_twisted(bta_ctx* c, void* ws, cudaStream_t s0, bool timed, 
       for (int q = 0; q < 2; ++q)
         if (s < ch[m][q].nt) {
           if (s % AHEAD == 0) {  // blocks s+2 .. s+AHEAD+1 (block s+1 receives this step's Schur update)
-            BTA_CUDA_OK(chain_to_big(ch[m][q], st[m][q]));
+            BTA_CUDA_OK(chain_to_big(ch[m][q], fs[m][q]));
             int rc = assemble_range(m, q, s + 2, s + 2 + AHEAD);
             if (rc != BTA_OK) return rc;
           }
-          BTA_CUDA_OK(chain_forward_step(ch[m][q], s, st[m][q]));
+          BTA_CUDA_OK(chain_forward_step(ch[m][q], s, fs[m][q]));
         }
+  for (int m = 0; m < 2; ++m)
+    for (int q = 0; q < 2; ++q) {
+      BTA_CUDA_OK(chain_to_big(ch[m][q], fs[m][q]));
+      BTA_CUDA_OK(hand_over(fs[m][q], st[m][q]));
+    }
   for (int m = 0; m < 2; ++m) {
     BTA_CUDA_OK(join_lanes(m, 0));
     BTA_CUDA_OK(join_lanes(m, 1));

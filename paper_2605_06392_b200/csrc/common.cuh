@@ -146,6 +146,12 @@ struct bta_ctx {
   cudaEvent_t ev[32];
   cudaStream_t s_hi[4];              // high-priority companions of the four chains (small kernels)
   cudaStream_t s_x[4];               // side streams of the four chains (off-chain work of the forward steps)
+  // Optional SM partition for the forward sweeps (BTA_FWD_RESERVE=R): the full-size products of the forward steps run
+  // on streams of a green context that owns all but ~R SMs, so the latency-bound kernels of the POTRF+TRTRI recursion
+  // (other chains' priority lanes) always find free SMs.  s_fwd[i] = nullptr: no partition.
+  cudaStream_t s_fwd[4];
+  void* green_ctx;                   // CUgreenCtx (opaque here)
+  int fwd_sms;                       // SMs of the forward partition (0 = none)
   cudaEvent_t ev_sw[256];            // lane-switch events, used round-robin
   unsigned ev_sw_next;
   long long launches;

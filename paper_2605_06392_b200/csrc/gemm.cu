@@ -16,6 +16,17 @@ namespace {
 
 constexpr int KPAD = 4;  // leading dimensions are == 4 (mod 16) doubles
 
+// Diagnostic CTA timeline (bta_debug_cta_trace; null in production): one record per CTA that did work,
+// {start ns, end ns, smid | BM << 16 | mode << 28, k-range | M << 32} from %globaltimer.
+__device__ unsigned long long* g_cta_trace = nullptr;
+__device__ unsigned int g_cta_cap = 0;
+__device__ unsigned int g_cta_n = 0;
+__device__ __forceinline__ unsigned long long global_ns() {
+  unsigned long long t;
+  asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+  return t;
+}
+
 __device__ __forceinline__ void cp_async16(void* smem, const void* gmem, int src_bytes) {
   unsigned s = (unsigned)__cvta_generic_to_shared(smem);
   asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;\n" ::"r"(s), "l"(gmem), "r"(src_bytes));
@@ -131,7 +142,7 @@ struct Cfg {
   static constexpr int SMEM = (2 + STAGES * (A_ST + B_ST)) * (int)sizeof(double);
 };
 
-template <int BM, int BN, int WM, int WN, bool A_KM, bool B_KM, int MINB, int BK, int STAGES>
+template <int BM, int BN, int WM, int WN, bool A_KM, bool B_KM, int MINB, int BK, int STAGES, bool TRACE = false>
 __global__ void __launch_bounds__(Cfg<BM, BN, WM, WN, A_KM, B_KM, BK, STAGES>::NT, MINB) gemm_kernel(GemmArgs g) {
   using C_ = Cfg<BM, BN, WM, WN, A_KM, B_KM, BK, STAGES>;
   constexpr int NT = C_::NT;
@@ -188,6 +199,9 @@ __global__ void __launch_bounds__(Cfg<BM, BN, WM, WN, A_KM, B_KM, BK, STAGES>::N
   if (g.khi == KHI_NEND) kend = min(K, n0 + BN);
   if (g.khi == KHI_MEND) kend = min(K, m0 + BM);
   kbeg = (kbeg / BK) * BK;
+  // TRACE instantiations only (bta_debug_cta_trace): measured, a run-time test here costs the production kernel 1.5 %
+  unsigned long long t_begin = 0ull;
+  if constexpr (TRACE) t_begin = threadIdx.x == 0 ? global_ns() : 0ull;
 
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int wm0 = (warp / C_::NWN) * WM, wn0 = (warp % C_::NWN) * WN;
@@ -309,12 +323,25 @@ __global__ void __launch_bounds__(Cfg<BM, BN, WM, WN, A_KM, B_KM, BK, STAGES>::N
       }
     }
   }
+  if constexpr (TRACE) {
+    unsigned long long* const cta_trace = g_cta_trace;
+    const unsigned idx = (cta_trace && tid == 0) ? atomicAdd(&g_cta_n, 1u) : 0xFFFFFFFFu;
+    if (cta_trace && tid == 0 && idx < g_cta_cap) {
+      unsigned smid;
+      asm volatile("mov.u32 %0, %%smid;" : "=r"(smid));
+      unsigned long long* r = cta_trace + 4ull * idx;
+      r[0] = t_begin;
+      r[1] = global_ns();
+      r[2] = (unsigned long long)smid | ((unsigned long long)BM << 16) | ((unsigned long long)g.mode << 28);
+      r[3] = (unsigned long long)(unsigned)(kend - kbeg) | ((unsigned long long)(unsigned)M << 32);
+    }
+  }
 }
 
-template <int BM, int BN, int WM, int WN, bool A_KM, bool B_KM, int MINB, int BK, int STAGES>
+template <int BM, int BN, int WM, int WN, bool A_KM, bool B_KM, int MINB, int BK, int STAGES, bool TRACE>
 cudaError_t launch_cfg(const GemmArgs& g, cudaStream_t st) {
   using C_ = Cfg<BM, BN, WM, WN, A_KM, B_KM, BK, STAGES>;
-  auto kern = gemm_kernel<BM, BN, WM, WN, A_KM, B_KM, MINB, BK, STAGES>;
+  auto kern = gemm_kernel<BM, BN, WM, WN, A_KM, B_KM, MINB, BK, STAGES, TRACE>;
   static bool attr_done = false;  // per instantiation
   if (!attr_done) {
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C_::SMEM);
@@ -333,12 +360,12 @@ cudaError_t launch_cfg(const GemmArgs& g, cudaStream_t st) {
   return cudaGetLastError();
 }
 
-template <int BM, int BN, int WM, int WN, int MINB, int BK, int STAGES = 3>
+template <int BM, int BN, int WM, int WN, int MINB, int BK, int STAGES = 3, bool TRACE = false>
 cudaError_t launch_mode(const GemmArgs& g, cudaStream_t st) {
   switch (g.mode) {
-    case GEMM_NN: return launch_cfg<BM, BN, WM, WN, false, true, MINB, BK, STAGES>(g, st);
-    case GEMM_NT: return launch_cfg<BM, BN, WM, WN, false, false, MINB, BK, STAGES>(g, st);
-    case GEMM_TN: return launch_cfg<BM, BN, WM, WN, true, true, MINB, BK, STAGES>(g, st);
+    case GEMM_NN: return launch_cfg<BM, BN, WM, WN, false, true, MINB, BK, STAGES, TRACE>(g, st);
+    case GEMM_NT: return launch_cfg<BM, BN, WM, WN, false, false, MINB, BK, STAGES, TRACE>(g, st);
+    case GEMM_TN: return launch_cfg<BM, BN, WM, WN, true, true, MINB, BK, STAGES, TRACE>(g, st);
   }
   return cudaErrorInvalidValue;
 }
@@ -400,8 +427,18 @@ bool gemm_uses_tiny_tiles(const GemmArgs& g) {
 }
 }  // namespace
 
+static bool g_trace_host = false;  // set while bta_debug_cta_trace is armed: launch the TRACE twins of the default tiles
+
 cudaError_t launch_gemm(const GemmArgs& g0, cudaStream_t st) {
   if (g0.M <= 0 || g0.N <= 0) return cudaSuccess;
+  if (g_trace_host) {
+    GemmArgs g = g0;
+    g.dbg = 0;
+    g.group = 16;
+    if (!gemm_uses_small_tiles(g)) return launch_mode<128, 128, 32, 32, 1, 16, 3, true>(g, st);
+    if (gemm_uses_tiny_tiles(g)) return launch_mode<32, 32, 16, 16, 4, 16, 3, true>(g, st);
+    return launch_mode<64, 64, 32, 32, 3, 16, 3, true>(g, st);
+  }
   static const int dbg = [] {
     const char* e = getenv("BTA_GEMM_DBG");
     return e ? atoi(e) : 0;
@@ -436,4 +473,22 @@ cudaError_t launch_gemm(const GemmArgs& g0, cudaStream_t st) {
     case 0: return launch_mode<64, 64, 32, 32, 2, 16>(g, st);
     default: return launch_mode<64, 64, 32, 32, 3, 16>(g, st);  // three CTAs per SM
   }
+}
+
+// Diagnostic: record one {start, end, sm, shape} entry per GEMM CTA into buf[cap][4] (device memory, caller-owned);
+// buf = nullptr switches it off.  Not part of the hot path's interface.
+extern "C" int bta_debug_cta_trace(unsigned long long* buf, unsigned int cap) {
+  const unsigned int zero = 0;
+  BTA_CUDA_OK(cudaDeviceSynchronize());
+  BTA_CUDA_OK(cudaMemcpyToSymbol(g_cta_trace, &buf, sizeof buf));
+  BTA_CUDA_OK(cudaMemcpyToSymbol(g_cta_cap, &cap, sizeof cap));
+  BTA_CUDA_OK(cudaMemcpyToSymbol(g_cta_n, &zero, sizeof zero));
+  g_trace_host = buf != nullptr;
+  return BTA_OK;
+}
+extern "C" int bta_debug_cta_trace_count(unsigned int* n) {
+  if (!n) return BTA_ERR_ARG;
+  BTA_CUDA_OK(cudaDeviceSynchronize());
+  BTA_CUDA_OK(cudaMemcpyFromSymbol(n, g_cta_n, sizeof *n));
+  return BTA_OK;
 }

@@ -2,12 +2,83 @@
 #include <cstdlib>
 #include <cstring>
 
+#include <cuda.h>
+
 #include "common.cuh"
 
 namespace {
 template <typename T>
 cudaError_t dev_alloc(T** p, size_t n) {
   return cudaMalloc((void**)p, (n ? n : 1) * sizeof(T));
+}
+}  // namespace
+
+// Green-context SM partition for the forward sweeps (common.cuh: s_fwd).  The driver entry points are looked up at run
+// time (cudaGetDriverEntryPoint), so the library keeps no link-time dependency on libcuda.  An optimisation only: on any
+// failure the partition is left off (fwd_sms = 0) and the reason goes to bta_last_error.
+namespace {
+template <class F>
+bool drv(const char* name, F& fn) {
+  void* p = nullptr;
+  cudaDriverEntryPointQueryResult qr;
+  if (cudaGetDriverEntryPoint(name, &p, cudaEnableDefault, &qr) != cudaSuccess || qr != cudaDriverEntryPointSuccess || !p)
+    return false;
+  fn = reinterpret_cast<F>(p);
+  return true;
+}
+void make_forward_partition(bta_ctx* c, int device, int reserve, int prio) {
+  CUresult (*getRes)(CUdevice, CUdevResource*, CUdevResourceType) = nullptr;
+  CUresult (*split)(CUdevResource*, unsigned int*, const CUdevResource*, CUdevResource*, unsigned int, unsigned int) =
+      nullptr;
+  CUresult (*genDesc)(CUdevResourceDesc*, CUdevResource*, unsigned int) = nullptr;
+  CUresult (*gcreate)(CUgreenCtx*, CUdevResourceDesc, CUdevice, unsigned int) = nullptr;
+  CUresult (*gstream)(CUstream*, CUgreenCtx, unsigned int, int) = nullptr;
+  CUresult (*devGet)(CUdevice*, int) = nullptr;
+  if (!drv("cuDeviceGetDevResource", getRes) || !drv("cuDevSmResourceSplitByCount", split) ||
+      !drv("cuDevResourceGenerateDesc", genDesc) || !drv("cuGreenCtxCreate", gcreate) ||
+      !drv("cuGreenCtxStreamCreate", gstream) || !drv("cuDeviceGet", devGet)) {
+    bta_set_error("BTA_FWD_RESERVE: green-context driver entry points not available");
+    return;
+  }
+  CUdevice dev;
+  CUdevResource all, part, rest;
+  if (devGet(&dev, device) != CUDA_SUCCESS || getRes(dev, &all, CU_DEV_RESOURCE_TYPE_SM) != CUDA_SUCCESS) {
+    bta_set_error("BTA_FWD_RESERVE: cuDeviceGetDevResource failed");
+    return;
+  }
+  const int total = (int)all.sm.smCount;
+  if (reserve >= total) return;
+  unsigned int ngroups = 1;
+  if (split(&part, &ngroups, &all, &rest, 0, (unsigned)(total - reserve)) != CUDA_SUCCESS || ngroups != 1) {
+    bta_set_error("BTA_FWD_RESERVE: cuDevSmResourceSplitByCount failed");
+    return;
+  }
+  CUdevResourceDesc desc;
+  CUgreenCtx g;
+  if (genDesc(&desc, &part, 1) != CUDA_SUCCESS || gcreate(&g, desc, dev, CU_GREEN_CTX_DEFAULT_STREAM) != CUDA_SUCCESS) {
+    bta_set_error("BTA_FWD_RESERVE: cuGreenCtxCreate failed");
+    return;
+  }
+  c->green_ctx = g;
+  for (auto& q : c->s_fwd) {
+    CUstream st = nullptr;
+    if (gstream(&st, g, CU_STREAM_NON_BLOCKING, prio) != CUDA_SUCCESS) {
+      bta_set_error("BTA_FWD_RESERVE: cuGreenCtxStreamCreate failed");
+      for (auto& r : c->s_fwd) {
+        if (r) cudaStreamDestroy(r);
+        r = nullptr;
+      }
+      return;
+    }
+    q = st;
+  }
+  c->fwd_sms = (int)part.sm.smCount;
+}
+void destroy_forward_partition(bta_ctx* c) {
+  if (!c->green_ctx) return;
+  CUresult (*gdestroy)(CUgreenCtx) = nullptr;
+  if (drv("cuGreenCtxDestroy", gdestroy)) gdestroy((CUgreenCtx)c->green_ctx);
+  c->green_ctx = nullptr;
 }
 }  // namespace
 
@@ -111,6 +182,13 @@ extern "C" int bta_create(bta_ctx** out, const bta_model_desc* desc, const bta_o
     BTA_CUDA_OK(cudaDeviceGetStreamPriorityRange(&plo, &phi));
     for (auto& q : c->s_hi) BTA_CUDA_OK(cudaStreamCreateWithPriority(&q, cudaStreamNonBlocking, phi));
     for (auto& q : c->s_x) BTA_CUDA_OK(cudaStreamCreateWithPriority(&q, cudaStreamNonBlocking, plo));
+    for (auto& q : c->s_fwd) q = nullptr;
+    c->green_ctx = nullptr;
+    c->fwd_sms = 0;
+    if (const char* e = getenv("BTA_FWD_RESERVE")) {
+      const int reserve = atoi(e);
+      if (reserve > 0) make_forward_partition(c, device, reserve, plo);
+    }
     for (auto& e : c->ev_sw) BTA_CUDA_OK(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
     c->ev_sw_next = 0;
   }
@@ -154,6 +232,9 @@ extern "C" int bta_destroy(bta_ctx* c) {
   for (auto& e : c->ev) cudaEventDestroy(e);
   for (auto& q : c->s_hi) cudaStreamDestroy(q);
   for (auto& q : c->s_x) cudaStreamDestroy(q);
+  for (auto& q : c->s_fwd)
+    if (q) cudaStreamDestroy(q);
+  destroy_forward_partition(c);
   for (auto& e : c->ev_sw) cudaEventDestroy(e);
   delete c;
   return BTA_OK;
