@@ -247,6 +247,34 @@ def test_gemm_tile_classes_and_ragged_edges():
         assert np.max(np.abs(gemm(1, t(Bm), t(Bm), z(), out=1).cpu().numpy() - np.tril(Bm @ Bm.T))) < tol
 
 
+def test_cta_trace_twins_are_bit_identical_and_count_ctas():
+    """The TRACE instantiations of the GEMM kernel (bta_debug_cta_trace; diagnostics only) are separate code: they must
+    return the same bits as the production kernels, record one entry per working CTA, and switch off again."""
+    import torch
+    from paper_2605_06392_b200 import gemm
+    from paper_2605_06392_b200.binding import cta_trace_count, cta_trace_start
+    rng = np.random.default_rng(2)
+    t = lambda x: torch.tensor(x, device="cuda")
+    cases = [(200, 200, 96, 32), (1000, 900, 130, 64), (2000, 1990, 70, 128)]   # 32x32, 64x64, 128x128 tile classes
+    for (Mm, Nn, Kk, tile) in cases:
+        A, B = rng.standard_normal((Mm, Kk)), rng.standard_normal((Kk, Nn))
+        plain = gemm(0, t(A), t(B), torch.zeros(Mm, Nn, dtype=torch.float64, device="cuda")).cpu().numpy()
+        buf = torch.zeros(4096, 4, dtype=torch.int64, device="cuda")
+        cta_trace_start(buf)
+        try:
+            traced = gemm(0, t(A), t(B), torch.zeros(Mm, Nn, dtype=torch.float64, device="cuda")).cpu().numpy()
+            n = cta_trace_count()
+        finally:
+            cta_trace_start(None)
+        assert np.array_equal(plain, traced)
+        assert n == -(-Mm // tile) * -(-Nn // tile), (n, Mm, Nn, tile)
+        r = buf[:n].cpu().numpy()
+        assert np.all(r[:, 1] >= r[:, 0]) and np.all((r[:, 2] >> 16) & 0xFFF == tile) and np.all((r[:, 2] & 0xFFFF) < 148)
+        # switched off again (which also resets the counter, include/bta.h): a further launch records nothing
+        gemm(0, t(A), t(B), torch.zeros(Mm, Nn, dtype=torch.float64, device="cuda"))
+        assert cta_trace_count() == 0
+
+
 @pytest.mark.parametrize("name", ["w0", "b81_two_tiles", "mv_k3_tiny", "mv_k2_b162"])
 def test_value_fd_gradient_and_hessian(name):
     """value-only pass, the finite-difference baseline (Eq. 2) and the Hessian by
