@@ -27,6 +27,13 @@
 #include <stddef.h>
 #include <stdint.h>
 
+/* The library is built with -fvisibility=hidden: only the entry points declared here (and in bta_diag.h) are exported. */
+#if defined(__GNUC__)
+#define BTA_API __attribute__((visibility("default")))
+#else
+#define BTA_API
+#endif
+
 #ifdef __cplusplus
 extern "C" {
 #endif
@@ -79,8 +86,8 @@ typedef struct {
 /* Model setup: copies the observations to the device and reduces
  * them to theta-independent aggregates (counts, covariate sums, Z^T Z, A^T y) with device kernels in a
  * deterministic order.  `device` is the CUDA ordinal.  *out is NULL on failure. */
-int bta_create(bta_ctx** out, const bta_model_desc* desc, const bta_obs* obs, int device);
-int bta_destroy(bta_ctx* ctx);
+BTA_API int bta_create(bta_ctx** out, const bta_model_desc* desc, const bta_obs* obs, int device);
+BTA_API int bta_destroy(bta_ctx* ctx);
 
 /* Storage policy of inla_value_and_grad.
  *   BTA_STORE_FACTOR (default): the factor blocks X_t = L_Dt^-1 and L_Bt are kept for the backward sweep
@@ -90,20 +97,20 @@ int bta_destroy(bta_ctx* ctx);
  *     sweep rebuilds X_t (one more Cholesky + inverse) and L_Bt (B_t is re-assembled, one more product) per block.
  * Changes bta_workspace_bytes.  Returns BTA_ERR_ARG for an unknown mode. */
 enum { BTA_STORE_FACTOR = 0, BTA_STORE_CARRY = 1 };
-int bta_set_store_mode(bta_ctx* ctx, int mode);
-int bta_get_store_mode(const bta_ctx* ctx);
+BTA_API int bta_set_store_mode(bta_ctx* ctx, int mode);
+BTA_API int bta_get_store_mode(const bta_ctx* ctx);
 
 /* Bytes of caller-provided device workspace needed by inla_value_and_grad (the largest user: both matrices'
  * blocks, per-chain temporaries).  bta_factor_logdet / bta_solve / bta_selinv need at most
  * bta_workspace_bytes_op(ctx) (three b x b temporaries + small vectors). */
-size_t bta_workspace_bytes(const bta_ctx* ctx);
-size_t bta_workspace_bytes_op(const bta_ctx* ctx);
+BTA_API size_t bta_workspace_bytes(const bta_ctx* ctx);
+BTA_API size_t bta_workspace_bytes_op(const bta_ctx* ctx);
 
 /* Q_p(theta) or Q_c(theta) = Q_p + sum_v tau_v A_v^T A_v and r = sum_v tau_v A_v^T y_v as dense blocks
  * (Eq. 10 for k > 1 with the weights of R12).  theta: HOST, d doubles.  D is written
  * with its strict upper triangle ZERO (the lower triangle is authoritative everywhere in this library);
  * B, C, T in full.  out.rhs (if not NULL) receives r for BTA_COND, zeros for BTA_PRIOR. */
-int bta_assemble(bta_ctx* ctx, const double* theta, int which, bta_blocks out, void* stream);
+BTA_API int bta_assemble(bta_ctx* ctx, const double* theta, int which, bta_blocks out, void* stream);
 
 /* Algorithm 1 (R8): block Cholesky Q = L L^T in place, and log det Q (HOST scalar).
  * The factor is kept in INVERSE-DIAGONAL FORM: on return
@@ -112,44 +119,44 @@ int bta_assemble(bta_ctx* ctx, const double* theta, int which, bta_blocks out, v
  * and diagL (device, N doubles, may be NULL) receives diag(L_D1), ..., diag(L_Dnt), diag(L_T).
  * `which` = BTA_PRIOR skips the arrow (C ignored, T factored on its own).  Only the lower triangles of the
  * D[t] and T are read.  ws: device workspace (bta_workspace_bytes_op). */
-int bta_factor_logdet(bta_ctx* ctx, bta_blocks inout, int which, double* logdet, double* diagL, void* ws,
+BTA_API int bta_factor_logdet(bta_ctx* ctx, bta_blocks inout, int which, double* logdet, double* diagL, void* ws,
                       void* stream);
 
 /* Both triangular sweeps L z = rhs, L^T x = z (Algorithm 1 line 5/11 and Eqs. 3-5) for
  * nrhs right-hand sides, in place: rhs_inout is DEVICE [nrhs][N].  L as left by bta_factor_logdet. */
-int bta_solve(bta_ctx* ctx, bta_blocks L, int which, double* rhs_inout, int nrhs, void* ws, void* stream);
+BTA_API int bta_solve(bta_ctx* ctx, bta_blocks L, int which, double* rhs_inout, int nrhs, void* ws, void* stream);
 
 /* BTA selected inversion (recurrences R10), in place over the factor left by
  * bta_factor_logdet: on return D[t] = Z_Dt = [Q^-1]_{tt} (both triangles), B[t] = Z_Bt = [Q^-1]_{t+1,t},
  * C[t] = Z_Ct = [Q^-1]_{T,t}, T = Z_T. */
-int bta_selinv(bta_ctx* ctx, bta_blocks inout, int which, void* ws, void* stream);
+BTA_API int bta_selinv(bta_ctx* ctx, bta_blocks inout, int which, void* ws, void* stream);
 
 /* The hot path (PAPER.md:44 Eq. 1, :121 Eq. 6): f(theta) and grad f(theta).  theta HOST [d]; f HOST scalar;
  * grad HOST [d]; stage_ms HOST [BTA_NSTAGES] or NULL (CUDA-event times of the stages, see BTA_STAGE_*);
  * ws DEVICE, bta_workspace_bytes(ctx) bytes.  Runs assemble -> fused forward sweep -> fused backward sweep
  * (upper solve + selected inversion + trace contractions) on Q_c and on Q_p, then the scalar assembly. */
-int inla_value_and_grad(bta_ctx* ctx, const double* theta, double* f, double* grad, double* stage_ms, void* ws,
+BTA_API int inla_value_and_grad(bta_ctx* ctx, const double* theta, double* f, double* grad, double* stage_ms, void* ws,
                         void* stream);
 
 /* the objective alone (Eq. 1): assemble -> factor Q_c and Q_p -> solve ->
  * scalars; no selected inversion, no contractions.  One evaluation of the finite-difference baseline. */
-int inla_value(bta_ctx* ctx, const double* theta, double* f, void* ws, void* stream);
+BTA_API int inla_value(bta_ctx* ctx, const double* theta, double* f, void* ws, void* stream);
 
 /* Central finite-difference gradient (Eq. 2; the DALIA baseline): 2d+1 calls of inla_value with
  * step h (the paper uses 1e-3).  f (may be NULL) receives f(theta), grad HOST [d].  Truncation error O(h^2). */
-int inla_fd_grad(bta_ctx* ctx, const double* theta, double h, double* f, double* grad, void* ws, void* stream);
+BTA_API int inla_fd_grad(bta_ctx* ctx, const double* theta, double h, double* f, double* grad, void* ws, void* stream);
 
 /* posterior Hessian by central differences of the exact gradient (Eq. 13):
  * H[:, j] = (grad f(theta + h e_j) - grad f(theta - h e_j)) / (2h), 2d+1 calls of inla_value_and_grad (the centre
  * call returns f and grad, either may be NULL).  H HOST [d][d], as differenced (not symmetrised). */
-int inla_hessian(bta_ctx* ctx, const double* theta, double h, double* f, double* grad, double* H, void* ws,
+BTA_API int inla_hessian(bta_ctx* ctx, const double* theta, double h, double* f, double* grad, double* H, void* ws,
                  void* stream);
 
 /* the INLA mode search: maximise f(theta) (reading R1: Eq. 1 is a
  * log-posterior) by L-BFGS on -f with exact gradients from inla_value_and_grad and an Armijo backtracking line search;
  * host driver, no new kernels.  Stops when ||grad||_inf <= gtol or after max_iter iterations.  Outputs (HOST, any may
  * be NULL): theta_opt[d], f_opt, grad_opt[d], iters, evals (number of inla_value_and_grad calls). */
-int inla_optimize(bta_ctx* ctx, const double* theta0, int max_iter, double gtol, double* theta_opt, double* f_opt,
+BTA_API int inla_optimize(bta_ctx* ctx, const double* theta0, int max_iter, double gtol, double* theta_opt, double* f_opt,
                   double* grad_opt, int* iters, int* evals, void* ws, void* stream);
 
 enum {
@@ -167,28 +174,14 @@ enum {
  * ld[2] = {log det Q_p, log det Q_c}; x DEVICE->HOST copy of x* [N]; parts[3*d] = Phase A, B, C per
  * hyperparameter (Eq. 6 terms before the -1/2, -1/2, +1/2 factors); rss[k] = ||y_v - A_v x*||^2;
  * quad = x*^T Q_p x*; ZT[a*a] = Z_T = [Q_c^-1]_{TT}. */
-int bta_last_intermediates(bta_ctx* ctx, double* ld, double* x, double* parts, double* rss, double* quad,
+BTA_API int bta_last_intermediates(bta_ctx* ctx, double* ld, double* x, double* parts, double* rss, double* quad,
                            double* ZT);
 
-int32_t bta_num_hyper(const bta_ctx* ctx);  /* d */
-int64_t bta_latent_size(const bta_ctx* ctx); /* N */
-int64_t bta_last_pivot(const bta_ctx* ctx);  /* 1-based global row of the first non-positive pivot, 0 if none */
-int64_t bta_kernel_launches(const bta_ctx* ctx); /* kernels launched by this ctx so far */
-const char* bta_last_error(void);
-
-/* Measurement helpers (bench.py): register-resident issue loops on all SMs, returning achieved FP64
- * TFLOP/s of `mma.sync.m8n8k4.f64` (kind 0) or DFMA (kind 1) -- the FP64 roofline denominators. */
-int bta_fp64_peak(int kind, int iters, double* tflops, double* ms, void* stream);
-/* Plain C = alpha op(A) op(B) + beta C through the library's DMMA GEMM (DEVICE pointers, row-major);
- * mode: 0 NN, 1 NT, 2 TN; klo/khi/out as in csrc/common.cuh (0 = full). */
-int bta_gemm(int mode, int M, int N, int K, double alpha, const double* A, int lda, const double* B, int ldb,
-             double beta, double* C, int ldc, int klo, int khi, int out, void* stream);
-
-/* Diagnostic (not on the hot path): one record {start ns, end ns, smid | tile << 16 | mode << 28, k-range | M << 32}
- * per GEMM CTA into buf[cap][4] (DEVICE memory, caller-owned, must outlive the tracing); buf = NULL switches it off.
- * Both calls synchronise the device.  bta_debug_cta_trace_count returns the number of CTAs seen since it was armed. */
-int bta_debug_cta_trace(unsigned long long* buf, unsigned int cap);
-int bta_debug_cta_trace_count(unsigned int* n);
+BTA_API int32_t bta_num_hyper(const bta_ctx* ctx);  /* d */
+BTA_API int64_t bta_latent_size(const bta_ctx* ctx); /* N */
+BTA_API int64_t bta_last_pivot(const bta_ctx* ctx);  /* 1-based global row of the first non-positive pivot, 0 if none */
+BTA_API int64_t bta_kernel_launches(const bta_ctx* ctx); /* kernels launched by this ctx so far */
+BTA_API const char* bta_last_error(void);
 
 #ifdef __cplusplus
 }

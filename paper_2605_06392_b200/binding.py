@@ -1,4 +1,4 @@
-"""ctypes binding with the same names as include/bta.h.  Marshalling only."""
+"""ctypes binding with the same names as include/bta.h (and include/bta_diag.h).  Marshalling only."""
 from __future__ import annotations
 
 import ctypes as C
@@ -79,6 +79,8 @@ def lib():
     L.bta_gemm.argtypes = [i32, i32, i32, i32, C.c_double, vp, i32, vp, i32, C.c_double, vp, i32, i32, i32, i32, vp]
     L.bta_debug_cta_trace.argtypes = [vp, C.c_uint]
     L.bta_debug_cta_trace_count.argtypes = [C.POINTER(C.c_uint)]
+    L.bta_set_option.argtypes = [vp, i32, i32]
+    L.bta_get_option.argtypes = [vp, i32]
     _lib = L
     return L
 
@@ -117,6 +119,7 @@ class Blocks:
 
 BTA_PRIOR, BTA_COND = 0, 1
 BTA_STORE_FACTOR, BTA_STORE_CARRY = 0, 1
+OPT_TWIST, OPT_LANES, OPT_SPLIT, OPT_GRAPH, OPT_SERIAL, OPT_PIPELINE = range(6)
 STAGES = ("assemble", "fwd_Qc", "bwd_Qc", "fwd_Qp", "bwd_Qp", "scalars", "total")
 
 
@@ -277,6 +280,13 @@ class BtaModel:
 
     def bta_get_store_mode(self):
         return lib().bta_get_store_mode(self._h)
+
+    def bta_set_option(self, option, value):
+        """include/bta_diag.h: OPT_TWIST / OPT_LANES / OPT_SPLIT / OPT_GRAPH / OPT_SERIAL / OPT_PIPELINE."""
+        _check(lib().bta_set_option(self._h, int(option), int(value)))
+
+    def bta_get_option(self, option):
+        return lib().bta_get_option(self._h, int(option))
 
     def kernel_launches(self):
         return lib().bta_kernel_launches(self._h)

@@ -126,7 +126,7 @@ extern "C" int bta_assemble(bta_ctx* c, const double* theta, int which, bta_bloc
   if (!out.D || (c->md.nt > 1 && !out.B) || !out.T) return bad("bta_assemble: D, B and T are required");
   cudaStream_t st = (cudaStream_t)stream;
   const ModelDims& md = c->md;
-  BTA_CUDA_OK(cudaSetDevice(c->device));
+  DeviceGuard guard(c->device);
   memcpy(c->host_pinned, theta, md.d * sizeof(double));
   BTA_CUDA_OK(cudaMemcpyAsync(c->theta_dev, c->host_pinned, md.d * sizeof(double), cudaMemcpyHostToDevice, st));
   BTA_CUDA_OK(launch_theta_prep(c, st));
@@ -145,7 +145,7 @@ extern "C" int bta_factor_logdet(bta_ctx* c, bta_blocks io, int which, double* l
     return bad("bta_factor_logdet: D, B, T (and C for BTA_COND) are required");
   cudaStream_t st = (cudaStream_t)stream;
   const ModelDims& md = c->md;
-  BTA_CUDA_OK(cudaSetDevice(c->device));
+  DeviceGuard guard(c->device);
   Bump bp(ws);
   OpWs w = carve_op(bp, md);
   SmallLayout L = small_layout(md);
@@ -195,7 +195,7 @@ extern "C" int bta_solve(bta_ctx* c, bta_blocks Lf, int which, double* rhs, int 
   if (!Lf.D || (c->md.nt > 1 && !Lf.B) || !Lf.T || (which == BTA_COND && !Lf.C)) return bad("bta_solve: missing factor");
   cudaStream_t st = (cudaStream_t)stream;
   const ModelDims& md = c->md;
-  BTA_CUDA_OK(cudaSetDevice(c->device));
+  DeviceGuard guard(c->device);
   Bump bp(ws);
   OpWs w = carve_op(bp, md);
   for (int r0 = 0; r0 < nrhs; r0 += SOLVE_CHUNK) {
@@ -252,7 +252,7 @@ extern "C" int bta_selinv(bta_ctx* c, bta_blocks io, int which, void* ws, void* 
   if (!io.D || (c->md.nt > 1 && !io.B) || !io.T || (which == BTA_COND && !io.C)) return bad("bta_selinv: missing factor");
   cudaStream_t st = (cudaStream_t)stream;
   const ModelDims& md = c->md;
-  BTA_CUDA_OK(cudaSetDevice(c->device));
+  DeviceGuard guard(c->device);
   Bump bp(ws);
   OpWs w = carve_op(bp, md);
   SmallLayout L = small_layout(md);
@@ -439,8 +439,9 @@ int enqueue_gradient(bta_ctx* c, void* ws, cudaStream_t s0, cudaStream_t s1, boo
   const int nout = 1 + md.d + 2 + 3 * md.d + md.k + 1;
   BTA_CUDA_OK(cudaMemcpyAsync(c->host_pinned + 64, c->small + L.out, nout * sizeof(double), cudaMemcpyDeviceToHost,
                               s0));
+  BTA_CUDA_OK(cudaMemcpyAsync(c->x_keep, wc.x, md.N * sizeof(double), cudaMemcpyDeviceToDevice, s0));
   REC(8, s0);
-  c->last_x_dev = wc.x;
+  c->have_x = true;
 #undef REC
   return BTA_OK;
 }
@@ -510,13 +511,7 @@ size_t twist_ws_bytes(const ModelDims& md, int store_mode) {
   return bp.off + 256;
 }
 
-bool use_twist(const ModelDims& md) {
-  static const int env = [] {
-    const char* e = getenv("BTA_TWIST");
-    return e ? atoi(e) : 1;
-  }();
-  return env != 0 && md.nt >= 3;
-}
+bool use_twist(const bta_ctx* c) { return c->opt.twist != 0 && c->md.nt >= 3; }
 
 // The three chains (up, down, separator) of one matrix.
 void make_twist_chains(bta_ctx* c, const MatWs& w, bool cond, bool value_only, Chain ch[3]) {
@@ -604,17 +599,6 @@ int enqueue_gradient_twisted(bta_ctx* c, void* ws, cudaStream_t s0, bool timed, 
   cudaEvent_t* ev = c->ev;
   // streams: [matrix][up, down]
   cudaStream_t st[2][2] = {{s0, c->s_aux[0]}, {c->s_side, c->s_aux[1]}};
-  // forward sweeps: the same streams, or (BTA_FWD_RESERVE) streams of the green context that leaves some SMs to the
-  // latency-bound kernels of the other chains' recursions (model.cu: make_forward_partition)
-  cudaStream_t fs[2][2];
-  for (int m = 0; m < 2; ++m)
-    for (int q = 0; q < 2; ++q) fs[m][q] = c->s_fwd[2 * m + q] ? c->s_fwd[2 * m + q] : st[m][q];
-  auto hand_over = [&](cudaStream_t from, cudaStream_t to) -> cudaError_t {
-    if (from == to) return cudaSuccess;
-    cudaEvent_t e = c->ev_sw[(c->ev_sw_next++) % BTA_NSW];
-    cudaError_t ce = cudaEventRecord(e, from);
-    return ce != cudaSuccess ? ce : cudaStreamWaitEvent(to, e, 0);
-  };
 #define REC(i, s)                                      \
   do {                                                 \
     if (timed) BTA_CUDA_OK(cudaEventRecord(ev[i], s)); \
@@ -632,10 +616,7 @@ int enqueue_gradient_twisted(bta_ctx* c, void* ws, cudaStream_t s0, bool timed, 
   make_twist_chains(c, wp, false, value_only, ch[1]);
   const MatWs* W[2] = {&wc, &wp};
   {
-    static const int lanes = [] {
-      const char* e = getenv("BTA_LANES");
-      return e ? atoi(e) : 1;
-    }();
+    const int lanes = c->opt.lanes;
     if (lanes)
       for (int m = 0; m < 2; ++m) {
         ch[m][0].hi = c->s_hi[2 * m];
@@ -648,11 +629,7 @@ int enqueue_gradient_twisted(bta_ctx* c, void* ws, cudaStream_t s0, bool timed, 
   for (int m = 0; m < 2; ++m)
     for (int q = 0; q < 3; ++q) ch[m][q].trace_id = 3 * m + q;
   {
-    static const int split = [] {
-      const char* e = getenv("BTA_SPLIT");
-      return e ? atoi(e) : 1;
-    }();
-    if (split)
+    if (c->opt.split)
       for (int m = 0; m < 2; ++m)
         for (int q = 0; q < 2; ++q) ch[m][q].xs = c->s_x[2 * m + q];
   }
@@ -673,7 +650,7 @@ int enqueue_gradient_twisted(bta_ctx* c, void* ws, cudaStream_t s0, bool timed, 
     hi = std::min(hi, top);
     if (lo >= hi) return BTA_OK;
     BTA_CUDA_OK(launch_assemble_seq(c, m == 0 ? BTA_COND : BTA_PRIOR, 0, k.tg(lo), k.tdir, hi - lo, 0,
-                                    k.D + (long long)lo * k.d_stride, k.d_stride, fs[m][q]));
+                                    k.D + (long long)lo * k.d_stride, k.d_stride, st[m][q]));
     return BTA_OK;
   };
   for (int m = 0; m < 2; ++m) {
@@ -690,10 +667,7 @@ int enqueue_gradient_twisted(bta_ctx* c, void* ws, cudaStream_t s0, bool timed, 
 
   // ---- forward: four sub-chains, launches interleaved block by block
   for (int m = 0; m < 2; ++m)
-    for (int q = 0; q < 2; ++q) {
-      BTA_CUDA_OK(hand_over(st[m][q], fs[m][q]));
-      BTA_CUDA_OK(chain_forward_begin(ch[m][q], fs[m][q]));
-    }
+    for (int q = 0; q < 2; ++q) BTA_CUDA_OK(chain_forward_begin(ch[m][q], st[m][q]));
   const int maxlen = std::max(ch[0][0].nt, ch[0][1].nt);
   for (int m = 0; m < 2; ++m)
     for (int q = 0; q < 2; ++q) {
@@ -705,17 +679,14 @@ int enqueue_gradient_twisted(bta_ctx* c, void* ws, cudaStream_t s0, bool timed, 
       for (int q = 0; q < 2; ++q)
         if (s < ch[m][q].nt) {
           if (s % AHEAD == 0) {  // blocks s+2 .. s+AHEAD+1 (block s+1 receives this step's Schur update)
-            BTA_CUDA_OK(chain_to_big(ch[m][q], fs[m][q]));
+            BTA_CUDA_OK(chain_to_big(ch[m][q], st[m][q]));
             int rc = assemble_range(m, q, s + 2, s + 2 + AHEAD);
             if (rc != BTA_OK) return rc;
           }
-          BTA_CUDA_OK(chain_forward_step(ch[m][q], s, fs[m][q]));
+          BTA_CUDA_OK(chain_forward_step(ch[m][q], s, st[m][q]));
         }
   for (int m = 0; m < 2; ++m)
-    for (int q = 0; q < 2; ++q) {
-      BTA_CUDA_OK(chain_to_big(ch[m][q], fs[m][q]));
-      BTA_CUDA_OK(hand_over(fs[m][q], st[m][q]));
-    }
+    for (int q = 0; q < 2; ++q) BTA_CUDA_OK(chain_to_big(ch[m][q], st[m][q]));
   for (int m = 0; m < 2; ++m) {
     BTA_CUDA_OK(join_lanes(m, 0));
     BTA_CUDA_OK(join_lanes(m, 1));
@@ -765,8 +736,9 @@ int enqueue_gradient_twisted(bta_ctx* c, void* ws, cudaStream_t s0, bool timed, 
   const int nout = 1 + md.d + 2 + 3 * md.d + md.k + 1;
   BTA_CUDA_OK(cudaMemcpyAsync(c->host_pinned + 64, c->small + L.out, nout * sizeof(double), cudaMemcpyDeviceToHost,
                               s0));
+  BTA_CUDA_OK(cudaMemcpyAsync(c->x_keep, wc.x, md.N * sizeof(double), cudaMemcpyDeviceToDevice, s0));
   REC(8, s0);
-  c->last_x_dev = wc.x;
+  c->have_x = true;
   (void)h;
 #undef REC
   return BTA_OK;
@@ -780,13 +752,11 @@ int value_and_grad_impl(bta_ctx* c, const double* theta, double* f, double* grad
   const int gi = value_only ? 1 : 0;
   cudaStream_t s0 = (cudaStream_t)stream;
   const ModelDims& md = c->md;
-  BTA_CUDA_OK(cudaSetDevice(c->device));
-  const char* env = getenv("BTA_SERIAL_CHAINS");
-  const bool serial = env && env[0] == '1';
+  DeviceGuard guard(c->device);
+  const bool serial = c->opt.serial != 0;
   // Small blocks are launch/latency-bound (tens of thousands of ~2 us kernels): from the second call on, replay
-  // the whole gradient as one CUDA graph.  BTA_GRAPH=0/1 overrides the size rule (b <= 1024).
-  const char* genv = getenv("BTA_GRAPH");
-  const bool want_graph = genv ? genv[0] == '1' : md.b <= 1024;
+  // the whole gradient as one CUDA graph.  BTA_OPT_GRAPH = 0/1 overrides the size rule (b <= 1024).
+  const bool want_graph = c->opt.graph >= 0 ? c->opt.graph == 1 : md.b <= 1024;
   cudaEvent_t* ev = c->ev;
   memcpy(c->host_pinned, theta, md.d * sizeof(double));
   cudaStream_t sync_stream = s0;
@@ -800,7 +770,7 @@ int value_and_grad_impl(bta_ctx* c, const double* theta, double* f, double* grad
       const long long n0 = c->launches;
       cudaGraph_t graph = nullptr;
       BTA_CUDA_OK(cudaStreamBeginCapture(c->s_main, cudaStreamCaptureModeThreadLocal));
-      int rc = use_twist(md) ? enqueue_gradient_twisted(c, ws, c->s_main, false, value_only)
+      int rc = use_twist(c) ? enqueue_gradient_twisted(c, ws, c->s_main, false, value_only)
                              : enqueue_gradient(c, ws, c->s_main, c->s_side, false, value_only);
       cudaError_t ce = cudaStreamEndCapture(c->s_main, &graph);
       if (rc != BTA_OK) return rc;
@@ -822,7 +792,7 @@ int value_and_grad_impl(bta_ctx* c, const double* theta, double* f, double* grad
     timed = false;
   } else {
     int rc;
-    if (use_twist(md) && !serial) {
+    if (use_twist(c) && !serial) {
       // run on the library's own prioritised streams; the caller's stream only orders the call
       BTA_CUDA_OK(cudaEventRecord(ev[11], s0));
       BTA_CUDA_OK(cudaStreamWaitEvent(c->s_main, ev[11], 0));
@@ -1037,6 +1007,7 @@ extern "C" int inla_optimize(bta_ctx* c, const double* theta0, int max_iter, dou
 extern "C" int bta_last_intermediates(bta_ctx* c, double* ld, double* x, double* parts, double* rss, double* quad,
                                       double* ZT) {
   if (!c) return bad("bta_last_intermediates: null ctx");
+  DeviceGuard guard(c->device);
   if (ld) {
     ld[0] = c->last_ld[0];
     ld[1] = c->last_ld[1];
@@ -1049,8 +1020,8 @@ extern "C" int bta_last_intermediates(bta_ctx* c, double* ld, double* x, double*
     BTA_CUDA_OK(cudaMemcpy(ZT, c->small + L.ZT[CH_COND], sizeof(double) * c->md.a * c->md.a, cudaMemcpyDeviceToHost));
   }
   if (x) {
-    if (!c->last_x_dev) return bad("bta_last_intermediates: no gradient has been computed yet");
-    BTA_CUDA_OK(cudaMemcpy(x, c->last_x_dev, c->md.N * sizeof(double), cudaMemcpyDeviceToHost));
+    if (!c->have_x) return bad("bta_last_intermediates: no gradient has been computed yet");
+    BTA_CUDA_OK(cudaMemcpy(x, c->x_keep, c->md.N * sizeof(double), cudaMemcpyDeviceToHost));
   }
   return BTA_OK;
 }

@@ -1,4 +1,4 @@
-// Error text, and the thin measurement entry points of include/bta.h.
+// Error text, and the thin measurement entry point bta_gemm of include/bta_diag.h.
 #include "common.cuh"
 
 static thread_local std::string g_err;

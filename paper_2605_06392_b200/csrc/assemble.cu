@@ -131,6 +131,32 @@ __global__ void site_fill_kernel(long long m, ModelDims md, const int* var, cons
   idx[start[s] + pos] = (int)i;
 }
 
+// In-place heapsort of idx[lo, hi) (ascending; the keys are distinct row indices, so the result is unique):
+// O(n log n) for a site with n observations -- station data can put 1e5 rows on one site.
+__device__ void sort_rows(int* idx, int lo, int hi) {
+  const int n = hi - lo;
+  int* a = idx + lo;
+  auto sift = [&](int root, int end) {
+    const int v = a[root];
+    for (;;) {
+      int ch = 2 * root + 1;
+      if (ch >= end) break;
+      if (ch + 1 < end && a[ch + 1] > a[ch]) ++ch;
+      if (a[ch] <= v) break;
+      a[root] = a[ch];
+      root = ch;
+    }
+    a[root] = v;
+  };
+  for (int r = n / 2 - 1; r >= 0; --r) sift(r, n);
+  for (int end = n - 1; end > 0; --end) {
+    const int t = a[0];
+    a[0] = a[end];
+    a[end] = t;
+    sift(0, end);
+  }
+}
+
 // One thread per latent site: sort its observation list by row index (fixed summation order), then sum.
 __global__ void site_reduce_kernel(ModelDims md, const int* start, int* idx, const int* var,
                                    const double* __restrict__ cov, const double* __restrict__ y,
@@ -139,14 +165,7 @@ __global__ void site_reduce_kernel(ModelDims md, const int* start, int* idx, con
   long long s = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (s >= S) return;
   const int lo = start[s], hi = start[s + 1];
-  for (int e = lo + 1; e < hi; ++e) {
-    int v = idx[e], q = e - 1;
-    while (q >= lo && idx[q] > v) {
-      idx[q + 1] = idx[q];
-      --q;
-    }
-    idx[q + 1] = v;
-  }
+  if (hi - lo > 1) sort_rows(idx, lo, hi);
   const long long t = s / md.b;
   const int j = (int)(s % md.b);
   double ys = 0.0, zs[AMAX];
@@ -261,10 +280,17 @@ cudaError_t run_setup_aggregates(bta_ctx* c, cudaStream_t st) {
   const long long S = (long long)md.nt * md.b, m = c->m;
   int *count = nullptr, *start = nullptr, *cursor = nullptr, *idx = nullptr;
   cudaError_t e;
-  if ((e = cudaMalloc(&count, (S + 1) * sizeof(int))) != cudaSuccess) return e;
-  if ((e = cudaMalloc(&start, (S + 1) * sizeof(int))) != cudaSuccess) return e;
-  if ((e = cudaMalloc(&cursor, (S + 1) * sizeof(int))) != cudaSuccess) return e;
-  if ((e = cudaMalloc(&idx, (m + 1) * sizeof(int))) != cudaSuccess) return e;
+  auto release = [&]() {
+    cudaFree(count);
+    cudaFree(start);
+    cudaFree(cursor);
+    cudaFree(idx);
+  };
+  if ((e = cudaMalloc(&count, (S + 1) * sizeof(int))) != cudaSuccess || (e = cudaMalloc(&start, (S + 1) * sizeof(int))) != cudaSuccess ||
+      (e = cudaMalloc(&cursor, (S + 1) * sizeof(int))) != cudaSuccess || (e = cudaMalloc(&idx, (m + 1) * sizeof(int))) != cudaSuccess) {
+    release();
+    return e;
+  }
   cudaMemsetAsync(count, 0, (S + 1) * sizeof(int), st);
   cudaMemsetAsync(cursor, 0, (S + 1) * sizeof(int), st);
   cudaMemsetAsync(c->ZZ, 0, sizeof(double) * md.k * md.a * md.a, st);
@@ -289,10 +315,7 @@ cudaError_t run_setup_aggregates(bta_ctx* c, cudaStream_t st) {
     BTA_COUNT(c);
   }
   e = cudaStreamSynchronize(st);
-  cudaFree(count);
-  cudaFree(start);
-  cudaFree(cursor);
-  cudaFree(idx);
+  release();
   if (e != cudaSuccess) return e;
   return cudaGetLastError();
 }

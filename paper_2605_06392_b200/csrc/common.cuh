@@ -7,6 +7,7 @@
 #include <vector>
 
 #include "../../include/bta.h"
+#include "../../include/bta_diag.h"
 
 #define BTA_CUDA_OK(call)                                                              \
   do {                                                                                 \
@@ -19,6 +20,36 @@
 
 void bta_set_error_cuda(cudaError_t e, const char* what, const char* file, int line);
 void bta_set_error(const char* msg);
+
+// Every entry point runs on the ctx's device and restores the caller's current device on return.
+struct DeviceGuard {
+  int prev = -1;
+  explicit DeviceGuard(int device) {
+    if (cudaGetDevice(&prev) != cudaSuccess) prev = -1;
+    if (prev != device) cudaSetDevice(device);
+    else prev = -1;
+  }
+  ~DeviceGuard() {
+    if (prev >= 0) cudaSetDevice(prev);
+  }
+  DeviceGuard(const DeviceGuard&) = delete;
+  DeviceGuard& operator=(const DeviceGuard&) = delete;
+};
+
+// cudaFuncSetAttribute(MaxDynamicSharedMemorySize) is a per-device setting: opt in once per (kernel, device).
+// `done` is one bit per device ordinal, owned by the caller (one static per kernel instantiation).
+template <class K>
+cudaError_t optin_smem(K kern, int bytes, unsigned long long* done_bits) {
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return e;
+  const unsigned long long bit = 1ull << (dev & 63);
+  if (__atomic_load_n(done_bits, __ATOMIC_ACQUIRE) & bit) return cudaSuccess;
+  e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+  if (e != cudaSuccess) return e;
+  __atomic_fetch_or(done_bits, bit, __ATOMIC_RELEASE);
+  return cudaSuccess;
+}
 
 // ------------------------------------------------------------------------------------------------
 // FP64 DMMA GEMM  (gemm.cu):  C = alpha * op(A) op(B) + beta * C, row-major, optionally batched
@@ -60,7 +91,6 @@ struct GemmArgs {
   int mode, klo, khi, out;
   const GemmSub* subs;  // device array (nsub problems; M,N,K above = maxima for the grid) or nullptr
   int nsub;
-  int dbg;              // diagnostics only (0 in production): 1 = no loads in the main loop, 2 = no barriers
   int group;            // tile-order grouping (set by launch_gemm): slow tile rows swept together, <= 1 = off
 };
 
@@ -70,9 +100,7 @@ bool gemm_uses_small_tiles(const GemmArgs& g);  // the 64x64-tile configuration 
 // ------------------------------------------------------------------------------------------------
 // Leaf / tip kernels (diag.cu)
 // ------------------------------------------------------------------------------------------------
-cudaError_t launch_potrf_inv_tile(double* A, int ld, int n, double* diagL, long long grow0,
-                                  unsigned long long* pivot_flag, cudaStream_t st);
-// leaf.cu: the blocked (16-wide panels) version of the same leaf
+// leaf.cu: POTRF + TRTRI of one n x n (n <= 128) diagonal tile in one CTA (16-wide panels, DMMA updates)
 cudaError_t launch_potrf_inv_blocked(double* A, int ld, int n, double* diagL, long long grow0,
                                      unsigned long long* pivot_flag, cudaStream_t st);
 cudaError_t launch_tip(const double* Tt, int a, int nr, int do_chol, double* LT, double* zT, double* xT, double* ZT,
@@ -120,8 +148,20 @@ struct ModelDims {
 
 constexpr int BTA_NSW = 256;
 
+// Run-time options (include/bta_diag.h: bta_set_option; defaults = the measured best, or BTA_* environment variables
+// read once in bta_create).
+struct Options {
+  int twist = 1;      // two-way elimination (four chains); 0: one chain per matrix
+  int lanes = 1;      // high-priority companion streams for the small kernels (2: forward sweeps only)
+  int split = 1;      // coupled forward step for b <= 1024
+  int graph = -1;     // CUDA-graph replay from the second call on: -1 = by size (b <= 1024), 0 off, 1 on
+  int serial = 0;     // both matrices on one stream, single chain (exclusive per-stage times)
+  int pipeline = 1;   // forward sweeps: start the next block's factorisation under the tail of this block's products
+};
+
 struct bta_ctx {
   ModelDims md;
+  Options opt;
   int device;
   long long m;
   // observations on the device
@@ -146,12 +186,6 @@ struct bta_ctx {
   cudaEvent_t ev[32];
   cudaStream_t s_hi[4];              // high-priority companions of the four chains (small kernels)
   cudaStream_t s_x[4];               // side streams of the four chains (off-chain work of the forward steps)
-  // Optional SM partition for the forward sweeps (BTA_FWD_RESERVE=R): the full-size products of the forward steps run
-  // on streams of a green context that owns all but ~R SMs, so the latency-bound kernels of the POTRF+TRTRI recursion
-  // (other chains' priority lanes) always find free SMs.  s_fwd[i] = nullptr: no partition.
-  cudaStream_t s_fwd[4];
-  void* green_ctx;                   // CUgreenCtx (opaque here)
-  int fwd_sms;                       // SMs of the forward partition (0 = none)
   cudaEvent_t ev_sw[256];            // lane-switch events, used round-robin
   unsigned ev_sw_next;
   long long launches;
@@ -159,7 +193,8 @@ struct bta_ctx {
   // last intermediates (host)
   double last_ld[2], last_quad;
   std::vector<double> last_parts, last_rss;
-  double* last_x_dev;                // device pointer into the caller's workspace (valid until it is reused)
+  double* x_keep;                    // library-owned copy of x* of the last gradient (N doubles)
+  bool have_x;
   // BTA_TRACE=<file>: phase marks of the sweeps (diagnostic timeline; events are created on demand)
   struct TraceRec { cudaEvent_t e; int chain, t, tag; };
   std::vector<TraceRec> trace;

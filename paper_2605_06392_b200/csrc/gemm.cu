@@ -8,7 +8,6 @@
 // in registers.  Triangular operands are exploited by restricting the k-range per output tile
 // (KLO_*/KHI_*), symmetric outputs by computing the lower tiles only (OUT_LOWER*).
 #include <algorithm>
-#include <cstdlib>
 
 #include "common.cuh"
 
@@ -342,12 +341,8 @@ template <int BM, int BN, int WM, int WN, bool A_KM, bool B_KM, int MINB, int BK
 cudaError_t launch_cfg(const GemmArgs& g, cudaStream_t st) {
   using C_ = Cfg<BM, BN, WM, WN, A_KM, B_KM, BK, STAGES>;
   auto kern = gemm_kernel<BM, BN, WM, WN, A_KM, B_KM, MINB, BK, STAGES, TRACE>;
-  static bool attr_done = false;  // per instantiation
-  if (!attr_done) {
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C_::SMEM);
-    if (e != cudaSuccess) return e;
-    attr_done = true;
-  }
+  static unsigned long long attr_done = 0ull;  // per instantiation, one bit per device
+  if (cudaError_t e = optin_smem(kern, C_::SMEM, &attr_done); e != cudaSuccess) return e;
   const int tilesM = (g.M + BM - 1) / BM, tilesN = (g.N + BN - 1) / BN;
   const bool swap = g.klo == KLO_N0 || g.khi == KHI_NEND;  // heavy-first enumeration (see the kernel)
   dim3 grid(swap ? tilesM : tilesN, swap ? tilesN : tilesM, g.subs ? g.nsub : 1);
@@ -380,13 +375,8 @@ long long big_tiles(const GemmArgs& g) {
   if (g.out != OUT_FULL) tiles128 = tiles128 / 2 + 1;
   return tiles128;
 }
-long long tile_threshold() {
-  static const long long thresh = [] {
-    const char* e = getenv("BTA_TILE_THRESH");
-    return e ? atoll(e) : 180LL;
-  }();
-  return thresh;
-}
+constexpr long long kTileThreshold = 180;  // fewer big tiles than this: 64x64 tiles (measured)
+constexpr long long kTinyThreshold = 148;  // at most this many 64x64 tiles: 32x32 tiles
 }  // namespace
 
 // Small tiles (64x64, three CTAs per SM) for launches of fewer than ~1.2 waves of big tiles, and wherever the last,
@@ -395,12 +385,7 @@ long long tile_threshold() {
 // 2.65 waves of 444.
 bool gemm_uses_small_tiles(const GemmArgs& g) {
   const long long t128 = big_tiles(g);
-  if (t128 < tile_threshold()) return true;
-  static const int wave_rule = [] {
-    const char* e = getenv("BTA_TILE_WAVES");
-    return e ? atoi(e) : 1;
-  }();
-  if (!wave_rule) return false;
+  if (t128 < kTileThreshold) return true;
   const long long nb = g.subs ? g.nsub : 1;
   const long long m64 = (g.M + 63) / 64, n64 = (g.N + 63) / 64;
   const long long t64 = (g.out != OUT_FULL ? std::min(m64, n64) * (std::min(m64, n64) + 1) / 2 : m64 * n64) * nb;
@@ -417,13 +402,9 @@ namespace {
 // after the other): 32x32 tiles (4 warps, 16x16 per warp) shorten each CTA's k-loop fourfold (4 DMMAs per k-step and
 // warp instead of 16) and spread the product over four times as many CTAs.
 bool gemm_uses_tiny_tiles(const GemmArgs& g) {
-  static const long long thresh = [] {
-    const char* e = getenv("BTA_TINY_THRESH");
-    return e ? atoll(e) : 148LL;
-  }();
   long long t64 = (long long)((g.M + 63) / 64) * ((g.N + 63) / 64) * (g.subs ? g.nsub : 1);
   if (g.out != OUT_FULL) t64 = t64 / 2 + 1;
-  return t64 <= thresh;
+  return t64 <= kTinyThreshold;
 }
 }  // namespace
 
@@ -431,48 +412,16 @@ static bool g_trace_host = false;  // set while bta_debug_cta_trace is armed: la
 
 cudaError_t launch_gemm(const GemmArgs& g0, cudaStream_t st) {
   if (g0.M <= 0 || g0.N <= 0) return cudaSuccess;
+  GemmArgs g = g0;
+  g.group = 16;  // tile-order grouping (sweep over 0/4/8/12/16/32)
   if (g_trace_host) {
-    GemmArgs g = g0;
-    g.dbg = 0;
-    g.group = 16;
     if (!gemm_uses_small_tiles(g)) return launch_mode<128, 128, 32, 32, 1, 16, 3, true>(g, st);
     if (gemm_uses_tiny_tiles(g)) return launch_mode<32, 32, 16, 16, 4, 16, 3, true>(g, st);
     return launch_mode<64, 64, 32, 32, 3, 16, 3, true>(g, st);
   }
-  static const int dbg = [] {
-    const char* e = getenv("BTA_GEMM_DBG");
-    return e ? atoi(e) : 0;
-  }();
-  GemmArgs g = g0;
-  g.dbg = dbg;
-  static const int group = [] {
-    const char* e = getenv("BTA_GEMM_GROUP");
-    return e ? atoi(e) : 16;
-  }();
-  g.group = group;
-  static const int big = [] {
-    const char* e = getenv("BTA_GEMM_CFG");
-    return e ? atoi(e) : 0;
-  }();
-  if (!gemm_uses_small_tiles(g)) {
-    switch (big) {
-      case 1: return launch_mode<128, 128, 32, 64, 1, 32>(g, st);
-      case 2: return launch_mode<128, 128, 32, 64, 1, 16>(g, st);
-      case 3: return launch_mode<128, 128, 32, 32, 1, 32>(g, st);
-      default: return launch_mode<128, 128, 32, 32, 1, 16>(g, st);  // 16 warps, 32x32 per warp
-    }
-  }
+  if (!gemm_uses_small_tiles(g)) return launch_mode<128, 128, 32, 32, 1, 16>(g, st);  // 16 warps, 32x32 per warp
   if (gemm_uses_tiny_tiles(g)) return launch_mode<32, 32, 16, 16, 4, 16>(g, st);
-  static const int small = [] {
-    const char* e = getenv("BTA_GEMM_SMALL");
-    return e ? atoi(e) : 3;
-  }();
-  switch (small) {
-    case 1: return launch_mode<64, 64, 32, 16, 2, 16>(g, st);
-    case 2: return launch_mode<64, 64, 32, 16, 3, 16>(g, st);
-    case 0: return launch_mode<64, 64, 32, 32, 2, 16>(g, st);
-    default: return launch_mode<64, 64, 32, 32, 3, 16>(g, st);  // three CTAs per SM
-  }
+  return launch_mode<64, 64, 32, 32, 3, 16>(g, st);                                  // three CTAs per SM
 }
 
 // Diagnostic: record one {start, end, sm, shape} entry per GEMM CTA into buf[cap][4] (device memory, caller-owned);

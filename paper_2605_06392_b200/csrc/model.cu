@@ -2,8 +2,6 @@
 #include <cstdlib>
 #include <cstring>
 
-#include <cuda.h>
-
 #include "common.cuh"
 
 namespace {
@@ -13,74 +11,9 @@ cudaError_t dev_alloc(T** p, size_t n) {
 }
 }  // namespace
 
-// Green-context SM partition for the forward sweeps (common.cuh: s_fwd).  The driver entry points are looked up at run
-// time (cudaGetDriverEntryPoint), so the library keeps no link-time dependency on libcuda.  An optimisation only: on any
-// failure the partition is left off (fwd_sms = 0) and the reason goes to bta_last_error.
 namespace {
-template <class F>
-bool drv(const char* name, F& fn) {
-  void* p = nullptr;
-  cudaDriverEntryPointQueryResult qr;
-  if (cudaGetDriverEntryPoint(name, &p, cudaEnableDefault, &qr) != cudaSuccess || qr != cudaDriverEntryPointSuccess || !p)
-    return false;
-  fn = reinterpret_cast<F>(p);
-  return true;
+int create_impl(bta_ctx* c, const bta_model_desc* desc, const bta_obs* obs);
 }
-void make_forward_partition(bta_ctx* c, int device, int reserve, int prio) {
-  CUresult (*getRes)(CUdevice, CUdevResource*, CUdevResourceType) = nullptr;
-  CUresult (*split)(CUdevResource*, unsigned int*, const CUdevResource*, CUdevResource*, unsigned int, unsigned int) =
-      nullptr;
-  CUresult (*genDesc)(CUdevResourceDesc*, CUdevResource*, unsigned int) = nullptr;
-  CUresult (*gcreate)(CUgreenCtx*, CUdevResourceDesc, CUdevice, unsigned int) = nullptr;
-  CUresult (*gstream)(CUstream*, CUgreenCtx, unsigned int, int) = nullptr;
-  CUresult (*devGet)(CUdevice*, int) = nullptr;
-  if (!drv("cuDeviceGetDevResource", getRes) || !drv("cuDevSmResourceSplitByCount", split) ||
-      !drv("cuDevResourceGenerateDesc", genDesc) || !drv("cuGreenCtxCreate", gcreate) ||
-      !drv("cuGreenCtxStreamCreate", gstream) || !drv("cuDeviceGet", devGet)) {
-    bta_set_error("BTA_FWD_RESERVE: green-context driver entry points not available");
-    return;
-  }
-  CUdevice dev;
-  CUdevResource all, part, rest;
-  if (devGet(&dev, device) != CUDA_SUCCESS || getRes(dev, &all, CU_DEV_RESOURCE_TYPE_SM) != CUDA_SUCCESS) {
-    bta_set_error("BTA_FWD_RESERVE: cuDeviceGetDevResource failed");
-    return;
-  }
-  const int total = (int)all.sm.smCount;
-  if (reserve >= total) return;
-  unsigned int ngroups = 1;
-  if (split(&part, &ngroups, &all, &rest, 0, (unsigned)(total - reserve)) != CUDA_SUCCESS || ngroups != 1) {
-    bta_set_error("BTA_FWD_RESERVE: cuDevSmResourceSplitByCount failed");
-    return;
-  }
-  CUdevResourceDesc desc;
-  CUgreenCtx g;
-  if (genDesc(&desc, &part, 1) != CUDA_SUCCESS || gcreate(&g, desc, dev, CU_GREEN_CTX_DEFAULT_STREAM) != CUDA_SUCCESS) {
-    bta_set_error("BTA_FWD_RESERVE: cuGreenCtxCreate failed");
-    return;
-  }
-  c->green_ctx = g;
-  for (auto& q : c->s_fwd) {
-    CUstream st = nullptr;
-    if (gstream(&st, g, CU_STREAM_NON_BLOCKING, prio) != CUDA_SUCCESS) {
-      bta_set_error("BTA_FWD_RESERVE: cuGreenCtxStreamCreate failed");
-      for (auto& r : c->s_fwd) {
-        if (r) cudaStreamDestroy(r);
-        r = nullptr;
-      }
-      return;
-    }
-    q = st;
-  }
-  c->fwd_sms = (int)part.sm.smCount;
-}
-void destroy_forward_partition(bta_ctx* c) {
-  if (!c->green_ctx) return;
-  CUresult (*gdestroy)(CUgreenCtx) = nullptr;
-  if (drv("cuGreenCtxDestroy", gdestroy)) gdestroy((CUgreenCtx)c->green_ctx);
-  c->green_ctx = nullptr;
-}
-}  // namespace
 
 extern "C" int bta_create(bta_ctx** out, const bta_model_desc* desc, const bta_obs* obs, int device) {
   if (!out) return BTA_ERR_ARG;
@@ -106,8 +39,21 @@ extern "C" int bta_create(bta_ctx** out, const bta_model_desc* desc, const bta_o
     bta_set_error("bta_create: device is not sm_100-class (kernels are built for sm_100a only; no fallback)");
     return BTA_ERR_NODEVICE;
   }
-  BTA_CUDA_OK(cudaSetDevice(device));
-  bta_ctx* c = new bta_ctx();
+  DeviceGuard guard(device);
+  bta_ctx* c = new bta_ctx();   // value-initialised: every pointer / handle starts as null, so bta_destroy is safe
+  c->device = device;
+  const int rc = create_impl(c, desc, obs);
+  if (rc != BTA_OK) {
+    bta_destroy(c);             // releases whatever had been allocated before the failure
+    return rc;
+  }
+  *out = c;
+  return BTA_OK;
+}
+
+namespace {
+int create_impl(bta_ctx* c, const bta_model_desc* desc, const bta_obs* obs) {
+  const int device = c->device;
   ModelDims& md = c->md;
   md.nt = desc->nt;
   md.g = desc->g;
@@ -120,16 +66,14 @@ extern "C" int bta_create(bta_ctx** out, const bta_model_desc* desc, const bta_o
   md.N = (long long)md.nt * md.b + md.a;
   md.h = desc->h;
   md.fixed_prec = desc->fixed_prec;
-  c->device = device;
   c->m = obs->m;
   c->launches = 0;
   c->last_pivot = 0;
-  c->last_x_dev = nullptr;
+  c->have_x = false;
   const long long m = obs->m;
   for (long long i = 0; i < m; ++i) {
     if (obs->var[i] < 0 || obs->var[i] >= md.k || obs->node[i] < 0 || obs->node[i] >= md.ns || obs->time[i] < 0 ||
         obs->time[i] >= md.nt) {
-      delete c;
       bta_set_error("bta_create: observation index out of range");
       return BTA_ERR_ARG;
     }
@@ -150,22 +94,19 @@ extern "C" int bta_create(bta_ctx** out, const bta_model_desc* desc, const bta_o
   BTA_CUDA_OK(dev_alloc(&c->P, 1));
   BTA_CUDA_OK(dev_alloc(&c->theta_dev, DMAX));
   BTA_CUDA_OK(dev_alloc(&c->pivot_flag, 1));
+  BTA_CUDA_OK(dev_alloc(&c->x_keep, (size_t)md.N));
   SmallLayout L = small_layout(md);
   c->small_doubles = L.total;
   BTA_CUDA_OK(dev_alloc(&c->small, L.total));
   BTA_CUDA_OK(cudaMemset(c->small, 0, L.total * sizeof(double)));
   BTA_CUDA_OK(cudaMallocHost((void**)&c->host_pinned, 4096 * sizeof(double)));
-  // Optional stream priorities (BTA_PRIORITY=1): Q_c chains highest, Q_p chains lowest.  Measured: the Q_c chains
-  // finish 25 % earlier but the Q_p chains are starved by the same amount -- with four chains in flight the GPU is
-  // throughput-bound, so the default is equal priorities.
+  // The four chains run at equal (lowest) priority: with four chains in flight the GPU is throughput-bound, and
+  // prioritising whole chains only moves time between them (measured in round 1).  Only the small latency-bound
+  // kernels of every chain get a high-priority companion stream (s_hi below).
   int prio_lo = 0, prio_hi = 0;
   BTA_CUDA_OK(cudaDeviceGetStreamPriorityRange(&prio_lo, &prio_hi));
-  {
-    const char* e = getenv("BTA_PRIORITY");
-    if (!(e && e[0] == '1')) prio_hi = prio_lo;
-  }
-  BTA_CUDA_OK(cudaStreamCreateWithPriority(&c->s_main, cudaStreamNonBlocking, prio_hi));
-  BTA_CUDA_OK(cudaStreamCreateWithPriority(&c->s_aux[0], cudaStreamNonBlocking, prio_hi));
+  BTA_CUDA_OK(cudaStreamCreateWithPriority(&c->s_main, cudaStreamNonBlocking, prio_lo));
+  BTA_CUDA_OK(cudaStreamCreateWithPriority(&c->s_aux[0], cudaStreamNonBlocking, prio_lo));
   BTA_CUDA_OK(cudaStreamCreateWithPriority(&c->s_side, cudaStreamNonBlocking, prio_lo));
   BTA_CUDA_OK(cudaStreamCreateWithPriority(&c->s_aux[1], cudaStreamNonBlocking, prio_lo));
   for (int q = 0; q < 2; ++q) {
@@ -175,23 +116,24 @@ extern "C" int bta_create(bta_ctx** out, const bta_model_desc* desc, const bta_o
   }
   c->grad_calls = 0;
   c->trace_on = getenv("BTA_TRACE") != nullptr;
+  {
+    auto env = [](const char* name, int dflt) {
+      const char* e = getenv(name);
+      return e ? atoi(e) : dflt;
+    };
+    c->opt.twist = env("BTA_TWIST", c->opt.twist);
+    c->opt.lanes = env("BTA_LANES", c->opt.lanes);
+    c->opt.split = env("BTA_SPLIT", c->opt.split);
+    c->opt.graph = env("BTA_GRAPH", c->opt.graph);
+    c->opt.serial = env("BTA_SERIAL_CHAINS", c->opt.serial);
+    c->opt.pipeline = env("BTA_PIPELINE", c->opt.pipeline);
+  }
   c->store_mode = BTA_STORE_FACTOR;
   for (auto& e : c->ev) BTA_CUDA_OK(cudaEventCreate(&e));
-  {
-    int plo = 0, phi = 0;
-    BTA_CUDA_OK(cudaDeviceGetStreamPriorityRange(&plo, &phi));
-    for (auto& q : c->s_hi) BTA_CUDA_OK(cudaStreamCreateWithPriority(&q, cudaStreamNonBlocking, phi));
-    for (auto& q : c->s_x) BTA_CUDA_OK(cudaStreamCreateWithPriority(&q, cudaStreamNonBlocking, plo));
-    for (auto& q : c->s_fwd) q = nullptr;
-    c->green_ctx = nullptr;
-    c->fwd_sms = 0;
-    if (const char* e = getenv("BTA_FWD_RESERVE")) {
-      const int reserve = atoi(e);
-      if (reserve > 0) make_forward_partition(c, device, reserve, plo);
-    }
-    for (auto& e : c->ev_sw) BTA_CUDA_OK(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
-    c->ev_sw_next = 0;
-  }
+  for (auto& q : c->s_hi) BTA_CUDA_OK(cudaStreamCreateWithPriority(&q, cudaStreamNonBlocking, prio_hi));
+  for (auto& q : c->s_x) BTA_CUDA_OK(cudaStreamCreateWithPriority(&q, cudaStreamNonBlocking, prio_lo));
+  for (auto& e : c->ev_sw) BTA_CUDA_OK(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+  c->ev_sw_next = 0;
   if (m > 0) {
     BTA_CUDA_OK(cudaMemcpy(c->o_var, obs->var, m * sizeof(int), cudaMemcpyHostToDevice));
     BTA_CUDA_OK(cudaMemcpy(c->o_node, obs->node, m * sizeof(int), cudaMemcpyHostToDevice));
@@ -200,13 +142,14 @@ extern "C" int bta_create(bta_ctx** out, const bta_model_desc* desc, const bta_o
     BTA_CUDA_OK(cudaMemcpy(c->o_y, obs->y, m * sizeof(double), cudaMemcpyHostToDevice));
   }
   BTA_CUDA_OK(run_setup_aggregates(c, 0));
-  *out = c;
+  (void)device;
   return BTA_OK;
 }
+}  // namespace
 
 extern "C" int bta_destroy(bta_ctx* c) {
   if (!c) return BTA_OK;
-  cudaSetDevice(c->device);
+  DeviceGuard guard(c->device);
   cudaFree(c->o_var);
   cudaFree(c->o_node);
   cudaFree(c->o_time);
@@ -223,19 +166,23 @@ extern "C" int bta_destroy(bta_ctx* c) {
   cudaFree(c->theta_dev);
   cudaFree(c->pivot_flag);
   cudaFree(c->small);
-  cudaFreeHost(c->host_pinned);
+  cudaFree(c->x_keep);
+  if (c->host_pinned) cudaFreeHost(c->host_pinned);
   for (int q = 0; q < 2; ++q)
     if (c->graph_exec[q]) cudaGraphExecDestroy(c->graph_exec[q]);
-  cudaStreamDestroy(c->s_side);
-  cudaStreamDestroy(c->s_main);
-  for (auto& q : c->s_aux) cudaStreamDestroy(q);
-  for (auto& e : c->ev) cudaEventDestroy(e);
-  for (auto& q : c->s_hi) cudaStreamDestroy(q);
-  for (auto& q : c->s_x) cudaStreamDestroy(q);
-  for (auto& q : c->s_fwd)
+  auto kill_stream = [](cudaStream_t q) {
     if (q) cudaStreamDestroy(q);
-  destroy_forward_partition(c);
-  for (auto& e : c->ev_sw) cudaEventDestroy(e);
+  };
+  auto kill_event = [](cudaEvent_t e) {
+    if (e) cudaEventDestroy(e);
+  };
+  kill_stream(c->s_side);
+  kill_stream(c->s_main);
+  for (auto& q : c->s_aux) kill_stream(q);
+  for (auto& q : c->s_hi) kill_stream(q);
+  for (auto& q : c->s_x) kill_stream(q);
+  for (auto& e : c->ev) kill_event(e);
+  for (auto& e : c->ev_sw) kill_event(e);
   delete c;
   return BTA_OK;
 }
@@ -259,3 +206,37 @@ extern "C" int bta_set_store_mode(bta_ctx* c, int mode) {
   return BTA_OK;
 }
 extern "C" int bta_get_store_mode(const bta_ctx* c) { return c ? c->store_mode : -1; }
+
+namespace {
+int* option_slot(bta_ctx* c, int option) {
+  switch (option) {
+    case BTA_OPT_TWIST: return &c->opt.twist;
+    case BTA_OPT_LANES: return &c->opt.lanes;
+    case BTA_OPT_SPLIT: return &c->opt.split;
+    case BTA_OPT_GRAPH: return &c->opt.graph;
+    case BTA_OPT_SERIAL: return &c->opt.serial;
+    case BTA_OPT_PIPELINE: return &c->opt.pipeline;
+  }
+  return nullptr;
+}
+}  // namespace
+
+extern "C" int bta_set_option(bta_ctx* c, int option, int value) {
+  int* slot = c ? option_slot(c, option) : nullptr;
+  if (!slot) {
+    bta_set_error("bta_set_option: null ctx or unknown option");
+    return BTA_ERR_ARG;
+  }
+  if (*slot != value)
+    for (int q = 0; q < 2; ++q)
+      if (c->graph_exec[q]) {  // a cached graph was captured with the other setting
+        cudaGraphExecDestroy(c->graph_exec[q]);
+        c->graph_exec[q] = nullptr;
+      }
+  *slot = value;
+  return BTA_OK;
+}
+extern "C" int bta_get_option(const bta_ctx* c, int option) {
+  int* slot = c ? option_slot(const_cast<bta_ctx*>(c), option) : nullptr;
+  return slot ? *slot : -1;
+}

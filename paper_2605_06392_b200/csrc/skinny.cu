@@ -14,8 +14,9 @@ namespace {
 template <int PT>
 __global__ void __launch_bounds__(256) skinny_nt_kernel(int P, int J, int K, const double* __restrict__ R, int ldr,
                                                         const double* __restrict__ M, int ldm, int tri,
-                                                        double alpha, double beta, const double* __restrict__ in,
-                                                        int ldin, double* __restrict__ out, int ldo) {
+                                                        double alpha, double beta, const double* in, int ldin,
+                                                        double* out, int ldo) {
+  // `in` and `out` may be the same buffer (in-place stack updates of the sweeps): no __restrict__ on them
   constexpr int KC = 256, RPW = NT_RPW;
   __shared__ double Rs[PT * KC];
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -121,8 +122,8 @@ __global__ void __launch_bounds__(256) skinny_nn_kernel(int P, int K, int J, con
 
 // out[p][j] = alpha * sum_ks part[ks][p][j] + beta * in[p][j]   (fixed order: deterministic)
 __global__ void skinny_nn_finish_kernel(int P, int J, int nks, const double* __restrict__ part, double alpha,
-                                        double beta, const double* __restrict__ in, int ldin,
-                                        double* __restrict__ out, int ldo) {
+                                        double beta, const double* in, int ldin, double* out, int ldo) {
+  // `in` may alias `out` (in-place update): no __restrict__ on them
   long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (e >= (long long)P * J) return;
   int p = (int)(e / J), j = (int)(e % J);
@@ -151,7 +152,7 @@ __global__ void __launch_bounds__(256) small_nt_kernel(int PU, int PV, int K, co
 // Y[r][j] = beta * In[r][j] + alpha * sum_q S[r][q] * E[q][j]   (tiny left factor: Z_T E_i, x_T^T L_C, ...)
 __global__ void small_left_mul_kernel(int R, int Q, int J, const double* __restrict__ S, int lds,
                                       const double* __restrict__ E, int lde, double alpha, double beta,
-                                      const double* __restrict__ In, int ldin, double* __restrict__ Y, int ldy) {
+                                      const double* In, int ldin, double* Y, int ldy) {  // In may alias Y
   int j = blockIdx.x * blockDim.x + threadIdx.x;
   if (j >= J) return;
   for (int r = 0; r < R; ++r) {

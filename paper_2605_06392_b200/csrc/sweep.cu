@@ -58,13 +58,10 @@ cudaError_t potrf_inv(bta_ctx* c, Chain* lch, double* A, int ld, int lo, int hi,
                       long long grow0, cudaStream_t st) {
   const int n = hi - lo;
   if (n <= 0) return cudaSuccess;
-  static const int LEAF = [] {
-    const char* e = getenv("BTA_LEAF");
-    return (e && atoi(e) == 64) ? 64 : 128;
-  }();
+  constexpr int LEAF = 128;
   if (n <= LEAF) {
     BTA_COUNT(c);
-    return launch_potrf_inv_tile(A + (long long)lo * ld + lo, ld, n, diagL ? diagL + lo : nullptr, grow0 + lo,
+    return launch_potrf_inv_blocked(A + (long long)lo * ld + lo, ld, n, diagL ? diagL + lo : nullptr, grow0 + lo,
                                  c->pivot_flag, SS);
   }
   const int ntile = (n + LEAF - 1) / LEAF;
@@ -234,10 +231,7 @@ cudaError_t chain_forward_step(Chain& ch, int t, cudaStream_t st) {
       CK(cudaMemcpyAsync(Dt, At, bb * sizeof(double), cudaMemcpyDeviceToDevice, SB));
       CK(potrf_inv(c, lch, Dt, b, 0, b, ch.W1, ch.Bs, ch.dvec ? ch.dvec + tg * b : nullptr, tg * b, st));
     } else {
-      static const int split_maxb = [] {
-        const char* e = getenv("BTA_SPLIT_MAXB");
-        return e ? atoi(e) : 1024;
-      }();
+      constexpr int split_maxb = 1024;  // the coupled step pays only where a step is latency-bound
       const bool has_coupling = t < nt - 1 || ch.tail_coupling;
       coupled = has_coupling && ch.xs && b > 128 && b <= split_maxb;
       if (coupled) {

@@ -1,5 +1,5 @@
 """Diagnostic: SM-slot occupancy timeline of the GEMM CTAs during one gradient ("Where the forward
-sweep loses time").  Not part of the hot path: it arms `bta_debug_cta_trace` (include/bta.h), runs one
+sweep loses time").  Not part of the hot path: it arms `bta_debug_cta_trace` (include/bta_diag.h), runs one
 `inla_value_and_grad` and bins the per-CTA {start, end, SM id, tile} records.
 
     python -m paper_2605_06392_b200.diagnostics --config 2 [--nt N] [--slices 20]

@@ -323,3 +323,57 @@ def test_mode_search_matches_scipy_on_the_oracle(name):
     assert np.max(np.abs(th - ref.x)) <= 1e-4
     r = O.value_and_grad(model, obs, th)            # the oracle agrees at the GPU optimum
     assert abs(r["f"] - f) <= TOL_F * abs(f) and np.max(np.abs(r["grad"])) <= 1e-4
+
+
+def test_workspace_canaries():
+    """compute-sanitizer is closed on this pool (profiles/r02_sanitizer_refusal.md), so out-of-bounds writes are
+    looked for directly: guard words on both sides of the caller-provided workspace must survive a gradient in either
+    store mode (ragged block size, twisted path, arrow width 3)."""
+    import torch
+    model, obs, th = CASES["b25_ragged"]()
+    ref = O.value_and_grad(model, obs, th)
+    M = _model(model, obs)
+    for mode in (0, 1):
+        M.bta_set_store_mode(mode)
+        need = M.workspace_bytes()
+        guard = 1 << 16
+        buf = torch.full((need + 2 * guard,), 0xA5, dtype=torch.uint8, device="cuda")
+        M._ws = buf[guard: guard + need]                       # the binding hands this view's pointer to the library
+        f, g = M.inla_value_and_grad(th)
+        assert abs(f - ref["f"]) <= TOL_F * abs(ref["f"]) and grad_ok(g, ref["grad"])
+        assert bool((buf[:guard] == 0xA5).all()) and bool((buf[guard + need:] == 0xA5).all())
+    M.close()
+
+
+def test_many_observations_on_one_site():
+    """Model setup sorts each site's observation list (fixed summation order): 20,000 rows on ONE latent site plus a
+    uniform remainder -- the O(n log n) per-site sort of assemble.cu, against the oracle's aggregates."""
+    model = make_model(6, 1, 4, 2)
+    obs = draw_obs(model, 25000, 51)
+    obs.node[:20000] = 7
+    obs.time[:20000] = 2
+    th = draw_theta(model, 51)
+    ref = O.value_and_grad(model, obs, th)
+    M = _model(model, obs)
+    f, g = M.inla_value_and_grad(th)
+    M.close()
+    assert abs(f - ref["f"]) <= TOL_F * abs(ref["f"]) and grad_ok(g, ref["grad"])
+
+
+def test_second_device_ordinal():
+    """cudaFuncSetAttribute is per device: a context on ordinal 1 must work after ordinal 0, and the caller's
+    current device is left alone (round-1 advisor finding)."""
+    import torch
+    if torch.cuda.device_count() < 2:
+        pytest.skip("needs two GPUs")
+    from paper_2605_06392_b200 import BtaModel
+    model, obs, th = CASES["b144_h07"]()
+    ref = O.value_and_grad(model, obs, th)
+    for dev in (0, 1):
+        torch.cuda.set_device(0)
+        M = BtaModel.from_workload(model, obs, device=dev)
+        with torch.cuda.device(dev):
+            f, g = M.inla_value_and_grad(th)
+        assert torch.cuda.current_device() == 0
+        M.close()
+        assert abs(f - ref["f"]) <= TOL_F * abs(ref["f"]) and grad_ok(g, ref["grad"])

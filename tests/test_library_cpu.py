@@ -20,9 +20,12 @@ def lib():
 
 
 def declared_symbols():
-    src = open(os.path.join(ROOT, "include", "bta.h")).read()
-    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
-    return sorted(set(re.findall(r"\b((?:bta|inla)_[a-z0-9_]+)\s*\(", src)))
+    names = set()
+    for hdr in ("bta.h", "bta_diag.h"):
+        src = open(os.path.join(ROOT, "include", hdr)).read()
+        src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+        names |= set(re.findall(r"\b((?:bta|inla)_[a-z0-9_]+)\s*\(", src))
+    return sorted(names)
 
 
 def test_every_declared_symbol_is_exported(lib):
@@ -35,6 +38,9 @@ def test_every_declared_symbol_is_exported(lib):
                          capture_output=True, text=True).stdout
     for n in names:
         assert re.search(rf"\bT {n}\b", out), n
+    # built with -fvisibility=hidden: nothing but the declared entry points is exported
+    exported = set(re.findall(r"\b[TDB] (\w+)", out))
+    assert exported == set(names), exported ^ set(names)
 
 
 def test_library_holds_sm100a_dmma_code():
