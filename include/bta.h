@@ -95,10 +95,20 @@ BTA_API int bta_destroy(bta_ctx* ctx);
  *   BTA_STORE_CARRY: the paper's carry-based reconstruction -- only the Schur-updated diagonal blocks
  *     D_t - S_{t-1} ("carries", nt b^2 doubles per matrix) and the O(a b) arrow rows / z_t are kept; the backward
  *     sweep rebuilds X_t (one more Cholesky + inverse) and L_Bt (B_t is re-assembled, one more product) per block.
+ *   BTA_STORE_HOST: carry mode with the carries staged in page-locked HOST memory (§III-C c): each
+ *     carry is copied out on a copy stream during the forward sweep and streamed back one block at a time, a few blocks
+ *     ahead, during the backward sweep; the device keeps a ring of 4 diagonal-block slots per sub-chain, so the device
+ *     workspace is O(b^2) whatever nt is.  Needs nt >= 3 (else it behaves as BTA_STORE_CARRY) and a host buffer of
+ *     bta_host_bytes(ctx) bytes registered with bta_set_host_buffer before the next inla_value_and_grad.
  * Changes bta_workspace_bytes.  Returns BTA_ERR_ARG for an unknown mode. */
-enum { BTA_STORE_FACTOR = 0, BTA_STORE_CARRY = 1 };
+enum { BTA_STORE_FACTOR = 0, BTA_STORE_CARRY = 1, BTA_STORE_HOST = 2 };
 BTA_API int bta_set_store_mode(bta_ctx* ctx, int mode);
 BTA_API int bta_get_store_mode(const bta_ctx* ctx);
+/* BTA_STORE_HOST: bytes of host staging memory needed (2 (nt-1) b^2 doubles), and its registration.  `host` is HOST
+ * memory owned by the caller; it should be page-locked (cudaHostAlloc / torch pin_memory) -- pageable memory works but
+ * the copies then do not overlap the sweeps.  It must stay valid until the mode is left or the ctx destroyed. */
+BTA_API size_t bta_host_bytes(const bta_ctx* ctx);
+BTA_API int bta_set_host_buffer(bta_ctx* ctx, void* host, size_t bytes);
 
 /* Bytes of caller-provided device workspace needed by inla_value_and_grad (the largest user: both matrices'
  * blocks, per-chain temporaries).  bta_factor_logdet / bta_solve / bta_selinv need at most

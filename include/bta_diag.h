@@ -24,6 +24,28 @@ BTA_API int bta_gemm(int mode, int M, int N, int K, double alpha, const double* 
 BTA_API int bta_debug_cta_trace(unsigned long long* buf, unsigned int cap);
 BTA_API int bta_debug_cta_trace_count(unsigned int* n);
 
+/* Per-kernel-class timing: between _begin and _end every kernel launch of the library is bracketed by a pair of CUDA
+ * events on its stream; _end synchronises the device and returns, per class, the summed event intervals (ms), the
+ * ALGORITHMIC flops and bytes of those launches (element-exact: triangular operands and lower-only outputs count what
+ * they need, not what the tiles execute; bandwidth classes count the bytes each launch must read or write once) and
+ * the number of launches.  Arrays of BTA_KC_COUNT entries; any may be NULL.  Use with BTA_OPT_SERIAL = 1 (one stream)
+ * so that the intervals are exclusive.  Process-global (not per ctx); launches inside a CUDA-graph capture are skipped. */
+enum {
+  BTA_KC_GEMM_BIG = 0,    /* gemm_kernel, 128x128 tiles */
+  BTA_KC_GEMM_SMALL = 1,  /* gemm_kernel, 64x64 tiles */
+  BTA_KC_GEMM_TINY = 2,   /* gemm_kernel, 32x32 tiles */
+  BTA_KC_LEAF = 3,        /* potrf_inv_blocked_kernel: flops 2/3 n^3 */
+  BTA_KC_SKINNY = 4,      /* skinny_nt / skinny_nn: bytes = the b x b operand (half if triangular) */
+  BTA_KC_CONTRACT = 5,    /* trace_stencil / noise_trace / quad_stencil: bytes = the gathered stencil entries */
+  BTA_KC_ASSEMBLE = 6,    /* assemble_*: bytes = the blocks written */
+  BTA_KC_OTHER = 7,       /* tips, small products, reductions, scalars */
+  BTA_KC_COUNT = 8
+};
+/* Host-only: the element-exact flop count the timing registers for one GEMM launch (klo/khi/out as in bta_gemm). */
+BTA_API double bta_diag_gemm_flop(int M, int N, int K, int klo, int khi, int out);
+BTA_API int bta_diag_ktime_begin(void);
+BTA_API int bta_diag_ktime_end(double* ms, double* flop, double* bytes, long long* count);
+
 /* Run-time switches of the sweep orchestration (diagnostics and A/B measurements; the defaults are the measured
  * best).  bta_create also reads the environment variables named below once, as initial values.
  *   BTA_OPT_TWIST (BTA_TWIST)          1: two-way elimination, four chains (default); 0: one chain per matrix
@@ -31,11 +53,15 @@ BTA_API int bta_debug_cta_trace_count(unsigned int* n);
  *   BTA_OPT_SPLIT (BTA_SPLIT)          1: coupled forward step for b <= 1024 (default); 0: off
  *   BTA_OPT_GRAPH (BTA_GRAPH)          -1: CUDA-graph replay for b <= 1024 (default); 0: never; 1: always
  *   BTA_OPT_SERIAL (BTA_SERIAL_CHAINS) 1: both matrices on one stream, single chain -- exclusive per-stage times
- *   BTA_OPT_PIPELINE (BTA_PIPELINE)    1: forward sweeps overlap the next block's factorisation with the tail of
- *                                      this block's products (default); 0: strict block-by-block order
+ *   BTA_OPT_PIPELINE (BTA_PIPELINE)    1: forward sweeps (b > 1024, factor mode) overlap the first half of the next
+ *                                      block's factorisation with the tail of this block's products (default);
+ *                                      0: strict block-by-block order
+ *   BTA_OPT_TILE_THRESH (BTA_TILE_THRESH), BTA_OPT_TILE_WAVES (BTA_TILE_WAVES): the GEMM tile rule (process-global):
+ *                                      launches of fewer 128x128 tiles than the threshold (180) use 64x64 tiles, and
+ *                                      (waves = 1) so do launches whose last wave of 128x128 tiles would be mostly empty
  * Returns BTA_ERR_ARG for an unknown option.  Cached CUDA graphs are dropped. */
 enum { BTA_OPT_TWIST = 0, BTA_OPT_LANES = 1, BTA_OPT_SPLIT = 2, BTA_OPT_GRAPH = 3, BTA_OPT_SERIAL = 4,
-       BTA_OPT_PIPELINE = 5 };
+       BTA_OPT_PIPELINE = 5, BTA_OPT_TILE_THRESH = 6, BTA_OPT_TILE_WAVES = 7 };
 BTA_API int bta_set_option(bta_ctx* ctx, int option, int value);
 BTA_API int bta_get_option(const bta_ctx* ctx, int option);
 

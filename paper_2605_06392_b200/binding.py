@@ -74,11 +74,18 @@ def lib():
     L.bta_kernel_launches.restype = i64
     L.bta_last_error.restype = C.c_char_p
     L.bta_set_store_mode.argtypes = [vp, i32]
+    L.bta_host_bytes.argtypes = [vp]
+    L.bta_host_bytes.restype = C.c_size_t
+    L.bta_set_host_buffer.argtypes = [vp, vp, C.c_size_t]
     L.bta_get_store_mode.argtypes = [vp]
     L.bta_fp64_peak.argtypes = [i32, i32, dp, dp, vp]
     L.bta_gemm.argtypes = [i32, i32, i32, i32, C.c_double, vp, i32, vp, i32, C.c_double, vp, i32, i32, i32, i32, vp]
     L.bta_debug_cta_trace.argtypes = [vp, C.c_uint]
     L.bta_debug_cta_trace_count.argtypes = [C.POINTER(C.c_uint)]
+    L.bta_diag_gemm_flop.argtypes = [i32, i32, i32, i32, i32, i32]
+    L.bta_diag_gemm_flop.restype = C.c_double
+    L.bta_diag_ktime_begin.argtypes = []
+    L.bta_diag_ktime_end.argtypes = [dp, dp, dp, C.POINTER(C.c_int64)]
     L.bta_set_option.argtypes = [vp, i32, i32]
     L.bta_get_option.argtypes = [vp, i32]
     _lib = L
@@ -118,7 +125,7 @@ class Blocks:
 
 
 BTA_PRIOR, BTA_COND = 0, 1
-BTA_STORE_FACTOR, BTA_STORE_CARRY = 0, 1
+BTA_STORE_FACTOR, BTA_STORE_CARRY, BTA_STORE_HOST = 0, 1, 2
 OPT_TWIST, OPT_LANES, OPT_SPLIT, OPT_GRAPH, OPT_SERIAL, OPT_PIPELINE = range(6)
 STAGES = ("assemble", "fwd_Qc", "bwd_Qc", "fwd_Qp", "bwd_Qp", "scalars", "total")
 
@@ -145,6 +152,7 @@ class BtaModel:
         self.N = lib().bta_latent_size(self._h)
         self._ws = None
         self._ws_op = None
+        self._host = None
 
     @classmethod
     def from_workload(cls, model, obs, device=0):
@@ -155,7 +163,7 @@ class BtaModel:
         if self._h:
             lib().bta_destroy(self._h)
             self._h = C.c_void_p()
-            self._ws = self._ws_op = None
+            self._ws = self._ws_op = self._host = None
 
     def __del__(self):
         try:
@@ -274,9 +282,23 @@ class BtaModel:
                     phaseC=parts[2 * self.d:], rss=rss, quad_p=quad.value)
 
     def bta_set_store_mode(self, mode):
-        """BTA_STORE_FACTOR (0) or BTA_STORE_CARRY (1); the gradient workspace is re-sized on next use."""
+        """BTA_STORE_FACTOR (0), BTA_STORE_CARRY (1) or BTA_STORE_HOST (2); the gradient workspace is re-sized on next
+        use.  For BTA_STORE_HOST a pinned torch tensor of bta_host_bytes() is allocated and registered."""
+        import torch
         _check(lib().bta_set_store_mode(self._h, int(mode)))
         self._ws = None
+        if int(mode) == BTA_STORE_HOST:
+            need = lib().bta_host_bytes(self._h)
+            if need and (self._host is None or self._host.numel() < need):
+                self._host = torch.empty(need, dtype=torch.uint8, pin_memory=True)
+            if need:
+                _check(lib().bta_set_host_buffer(self._h, self._host.data_ptr(), need))
+        else:
+            _check(lib().bta_set_host_buffer(self._h, None, 0))
+            self._host = None
+
+    def bta_host_bytes(self):
+        return lib().bta_host_bytes(self._h)
 
     def bta_get_store_mode(self):
         return lib().bta_get_store_mode(self._h)
@@ -316,6 +338,28 @@ def gemm(mode, A, B, Cm, alpha=1.0, beta=0.0, klo=0, khi=0, out=0):
     _check(lib().bta_gemm(mode, M, N, K, alpha, A.data_ptr(), A.stride(0), B.data_ptr(), B.stride(0), beta,
                           Cm.data_ptr(), Cm.stride(0), klo, khi, out, _stream()))
     return Cm
+
+
+KCLASSES = ("gemm_128", "gemm_64", "gemm_32", "leaf", "skinny", "contract", "assemble", "other")
+
+
+def ktime_begin():
+    """include/bta_diag.h: arm the per-kernel-class timing (every launch bracketed by CUDA events)."""
+    _check(lib().bta_diag_ktime_begin())
+
+
+def ktime_end():
+    """-> {class: dict(ms, flop, bytes, launches)} of the launches since ktime_begin (synchronises the device)."""
+    n = len(KCLASSES)
+    ms, fl, by = np.zeros(n), np.zeros(n), np.zeros(n)
+    cnt = np.zeros(n, dtype=np.int64)
+    _check(lib().bta_diag_ktime_end(_dptr(ms), _dptr(fl), _dptr(by), cnt.ctypes.data_as(C.POINTER(C.c_int64))))
+    return {k: dict(ms=float(ms[i]), flop=float(fl[i]), bytes=float(by[i]), launches=int(cnt[i]))
+            for i, k in enumerate(KCLASSES)}
+
+
+def gemm_alg_flop(M, N, K, klo=0, khi=0, out=0):
+    return lib().bta_diag_gemm_flop(M, N, K, klo, khi, out)
 
 
 def cta_trace_start(buf):

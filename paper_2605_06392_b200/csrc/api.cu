@@ -4,20 +4,9 @@
 #include <cstdlib>
 #include <cstring>
 
-#include "sweep.h"
+#include "api_util.h"
 
 namespace {
-
-struct Bump {
-  char* base;
-  size_t off = 0;
-  explicit Bump(void* p) : base((char*)p) {}
-  double* take(size_t doubles) {
-    double* r = (double*)(base + off);
-    off += (doubles * sizeof(double) + 255) / 256 * 256;
-    return r;
-  }
-};
 
 struct ChainWs {
   double *D, *B, *W1, *W2, *W3, *Rin, *Rout, *ubuf, *Ebuf, *Ybuf, *ZC0, *ZC1, *part, *x, *dvec, *T, *rtip, *Xs, *LBs, *Bs;
@@ -30,7 +19,7 @@ ChainWs carve_chain(Bump& bp, const ModelDims& md, bool cond, int store_mode) {
   const size_t bb = (size_t)md.b * md.b;
   const int P = md.a + 1;
   w.D = bp.take(bb * md.nt);
-  if (store_mode == BTA_STORE_CARRY) {
+  if (store_mode != BTA_STORE_FACTOR) {
     w.Xs = bp.take(bb);
     w.LBs = bp.take(bb);
     w.Bs = bp.take(bb);
@@ -104,11 +93,6 @@ int check_pivot(bta_ctx* c, cudaStream_t st) {
   }
   c->last_pivot = 0;
   return BTA_OK;
-}
-
-int bad(const char* msg) {
-  bta_set_error(msg);
-  return BTA_ERR_ARG;
 }
 
 }  // namespace
@@ -303,7 +287,7 @@ int enqueue_gradient(bta_ctx* c, void* ws, cudaStream_t s0, cudaStream_t s1, boo
   const ModelDims& md = c->md;
   const bool serial = (s0 == s1);
   Bump bp(ws);
-  const bool carry = c->store_mode == BTA_STORE_CARRY;
+  const bool carry = c->store_mode != BTA_STORE_FACTOR;  // host staging needs the two-way sweep (nt >= 3): plain carry here
   ChainWs wc = carve_chain(bp, md, true, c->store_mode);
   ChainWs wp = carve_chain(bp, md, false, c->store_mode);
   SmallLayout L = small_layout(md);
@@ -454,8 +438,9 @@ int enqueue_gradient(bta_ctx* c, void* ws, cudaStream_t s0, cudaStream_t s1, boo
 // same results up to rounding order -- but four independent chains (two per matrix) instead of two, so the
 // latency-bound POTRF phases of one chain overlap the GEMMs of three others.
 struct SubWs {
-  double *B, *W1, *W2, *W3, *Xs, *LBs, *Bs, *ubuf, *Ebuf, *Ybuf, *ZC0, *ZC1, *part;
+  double *B, *W1, *W2, *W3, *Xs, *LBs, *Bs, *ubuf, *Ebuf, *Ybuf, *ZC0, *ZC1, *part, *ring;
 };
+constexpr int HOST_RING = 4;  // device slots per sub-chain for the diagonal blocks in BTA_STORE_HOST
 struct MatWs {
   double *D, *dvec, *T, *Rin, *Rout, *x, *rtip, *Tt2;
   SubWs sub[3];  // up, down, separator
@@ -468,7 +453,7 @@ MatWs carve_twist(Bump& bp, const ModelDims& md, bool cond, int store_mode) {
   const size_t bb = (size_t)md.b * md.b;
   const int P = md.a + 1, h = twist_h(md);
   const int len[3] = {h, md.nt - 1 - h, 1};
-  w.D = bp.take(bb * md.nt);
+  w.D = bp.take(store_mode == BTA_STORE_HOST ? bb : bb * md.nt);  // host staging: only the separator block
   w.dvec = bp.take(md.N);
   w.T = bp.take(md.a * md.a);
   w.Tt2 = bp.take(md.a * (md.a + 1));
@@ -484,10 +469,11 @@ MatWs carve_twist(Bump& bp, const ModelDims& md, bool cond, int store_mode) {
     s.W2 = bp.take(bb);
     s.W3 = bp.take(bb);
     if (q < 2) {
-      if (store_mode == BTA_STORE_CARRY) {
+      if (store_mode != BTA_STORE_FACTOR) {
         s.Xs = bp.take(bb);
         s.LBs = bp.take(bb);
         s.Bs = bp.take(bb);
+        if (store_mode == BTA_STORE_HOST) s.ring = bp.take(bb * HOST_RING);
       } else {
         s.B = bp.take(bb * (len[q] + 1));
       }
@@ -520,7 +506,7 @@ void make_twist_chains(bta_ctx* c, const MatWs& w, bool cond, bool value_only, C
   const long long bb = (long long)md.b * md.b;
   const int P = md.a + 1, h = twist_h(md);
   const int chs = cond ? CH_COND : CH_PRIOR;
-  const bool carry = c->store_mode == BTA_STORE_CARRY;
+  const bool carry = c->store_mode != BTA_STORE_FACTOR, host = c->store_mode == BTA_STORE_HOST;
   const long long rs = (long long)P * md.b;
   for (int q = 0; q < 3; ++q) {
     Chain& k = ch[q];
@@ -543,6 +529,17 @@ void make_twist_chains(bta_ctx* c, const MatWs& w, bool cond, bool value_only, C
     k.carry = carry && q < 2;
     k.D = w.D + (long long)k.t0 * bb;
     k.d_stride = k.tdir * bb;
+    if (host) {
+      k.D = q < 2 ? s.ring : w.D;
+      k.d_stride = bb;
+      if (q < 2) {
+        const int mi = cond ? 0 : 1;
+        k.ring = HOST_RING;
+        k.hostD = c->host_buf + ((long long)mi * (md.nt - 1) + (q == 1 ? h : 0)) * bb;
+        k.cs = c->s_copy[2 * mi + q];
+        k.ring_ev = c->ev_ring[2 * mi + q];
+      }
+    }
     k.Bin = (q < 2 && !carry) ? s.B + bb : nullptr;
     k.Bout = s.B;
     k.b_stride = bb;
@@ -595,7 +592,9 @@ int enqueue_gradient_twisted(bta_ctx* c, void* ws, cudaStream_t s0, bool timed, 
   SmallLayout L = small_layout(md);
   const long long bb = (long long)md.b * md.b;
   const int P = md.a + 1, h = twist_h(md);
-  const bool carry = c->store_mode == BTA_STORE_CARRY;
+  const bool carry = c->store_mode != BTA_STORE_FACTOR, host = c->store_mode == BTA_STORE_HOST;
+  if (host && (!c->host_buf || c->host_bytes < bta_host_bytes(c)))
+    return bad("inla_value_and_grad: BTA_STORE_HOST needs bta_set_host_buffer(ctx, pinned, bta_host_bytes(ctx)) first");
   cudaEvent_t* ev = c->ev;
   // streams: [matrix][up, down]
   cudaStream_t st[2][2] = {{s0, c->s_aux[0]}, {c->s_side, c->s_aux[1]}};
@@ -628,11 +627,12 @@ int enqueue_gradient_twisted(bta_ctx* c, void* ws, cudaStream_t s0, bool timed, 
   auto join_lanes = [&](int m, int q) { return chain_to_big(ch[m][q], st[m][q == 2 ? 0 : q]); };
   for (int m = 0; m < 2; ++m)
     for (int q = 0; q < 3; ++q) ch[m][q].trace_id = 3 * m + q;
-  {
-    if (c->opt.split)
-      for (int m = 0; m < 2; ++m)
-        for (int q = 0; q < 2; ++q) ch[m][q].xs = c->s_x[2 * m + q];
-  }
+  // side streams: off-chain work of the coupled forward step (b <= 1024); the events of the pipelined forward steps
+  for (int m = 0; m < 2; ++m)
+    for (int q = 0; q < 2; ++q) {
+      if (c->opt.split) ch[m][q].xs = c->s_x[2 * m + q];
+      ch[m][q].pipe_ev = c->ev_pipe[2 * m + q];
+    }
 
   // ---- assemble: D (all blocks), arrow/rhs rows, tip on the up stream; coupling blocks per sub-chain
   // The diagonal blocks are assembled lazily, a few blocks ahead of each sub-chain (assemble_ahead below): the 2 nt
@@ -669,16 +669,31 @@ int enqueue_gradient_twisted(bta_ctx* c, void* ws, cudaStream_t s0, bool timed, 
   for (int m = 0; m < 2; ++m)
     for (int q = 0; q < 2; ++q) BTA_CUDA_OK(chain_forward_begin(ch[m][q], st[m][q]));
   const int maxlen = std::max(ch[0][0].nt, ch[0][1].nt);
-  for (int m = 0; m < 2; ++m)
+  // host staging: one block at a time into the ring slot, once the carry that lived there has been copied out
+  auto assemble_slot = [&](int m, int q, int s) -> int {
+    const Chain& k = ch[m][q];
+    if (s >= k.nt) return BTA_OK;
+    BTA_CUDA_OK(cudaStreamWaitEvent(st[m][q], k.ring_ev[s % k.ring], 0));
+    BTA_CUDA_OK(launch_assemble_seq(c, m == 0 ? BTA_COND : BTA_PRIOR, 0, k.tg(s), 1, 1, 0, k.Dp(s), 0, st[m][q]));
+    return BTA_OK;
+  };
+  for (int m = 0; m < 2; ++m) {
+    if (host)
+      BTA_CUDA_OK(launch_assemble_seq(c, m == 0 ? BTA_COND : BTA_PRIOR, 0, h, 1, 1, 0, ch[m][2].D, 0, st[m][0]));
     for (int q = 0; q < 2; ++q) {
-      int rc = assemble_range(m, q, 0, 2);
+      int rc = host ? assemble_slot(m, q, 0) : assemble_range(m, q, 0, 2);
       if (rc != BTA_OK) return rc;
     }
+  }
   for (int s = 0; s < maxlen; ++s)
     for (int m = 0; m < 2; ++m)
       for (int q = 0; q < 2; ++q)
         if (s < ch[m][q].nt) {
-          if (s % AHEAD == 0) {  // blocks s+2 .. s+AHEAD+1 (block s+1 receives this step's Schur update)
+          if (host) {  // block s+1 receives this step's Schur update
+            BTA_CUDA_OK(chain_to_big(ch[m][q], st[m][q]));
+            int rc = assemble_slot(m, q, s + 1);
+            if (rc != BTA_OK) return rc;
+          } else if (s % AHEAD == 0) {  // blocks s+2 .. s+AHEAD+1 (block s+1 receives this step's Schur update)
             BTA_CUDA_OK(chain_to_big(ch[m][q], st[m][q]));
             int rc = assemble_range(m, q, s + 2, s + 2 + AHEAD);
             if (rc != BTA_OK) return rc;
@@ -717,7 +732,14 @@ int enqueue_gradient_twisted(bta_ctx* c, void* ws, cudaStream_t s0, bool timed, 
     }
   // join: everything back onto s0
   for (int m = 0; m < 2; ++m)
-    for (int q = 0; q < 2; ++q) BTA_CUDA_OK(join_lanes(m, q));
+    for (int q = 0; q < 2; ++q) {
+      BTA_CUDA_OK(join_lanes(m, q));
+      if (host) {  // trailing copies of the staging streams
+        cudaEvent_t e = c->ev_sw[(c->ev_sw_next++) % BTA_NSW];
+        BTA_CUDA_OK(cudaEventRecord(e, ch[m][q].cs));
+        BTA_CUDA_OK(cudaStreamWaitEvent(st[m][q], e, 0));
+      }
+    }
   BTA_CUDA_OK(cudaEventRecord(ev[18], st[0][1]));
   BTA_CUDA_OK(cudaStreamWaitEvent(s0, ev[18], 0));
   BTA_CUDA_OK(cudaMemcpyAsync(wc.x + (long long)md.nt * md.b, ch[0][2].xT, md.a * sizeof(double),
@@ -1030,5 +1052,6 @@ extern "C" size_t bta_workspace_bytes(const bta_ctx* c) {
   if (!c) return 0;
   const size_t one = grad_ws_bytes(c->md, c->store_mode);
   const size_t two = c->md.nt >= 3 ? twist_ws_bytes(c->md, c->store_mode) : (size_t)0;
+  if (c->store_mode == BTA_STORE_HOST && use_twist(c)) return two;  // O(b^2): the point of the mode
   return one > two ? one : two;
 }

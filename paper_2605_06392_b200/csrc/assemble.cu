@@ -237,6 +237,9 @@ cudaError_t launch_assemble(bta_ctx* c, int which, double* D, long long d_stride
                             double* rhs_tip, int rhs_tip_stride, cudaStream_t st) {
   const ModelDims& md = c->md;
   const int cond = which == BTA_COND;
+  const double bb8 = 8.0 * md.b * (double)md.b;
+  KTimeScope kt(BTA_KC_ASSEMBLE, st, 0.0,
+                (D ? bb8 * md.nt : 0.0) + (B ? bb8 * (md.nt - 1) : 0.0) + (C ? 8.0 * md.a * (double)md.b * md.nt : 0.0));
   dim3 gx((md.b + 255) / 256, md.b, md.nt);
   if (D) {
     assemble_blocks_kernel<<<gx, 256, 0, st>>>(md, c->P, 0, cond, c->cnt, D, d_stride, 0, 1, 0);
@@ -269,6 +272,7 @@ cudaError_t launch_assemble_seq(bta_ctx* c, int which, int kind, int t0, int tdi
   if (count <= 0) return cudaSuccess;
   const ModelDims& md = c->md;
   dim3 g1((md.b + 255) / 256, md.b, count);
+  KTimeScope kt(BTA_KC_ASSEMBLE, st, 0.0, 8.0 * md.b * (double)md.b * count);
   assemble_blocks_kernel<<<g1, 256, 0, st>>>(md, c->P, kind, which == BTA_COND, c->cnt, out, stride, t0, tdir,
                                              transpose);
   BTA_COUNT(c);

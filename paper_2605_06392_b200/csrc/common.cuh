@@ -51,6 +51,17 @@ cudaError_t optin_smem(K kern, int bytes, unsigned long long* done_bits) {
   return cudaSuccess;
 }
 
+// Per-kernel-class timing (ktime.cu; bta_diag.h: BTA_KC_*): a scope object around each kernel launch.
+extern bool g_ktime_on;
+struct KTimeScope {
+  long long idx;
+  cudaStream_t stream;
+  KTimeScope(int cls, cudaStream_t st, double flop, double bytes);
+  ~KTimeScope();
+  KTimeScope(const KTimeScope&) = delete;
+  KTimeScope& operator=(const KTimeScope&) = delete;
+};
+
 // ------------------------------------------------------------------------------------------------
 // FP64 DMMA GEMM  (gemm.cu):  C = alpha * op(A) op(B) + beta * C, row-major, optionally batched
 // ------------------------------------------------------------------------------------------------
@@ -94,6 +105,8 @@ struct GemmArgs {
   int group;            // tile-order grouping (set by launch_gemm): slow tile rows swept together, <= 1 = off
 };
 
+extern long long g_tile_thresh;
+extern int g_tile_waves;
 cudaError_t launch_gemm(const GemmArgs& g, cudaStream_t st);
 bool gemm_uses_small_tiles(const GemmArgs& g);  // the 64x64-tile configuration (few CTAs)
 
@@ -186,6 +199,11 @@ struct bta_ctx {
   cudaEvent_t ev[32];
   cudaStream_t s_hi[4];              // high-priority companions of the four chains (small kernels)
   cudaStream_t s_x[4];               // side streams of the four chains (off-chain work of the forward steps)
+  double* host_buf;                  // BTA_STORE_HOST: caller-owned page-locked staging memory for the carries
+  size_t host_bytes;
+  cudaStream_t s_copy[4];            // its copy streams (one per sub-chain) and ring-slot events
+  cudaEvent_t ev_ring[4][8];
+  cudaEvent_t ev_pipe[4][3];         // forward pipelining events of the four chains (sweep.h: Chain::pipe_ev)
   cudaEvent_t ev_sw[256];            // lane-switch events, used round-robin
   unsigned ev_sw_next;
   long long launches;

@@ -288,6 +288,8 @@ cudaError_t launch_trace_stencil(bta_ctx* c, int chain, int t, int kind, const d
   SmallLayout L = small_layout(md);
   double* out = c->small + L.trc[chain] + ((size_t)t * 2 + kind) * md.k * md.k * L.nx * 3;
   dim3 grid(L.nx, md.k, md.k);
+  // bytes: the <= 13 gathered entries of every row of every sub-block (payload, not sectors)
+  KTimeScope kt(BTA_KC_CONTRACT, st, 6.0 * 13.0 * md.k * (double)md.b, 8.0 * 13.0 * md.k * (double)md.b);
   trace_stencil_kernel<<<grid, 256, 0, st>>>(md, Z, ld, out);
   BTA_COUNT(c);
   return cudaGetLastError();
@@ -298,6 +300,7 @@ cudaError_t launch_noise_trace(bta_ctx* c, int t, const double* ZD, int ld, cons
   const ModelDims& md = c->md;
   SmallLayout L = small_layout(md);
   dim3 grid(L.nx, md.k);
+  KTimeScope kt(BTA_KC_CONTRACT, st, 2.0 * (1 + md.a) * (double)md.b, 8.0 * 2.0 * (1 + md.a) * (double)md.b);
   noise_trace_kernel<<<grid, 256, 0, st>>>(md, t, ZD, ld, ZC, ldzc, c->cnt, c->zsum, c->small + L.noise);
   BTA_COUNT(c);
   return cudaGetLastError();
@@ -307,6 +310,7 @@ cudaError_t launch_quad_stencil(bta_ctx* c, const double* x, cudaStream_t st) {
   const ModelDims& md = c->md;
   SmallLayout L = small_layout(md);
   dim3 grid(L.nx, md.k * md.k, md.nt * 2);
+  KTimeScope kt(BTA_KC_CONTRACT, st, 2.0 * 7.0 * 13.0 * md.k * (double)md.b * md.nt, 8.0 * 2.0 * md.k * (double)md.N);
   quad_stencil_kernel<<<grid, 256, 0, st>>>(md, x, c->small + L.qd);
   BTA_COUNT(c);
   return cudaGetLastError();
@@ -314,6 +318,7 @@ cudaError_t launch_quad_stencil(bta_ctx* c, const double* x, cudaStream_t st) {
 
 cudaError_t launch_logdet_partial(bta_ctx* c, int chain, const double* dvec, cudaStream_t st) {
   SmallLayout L = small_layout(c->md);
+  KTimeScope kt(BTA_KC_OTHER, st, 0.0, 8.0 * (double)c->md.N);
   logdet_partial_kernel<<<64, 256, 0, st>>>(c->md.N, dvec, c->small + L.ldpart[chain]);
   BTA_COUNT(c);
   return cudaGetLastError();
@@ -321,6 +326,7 @@ cudaError_t launch_logdet_partial(bta_ctx* c, int chain, const double* dvec, cud
 
 cudaError_t launch_residual(bta_ctx* c, const double* x, cudaStream_t st) {
   SmallLayout L = small_layout(c->md);
+  KTimeScope kt(BTA_KC_OTHER, st, 0.0, (double)c->m * (12.0 + 8.0 * c->md.apr + 8.0));
   residual_kernel<<<256, 256, 0, st>>>(c->m, c->md, c->o_var, c->o_node, c->o_time, c->o_cov, c->o_y, x,
                                        c->small + L.rsspart);
   BTA_COUNT(c);
@@ -329,6 +335,7 @@ cudaError_t launch_residual(bta_ctx* c, const double* x, cudaStream_t st) {
 
 cudaError_t launch_scalars(bta_ctx* c, cudaStream_t st) {
   ScalarArgs A{c->md, small_layout(c->md), c->P, c->small, c->ZZ, c->mv};
+  KTimeScope kt(BTA_KC_OTHER, st, 0.0, 0.0);
   scalars_kernel<<<1, 160, 0, st>>>(A);
   BTA_COUNT(c);
   return cudaGetLastError();

@@ -103,12 +103,14 @@ __global__ void tip_inverse_kernel(const double* __restrict__ LT, int a, double*
 
 cudaError_t launch_tip(const double* Tt, int a, int nr, int do_chol, double* LT, double* zT, double* xT, double* ZT,
                        double* diagL, long long grow0, unsigned long long* pivot_flag, cudaStream_t st) {
+  KTimeScope kt(BTA_KC_OTHER, st, 0.0, 0.0);
   tip_kernel<<<1, 32, 0, st>>>(Tt, a, nr, do_chol, LT, zT, xT, ZT, diagL, grow0, pivot_flag);
   return cudaGetLastError();
 }
 
 cudaError_t launch_zero_upper(double* A, int ld, int n, cudaStream_t st) {
   dim3 grid((n + 255) / 256, n);
+  KTimeScope kt(BTA_KC_OTHER, st, 0.0, 4.0 * n * (double)n);
   zero_upper_kernel<<<grid, 256, 0, st>>>(A, ld, n);
   return cudaGetLastError();
 }

@@ -141,7 +141,10 @@ struct Cfg {
   static constexpr int SMEM = (2 + STAGES * (A_ST + B_ST)) * (int)sizeof(double);
 };
 
-template <int BM, int BN, int WM, int WN, bool A_KM, bool B_KM, int MINB, int BK, int STAGES, bool TRACE = false>
+// CLIP: per-warp clipping of the k-range (see below); measured to pay in the 64x64-tile class only (+2 % on triangular
+// products at b = 2304; the 128x128 and 32x32 classes lose 1-2 % to the extra branch), so only that class carries it.
+template <int BM, int BN, int WM, int WN, bool A_KM, bool B_KM, int MINB, int BK, int STAGES, bool TRACE = false,
+          bool CLIP = (BM == 64)>
 __global__ void __launch_bounds__(Cfg<BM, BN, WM, WN, A_KM, B_KM, BK, STAGES>::NT, MINB) gemm_kernel(GemmArgs g) {
   using C_ = Cfg<BM, BN, WM, WN, A_KM, B_KM, BK, STAGES>;
   constexpr int NT = C_::NT;
@@ -216,6 +219,19 @@ __global__ void __launch_bounds__(Cfg<BM, BN, WM, WN, A_KM, B_KM, BK, STAGES>::N
     for (int j = 0; j < WN / 8; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
 
   const int nk = (kend > kbeg) ? (kend - kbeg + BK - 1) / BK : 0;
+  // Per-warp clipping of the k-range: the CTA's range [kbeg, kend) is tile-granular; inside a tile that touches the
+  // diagonal of a triangular operand (or of a lower-only output) a warp's WM x WN sub-tile needs less -- e.g. with
+  // KHI_NEND the columns [n, n + WN) need only k < n + WN.  A warp outside its live k-tiles issues no fragment loads
+  // and no DMMAs (the tensor pipe is the bottleneck: the other warps of the SM sub-partition take the issue slots),
+  // but keeps taking part in the stage barriers.  Saves ~2 % of the DMMAs of a triangular b^3 product.
+  int kw_lo = kbeg, kw_hi = kend;
+  if (g.klo == KLO_N0) kw_lo = max(kw_lo, n0 + wn0);
+  if (g.klo == KLO_M0) kw_lo = max(kw_lo, m0 + wm0);
+  if (g.khi == KHI_NEND) kw_hi = min(kw_hi, n0 + wn0 + WN);
+  if (g.khi == KHI_MEND) kw_hi = min(kw_hi, m0 + wm0 + WM);
+  if (g.out != OUT_FULL && n0 + wn0 > m0 + wm0 + WM - 1) kw_hi = kw_lo;  // sub-tile entirely above the diagonal
+  const int itw_lo = CLIP ? (kw_lo - kbeg) / BK : 0;
+  const int itw_hi = CLIP ? (kw_hi > kw_lo ? (kw_hi - kbeg + BK - 1) / BK : itw_lo) : nk;
 
   // per-thread origins of the fast path (interior tile, aligned operands)
   const bool fast = vecA && vecB && (m0 + BM <= M) && (n0 + BN <= N);
@@ -271,27 +287,32 @@ __global__ void __launch_bounds__(Cfg<BM, BN, WM, WN, A_KM, B_KM, BK, STAGES>::N
   for (int it = 0; it < nk; ++it) {
     const double* as = As + (it % STAGES) * C_::A_ST;
     const double* bs = Bs + (it % STAGES) * C_::B_ST;
+    const bool live = !CLIP || (it >= itw_lo && it < itw_hi);  // warp-uniform
 #pragma unroll
     for (int kk = 0; kk < BK; kk += 4) {
       double af[WM / 8], bf[WN / 8];
+      if (live) {
 #pragma unroll
-      for (int i = 0; i < WM / 8; ++i) {
-        int m = wm0 + i * 8 + gid, k = kk + tig;
-        af[i] = A_KM ? as[k * (BM + KPAD) + m] : as[m * (BK + KPAD) + k];
-      }
+        for (int i = 0; i < WM / 8; ++i) {
+          int m = wm0 + i * 8 + gid, k = kk + tig;
+          af[i] = A_KM ? as[k * (BM + KPAD) + m] : as[m * (BK + KPAD) + k];
+        }
 #pragma unroll
-      for (int j = 0; j < WN / 8; ++j) {
-        int n = wn0 + j * 8 + gid, k = kk + tig;
-        bf[j] = B_KM ? bs[k * (BN + KPAD) + n] : bs[n * (BK + KPAD) + k];
+        for (int j = 0; j < WN / 8; ++j) {
+          int n = wn0 + j * 8 + gid, k = kk + tig;
+          bf[j] = B_KM ? bs[k * (BN + KPAD) + n] : bs[n * (BK + KPAD) + k];
+        }
       }
       if (kk == BK - 4) {
         cp_async_wait<STAGES - 2>();
         mbar_arrive(bar);
       }
+      if (live) {
 #pragma unroll
-      for (int i = 0; i < WM / 8; ++i)
+        for (int i = 0; i < WM / 8; ++i)
 #pragma unroll
-        for (int j = 0; j < WN / 8; ++j) dmma884(acc[i][j][0], acc[i][j][1], af[i], bf[j]);
+          for (int j = 0; j < WN / 8; ++j) dmma884(acc[i][j][0], acc[i][j][1], af[i], bf[j]);
+      }
       if (kk == 0) issue(it + STAGES - 1);
       if (kk == BK - 4) mbar_wait(bar, (unsigned)(it & 1));
     }
@@ -337,6 +358,40 @@ __global__ void __launch_bounds__(Cfg<BM, BN, WM, WN, A_KM, B_KM, BK, STAGES>::N
   }
 }
 
+// Element-exact flop count of one launch: 2 * sum over the written (m, n) of the length of the k-range that element
+// needs (triangular operands: KLO_* / KHI_*; lower-only outputs: m >= n).  Batched launches are not used by the sweeps.
+double gemm_alg_flop(const GemmArgs& g) {
+  double total = 0.0;
+  for (int n = 0; n < g.N; ++n) {
+    // rows m in [mlo, M) are written for this column
+    const int mlo = g.out != OUT_FULL ? n : 0;
+    if (mlo >= g.M) continue;
+    const double rows = g.M - mlo;
+    auto series = [](double first, double last, double cnt) { return cnt > 0 ? 0.5 * (first + last) * cnt : 0.0; };
+    if (g.klo == KLO_M0 && g.khi != KHI_MEND) {          // len(m) = H - m for m < H
+      const int H = g.khi == KHI_NEND ? std::min(g.K, n + 1) : g.K;
+      const int mhi = std::min(g.M, H);
+      if (mhi > mlo) total += series(H - mlo, H - (mhi - 1), mhi - mlo);
+    } else if (g.khi == KHI_MEND && g.klo != KLO_M0) {   // len(m) = min(K, m + 1) - L for m + 1 > L
+      const int L = g.klo == KLO_N0 ? n : 0;
+      const int m0 = std::max(mlo, L);                   // first row with a non-empty range
+      const int msat = std::max(m0, g.K - 1);            // from here on the range is [L, K)
+      if (g.M > m0) {
+        const int mramp = std::min(g.M, msat);
+        if (mramp > m0) total += series(m0 + 1 - L, mramp - L, mramp - m0);
+        if (g.M > msat && g.K > L) total += (double)(g.M - msat) * (g.K - L);
+      }
+    } else if (g.klo == KLO_M0 && g.khi == KHI_MEND) {   // one k per element
+      total += std::max(0, std::min(g.M, g.K) - mlo);
+    } else {
+      const int hi = g.khi == KHI_NEND ? std::min(g.K, n + 1) : g.K;
+      const int lo = g.klo == KLO_N0 ? n : 0;
+      if (hi > lo) total += rows * (hi - lo);
+    }
+  }
+  return 2.0 * total * (g.subs ? g.nsub : 1);
+}
+
 template <int BM, int BN, int WM, int WN, bool A_KM, bool B_KM, int MINB, int BK, int STAGES, bool TRACE>
 cudaError_t launch_cfg(const GemmArgs& g, cudaStream_t st) {
   using C_ = Cfg<BM, BN, WM, WN, A_KM, B_KM, BK, STAGES>;
@@ -351,6 +406,8 @@ cudaError_t launch_cfg(const GemmArgs& g, cudaStream_t st) {
     const int ngroups = ((int)grid.y + ga.group - 1) / ga.group;
     ga.group = ((int)grid.y + ngroups - 1) / ngroups;
   }
+  KTimeScope kt(BM == 128 ? BTA_KC_GEMM_BIG : (BM == 64 ? BTA_KC_GEMM_SMALL : BTA_KC_GEMM_TINY), st,
+                g_ktime_on ? gemm_alg_flop(g) : 0.0, 0.0);
   kern<<<grid, C_::NT, C_::SMEM, st>>>(ga);
   return cudaGetLastError();
 }
@@ -367,6 +424,10 @@ cudaError_t launch_mode(const GemmArgs& g, cudaStream_t st) {
 
 }  // namespace
 
+// Tile-choice parameters (bta_set_option: BTA_OPT_TILE_THRESH / BTA_OPT_TILE_WAVES; process-global)
+long long g_tile_thresh = 180;  // fewer big tiles than this: 64x64 tiles (measured)
+int g_tile_waves = 1;           // 1: also prefer 64x64 tiles where the last wave of big tiles would be mostly empty
+
 // Tile choice: 128x128 (16 warps, 32x32 per warp) once the problem fills the chip with big tiles,
 // else 64x64 (4 warps, 32x32 per warp, three CTAs per SM), and 32x32 for the latency-bound launches.
 namespace {
@@ -375,7 +436,6 @@ long long big_tiles(const GemmArgs& g) {
   if (g.out != OUT_FULL) tiles128 = tiles128 / 2 + 1;
   return tiles128;
 }
-constexpr long long kTileThreshold = 180;  // fewer big tiles than this: 64x64 tiles (measured)
 constexpr long long kTinyThreshold = 148;  // at most this many 64x64 tiles: 32x32 tiles
 }  // namespace
 
@@ -385,7 +445,8 @@ constexpr long long kTinyThreshold = 148;  // at most this many 64x64 tiles: 32x
 // 2.65 waves of 444.
 bool gemm_uses_small_tiles(const GemmArgs& g) {
   const long long t128 = big_tiles(g);
-  if (t128 < kTileThreshold) return true;
+  if (t128 < g_tile_thresh) return true;
+  if (!g_tile_waves) return false;
   const long long nb = g.subs ? g.nsub : 1;
   const long long m64 = (g.M + 63) / 64, n64 = (g.N + 63) / 64;
   const long long t64 = (g.out != OUT_FULL ? std::min(m64, n64) * (std::min(m64, n64) + 1) / 2 : m64 * n64) * nb;
@@ -422,6 +483,11 @@ cudaError_t launch_gemm(const GemmArgs& g0, cudaStream_t st) {
   if (!gemm_uses_small_tiles(g)) return launch_mode<128, 128, 32, 32, 1, 16>(g, st);  // 16 warps, 32x32 per warp
   if (gemm_uses_tiny_tiles(g)) return launch_mode<32, 32, 16, 16, 4, 16>(g, st);
   return launch_mode<64, 64, 32, 32, 3, 16>(g, st);                                  // three CTAs per SM
+}
+
+extern "C" double bta_diag_gemm_flop(int M, int N, int K, int klo, int khi, int out) {
+  GemmArgs g{nullptr, nullptr, nullptr, M, N, K, 0, 0, 0, 1.0, 0.0, GEMM_NN, klo, khi, out, nullptr, 0, 0};
+  return gemm_alg_flop(g);
 }
 
 // Diagnostic: record one {start, end, sm, shape} entry per GEMM CTA into buf[cap][4] (device memory, caller-owned);

@@ -127,12 +127,19 @@ int create_impl(bta_ctx* c, const bta_model_desc* desc, const bta_obs* obs) {
     c->opt.graph = env("BTA_GRAPH", c->opt.graph);
     c->opt.serial = env("BTA_SERIAL_CHAINS", c->opt.serial);
     c->opt.pipeline = env("BTA_PIPELINE", c->opt.pipeline);
+    g_tile_thresh = env("BTA_TILE_THRESH", (int)g_tile_thresh);
+    g_tile_waves = env("BTA_TILE_WAVES", g_tile_waves);
   }
   c->store_mode = BTA_STORE_FACTOR;
   for (auto& e : c->ev) BTA_CUDA_OK(cudaEventCreate(&e));
   for (auto& q : c->s_hi) BTA_CUDA_OK(cudaStreamCreateWithPriority(&q, cudaStreamNonBlocking, prio_hi));
   for (auto& q : c->s_x) BTA_CUDA_OK(cudaStreamCreateWithPriority(&q, cudaStreamNonBlocking, prio_lo));
   for (auto& e : c->ev_sw) BTA_CUDA_OK(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+  for (auto& q : c->s_copy) BTA_CUDA_OK(cudaStreamCreateWithPriority(&q, cudaStreamNonBlocking, prio_lo));
+  for (auto& q : c->ev_ring)
+    for (auto& e : q) BTA_CUDA_OK(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+  for (auto& q : c->ev_pipe)
+    for (auto& e : q) BTA_CUDA_OK(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
   c->ev_sw_next = 0;
   if (m > 0) {
     BTA_CUDA_OK(cudaMemcpy(c->o_var, obs->var, m * sizeof(int), cudaMemcpyHostToDevice));
@@ -181,8 +188,13 @@ extern "C" int bta_destroy(bta_ctx* c) {
   for (auto& q : c->s_aux) kill_stream(q);
   for (auto& q : c->s_hi) kill_stream(q);
   for (auto& q : c->s_x) kill_stream(q);
+  for (auto& q : c->s_copy) kill_stream(q);
+  for (auto& q : c->ev_ring)
+    for (auto& e : q) kill_event(e);
   for (auto& e : c->ev) kill_event(e);
   for (auto& e : c->ev_sw) kill_event(e);
+  for (auto& q : c->ev_pipe)
+    for (auto& e : q) kill_event(e);
   delete c;
   return BTA_OK;
 }
@@ -193,7 +205,7 @@ extern "C" int64_t bta_last_pivot(const bta_ctx* c) { return c ? c->last_pivot :
 extern "C" int64_t bta_kernel_launches(const bta_ctx* c) { return c ? c->launches : 0; }
 
 extern "C" int bta_set_store_mode(bta_ctx* c, int mode) {
-  if (!c || (mode != BTA_STORE_FACTOR && mode != BTA_STORE_CARRY)) {
+  if (!c || (mode != BTA_STORE_FACTOR && mode != BTA_STORE_CARRY && mode != BTA_STORE_HOST)) {
     bta_set_error("bta_set_store_mode: null ctx or unknown mode");
     return BTA_ERR_ARG;
   }
@@ -206,6 +218,25 @@ extern "C" int bta_set_store_mode(bta_ctx* c, int mode) {
   return BTA_OK;
 }
 extern "C" int bta_get_store_mode(const bta_ctx* c) { return c ? c->store_mode : -1; }
+
+extern "C" size_t bta_host_bytes(const bta_ctx* c) {
+  if (!c || c->md.nt < 3) return 0;
+  return (size_t)2 * (size_t)(c->md.nt - 1) * (size_t)c->md.b * (size_t)c->md.b * sizeof(double);
+}
+extern "C" int bta_set_host_buffer(bta_ctx* c, void* host, size_t bytes) {
+  if (!c || (host && bytes < bta_host_bytes(c))) {
+    bta_set_error("bta_set_host_buffer: null ctx, or fewer than bta_host_bytes(ctx) bytes");
+    return BTA_ERR_ARG;
+  }
+  for (int q = 0; q < 2; ++q)
+    if (c->graph_exec[q]) {  // a cached graph holds the old host pointers
+      cudaGraphExecDestroy(c->graph_exec[q]);
+      c->graph_exec[q] = nullptr;
+    }
+  c->host_buf = (double*)host;
+  c->host_bytes = host ? bytes : 0;
+  return BTA_OK;
+}
 
 namespace {
 int* option_slot(bta_ctx* c, int option) {
@@ -222,6 +253,17 @@ int* option_slot(bta_ctx* c, int option) {
 }  // namespace
 
 extern "C" int bta_set_option(bta_ctx* c, int option, int value) {
+  if (option == BTA_OPT_TILE_THRESH || option == BTA_OPT_TILE_WAVES) {  // process-global GEMM tile rule
+    if (option == BTA_OPT_TILE_THRESH) g_tile_thresh = value;
+    else g_tile_waves = value;
+    if (c)
+      for (int q = 0; q < 2; ++q)
+        if (c->graph_exec[q]) {
+          cudaGraphExecDestroy(c->graph_exec[q]);
+          c->graph_exec[q] = nullptr;
+        }
+    return BTA_OK;
+  }
   int* slot = c ? option_slot(c, option) : nullptr;
   if (!slot) {
     bta_set_error("bta_set_option: null ctx or unknown option");

@@ -170,6 +170,7 @@ cudaError_t launch_skinny_nt(int P, int J, int K, const double* R, int ldr, cons
                              double alpha, double beta, const double* in, int ldin, double* out, int ldo,
                              cudaStream_t st) {
   if (P <= 0 || J <= 0) return cudaSuccess;
+  KTimeScope kt(BTA_KC_SKINNY, st, 2.0 * P * (double)J * K * (tri ? 0.5 : 1.0), 8.0 * (double)J * K * (tri ? 0.5 : 1.0));
   dim3 grid((J + 8 * NT_RPW - 1) / (8 * NT_RPW));
   if (P <= 1)
     skinny_nt_kernel<1><<<grid, 256, 0, st>>>(P, J, K, R, ldr, M, ldm, tri, alpha, beta, in, ldin, out, ldo);
@@ -190,6 +191,7 @@ cudaError_t launch_skinny_nn(int P, int K, int J, const double* R, int ldr, cons
                              double alpha, double beta, const double* in, int ldin, double* out, int ldo,
                              double* part, cudaStream_t st) {
   if (P <= 0 || J <= 0) return cudaSuccess;
+  KTimeScope kt(BTA_KC_SKINNY, st, 2.0 * P * (double)J * K * (tri ? 0.5 : 1.0), 8.0 * (double)J * K * (tri ? 0.5 : 1.0));
   const int nks = (K + NN_KCH - 1) / NN_KCH;
   dim3 grid((J + 127) / 128, nks);
   if (P <= 1)
@@ -211,6 +213,7 @@ cudaError_t launch_skinny_nn(int P, int K, int J, const double* R, int ldr, cons
 cudaError_t launch_small_nt(int PU, int PV, int K, const double* U, int ldu, const double* V, int ldv, double alpha,
                             double* Tt, int ldt, cudaStream_t st) {
   if (PU <= 0 || PV <= 0) return cudaSuccess;
+  KTimeScope kt(BTA_KC_OTHER, st, 2.0 * PU * (double)PV * K, 8.0 * (double)(PU + PV) * K);
   small_nt_kernel<<<8, 256, 0, st>>>(PU, PV, K, U, ldu, V, ldv, alpha, Tt, ldt);
   return cudaGetLastError();
 }
@@ -219,6 +222,7 @@ cudaError_t launch_small_left_mul(int R, int Q, int J, const double* S, int lds,
                                   double alpha, double beta, const double* In, int ldin, double* Y, int ldy,
                                   cudaStream_t st) {
   if (R <= 0 || J <= 0) return cudaSuccess;
+  KTimeScope kt(BTA_KC_OTHER, st, 2.0 * R * (double)Q * J, 8.0 * (double)(Q + 2 * R) * J);
   small_left_mul_kernel<<<(J + 255) / 256, 256, 0, st>>>(R, Q, J, S, lds, E, lde, alpha, beta, In, ldin, Y, ldy);
   return cudaGetLastError();
 }

@@ -54,23 +54,30 @@ cudaError_t gemm_lane(Chain* lch, cudaStream_t st, const GemmArgs& g) {
 // A[lo:hi, lo:hi] (lower, SPD) -> X = L^-1 in place; T1, T2: scratch with the same leading dimension.
 // Recursive on 128-wide tiles (leaf: diag.cu):  chol/inv(A11);  L21 = A21 X11^T;  A22 -= L21 L21^T;  chol/inv(A22);
 // X21 = -X22 (L21 X11).  b^3/3 (POTRF) + b^3/3 (TRTRI) flops, all but the 128x128 leaves in DMMA GEMMs.
+constexpr int LEAF = 128;
+int potrf_split(int n) {
+  if (n <= LEAF) return n;
+  const int ntile = (n + LEAF - 1) / LEAF;
+  return LEAF * ((ntile + 1) / 2);
+}
+
 cudaError_t potrf_inv(bta_ctx* c, Chain* lch, double* A, int ld, int lo, int hi, double* T1, double* T2, double* diagL,
-                      long long grow0, cudaStream_t st) {
+                      long long grow0, cudaStream_t st, int phase) {
   const int n = hi - lo;
   if (n <= 0) return cudaSuccess;
-  constexpr int LEAF = 128;
   if (n <= LEAF) {
+    if (phase == 2) return cudaSuccess;
     BTA_COUNT(c);
     return launch_potrf_inv_blocked(A + (long long)lo * ld + lo, ld, n, diagL ? diagL + lo : nullptr, grow0 + lo,
                                  c->pivot_flag, SS);
   }
-  const int ntile = (n + LEAF - 1) / LEAF;
-  const int mid = lo + LEAF * ((ntile + 1) / 2);
+  const int mid = lo + potrf_split(n);
   const int s1 = mid - lo, s2 = hi - mid;
   const bool top = lch && n == ld && c->trace_on;
 #define PM(tag) \
   if (top) trace_mark(c, lane(lch, st, lch->on_small), lch->trace_id, (int)(grow0 / ld), tag)
-  CK(potrf_inv(c, lch, A, ld, lo, mid, T1, T2, diagL, grow0, st));
+  if (phase != 2) CK(potrf_inv(c, lch, A, ld, lo, mid, T1, T2, diagL, grow0, st));
+  if (phase == 1) return cudaSuccess;
   PM(10);
   double* A11 = A + (long long)lo * ld + lo;
   double* A21 = A + (long long)mid * ld + lo;
@@ -101,9 +108,7 @@ cudaError_t potrf_inv_coupled(bta_ctx* c, Chain* lch, double* A, int b, double* 
                               cudaStream_t xs) {
   Chain& ch = *lch;
   const int t = (int)(grow0 / b);
-  const int LEAF = 128;
-  const int ntile = (b + LEAF - 1) / LEAF;
-  const int mid = LEAF * ((ntile + 1) / 2);
+  const int mid = potrf_split(b);
   const int s1 = mid, s2 = b - mid, ld = b;
   auto ev_next = [&]() { return c->ev_sw[(c->ev_sw_next++) % BTA_NSW]; };
   auto cur = [&]() { return lane(lch, st, ch.on_small); };
@@ -193,9 +198,23 @@ cudaError_t chain_forward_step(Chain& ch, int t, cudaStream_t st) {
   const int b = ch.b, nt = ch.nt, a = ch.a, P = ch.P(), ldt = a + ch.nr;
   const long long bb = (long long)b * b;
   const long long tg = ch.tg(t);                  // global time block (diag(L) position, pivot row)
-  double* At = ch.D + t * ch.d_stride;           // D_t - S_{t-1}
+  double* At = ch.Dp(t);           // D_t - S_{t-1}
   double* Dt = ch.carry ? ch.Xs : At;            // where X_t = L_Dt^-1 is built
   const double* LBprev = ch.carry ? ch.LBs : (t > 0 ? ch.Bout + (t - 1) * ch.b_stride : nullptr);
+  // Forward pipelining: when the previous step issued its products in split form (see the end of this function), the
+  // first half of this block's POTRF+TRTRI (A11 = the top-left part of D_t - S_{t-1}) depends only on the first two of
+  // those five launches.  It starts now on the chain's priority lane, next to the rest of the previous step's products
+  // on the main lane -- the chain offers the GPU latency-bound and chip-filling work at the same time.
+  constexpr int split_maxb = 1024;  // the coupled step (below) pays only where a step is latency-bound
+  const bool can_pipe = ch.pipe_ev && ch.hi && c->opt.pipeline && ch.factor_blocks && !ch.carry && !ch.zero_upper &&
+                        b > split_maxb;
+  bool early = false;
+  if (can_pipe && ch.pipe_armed) {
+    ch.on_small = true;  // enter the priority lane WITHOUT ordering it after the tail of the main lane ...
+    CK(cudaStreamWaitEvent(ch.hi, ch.pipe_ev[0], 0));  // ... only after the Schur update of A11
+    CK(potrf_inv(c, lch, At, b, 0, b, ch.W2, ch.W3, ch.dvec ? ch.dvec + tg * b : nullptr, tg * b, st, 1));
+    early = true;
+  }
   // stack rows: arrow rows (factor mode) then right-hand-side rows.
   //   R~_t = R_t - R^_{t-1} L_B{t-1}^T  (lines 4-5), done first: in carry mode L_B{t-1} is overwritten below
   const double* src = nullptr;
@@ -210,6 +229,7 @@ cudaError_t chain_forward_step(Chain& ch, int t, cudaStream_t st) {
       ld_src = b;
     }
     if (t > 0) {
+      if (early) CK(cudaStreamWaitEvent(SS, ch.pipe_ev[1], 0));  // L_B{t-1} is complete
       double* tmp = ch.Rtmp ? ch.Rtmp : ch.Rin + t * ch.rin_stride;
       const int ld_tmp = ch.Rtmp ? b : ch.ld_rin;
       CK(launch_skinny_nt(P, b, b, ch.Rout + (t - 1) * ch.rout_stride, ch.ld_rout, LBprev, b, 0, -1.0, 1.0, src, ld_src,
@@ -219,6 +239,9 @@ cudaError_t chain_forward_step(Chain& ch, int t, cudaStream_t st) {
       ld_src = ld_tmp;
     }
   }
+  if (early)  // everything else of this step comes after all products of the previous step
+    CK(cudaStreamWaitEvent(lane(lch, st, ch.on_small), ch.pipe_ev[2], 0));
+  ch.pipe_armed = false;
 #define TM(tag) trace_mark(c, lane(lch, st, ch.on_small), ch.trace_id, t, tag)
   TM(0);
   bool coupled = false;  // L_B and the Schur update were folded into the recursion (potrf_inv_coupled)
@@ -229,20 +252,26 @@ cudaError_t chain_forward_step(Chain& ch, int t, cudaStream_t st) {
     }
     if (ch.carry) {  // the carry D_t - S_{t-1} stays in its slot; factor a copy
       CK(cudaMemcpyAsync(Dt, At, bb * sizeof(double), cudaMemcpyDeviceToDevice, SB));
+      if (ch.ring) {  // host staging: the carry is final (S_{t-1} was applied in main-lane order) -- copy it out
+        cudaEvent_t e = c->ev_sw[(c->ev_sw_next++) % BTA_NSW];
+        CK(cudaEventRecord(e, SB));
+        CK(cudaStreamWaitEvent(ch.cs, e, 0));
+        CK(cudaMemcpyAsync(ch.hostD + (long long)t * bb, At, bb * sizeof(double), cudaMemcpyDeviceToHost, ch.cs));
+        CK(cudaEventRecord(ch.ring_ev[t % ch.ring], ch.cs));
+      }
       CK(potrf_inv(c, lch, Dt, b, 0, b, ch.W1, ch.Bs, ch.dvec ? ch.dvec + tg * b : nullptr, tg * b, st));
     } else {
-      constexpr int split_maxb = 1024;  // the coupled step pays only where a step is latency-bound
       const bool has_coupling = t < nt - 1 || ch.tail_coupling;
       coupled = has_coupling && ch.xs && b > 128 && b <= split_maxb;
       if (coupled) {
         double* Bi = ch.Bin + t * ch.b_stride;
         double* Bo = ch.Bout + t * ch.b_stride;
         double* dst = (Bi == Bo) ? ch.W1 : Bo;
-        CK(potrf_inv_coupled(c, lch, Dt, b, Bi, dst, t < nt - 1 ? ch.D + (t + 1) * ch.d_stride : nullptr, ch.W2, ch.W3,
+        CK(potrf_inv_coupled(c, lch, Dt, b, Bi, dst, t < nt - 1 ? ch.Dp(t + 1) : nullptr, ch.W2, ch.W3,
                              ch.dvec ? ch.dvec + tg * b : nullptr, tg * b, st, ch.xs));
         if (dst != Bo) CK(cudaMemcpyAsync(Bo, dst, bb * sizeof(double), cudaMemcpyDeviceToDevice, SB));
       } else {
-        CK(potrf_inv(c, lch, Dt, b, 0, b, ch.W2, ch.W3, ch.dvec ? ch.dvec + tg * b : nullptr, tg * b, st));
+        CK(potrf_inv(c, lch, Dt, b, 0, b, ch.W2, ch.W3, ch.dvec ? ch.dvec + tg * b : nullptr, tg * b, st, early ? 2 : 0));
       }
     }
   }
@@ -276,17 +305,56 @@ cudaError_t chain_forward_step(Chain& ch, int t, cudaStream_t st) {
       dst = (Bi == Bo) ? ch.W1 : Bo;
     }
     TM(2);
-    CK(launch_gemm(G(GEMM_NT, b, b, b, 1.0, Bi, b, Dt, b, 0.0, dst, b, KLO_ZERO, KHI_NEND, OUT_FULL), SB));
-    BTA_COUNT(c);
-    TM(3);
-    if (t < nt - 1) {  // the Schur update of a separator is applied by the separator stage (two chains meet there)
-      CK(launch_gemm(G(GEMM_NT, b, b, b, -1.0, dst, b, dst, b, 1.0, ch.D + (t + 1) * ch.d_stride, b, KLO_ZERO, KHI_K,
+    if (can_pipe && t < nt - 1) {
+      // Split form: rows [0, h) of L_B and the top-left h x h part of the Schur update first (h = the next block's
+      // A11), then the rest.  Same flops.
+      double* Dn = ch.Dp(t + 1);
+      const int h = potrf_split(b), r = b - h;
+      const long long ho = (long long)h * b;
+      CK(launch_gemm(G(GEMM_NT, h, b, b, 1.0, Bi, b, Dt, b, 0.0, dst, b, KLO_ZERO, KHI_NEND, OUT_FULL), SB));
+      CK(launch_gemm(G(GEMM_NT, h, h, b, -1.0, dst, b, dst, b, 1.0, Dn, b, KLO_ZERO, KHI_K, OUT_LOWER), SB));
+      CK(cudaEventRecord(ch.pipe_ev[0], SB));
+      CK(launch_gemm(G(GEMM_NT, r, b, b, 1.0, Bi + ho, b, Dt, b, 0.0, dst + ho, b, KLO_ZERO, KHI_NEND, OUT_FULL), SB));
+      CK(cudaEventRecord(ch.pipe_ev[1], SB));
+      TM(3);
+      CK(launch_gemm(G(GEMM_NT, r, h, b, -1.0, dst + ho, b, dst, b, 1.0, Dn + ho, b, KLO_ZERO, KHI_K, OUT_FULL), SB));
+      CK(launch_gemm(G(GEMM_NT, r, r, b, -1.0, dst + ho, b, dst + ho, b, 1.0, Dn + ho + h, b, KLO_ZERO, KHI_K,
                        OUT_LOWER),
                      SB));
+      c->launches += 5;
+      if (dst != Bo) CK(cudaMemcpyAsync(Bo, dst, bb * sizeof(double), cudaMemcpyDeviceToDevice, SB));
+      CK(cudaEventRecord(ch.pipe_ev[2], SB));
+      ch.pipe_armed = true;
+    } else {
+      CK(launch_gemm(G(GEMM_NT, b, b, b, 1.0, Bi, b, Dt, b, 0.0, dst, b, KLO_ZERO, KHI_NEND, OUT_FULL), SB));
+      BTA_COUNT(c);
+      TM(3);
+      if (t < nt - 1) {  // the Schur update of a separator is applied by the separator stage (two chains meet there)
+        CK(launch_gemm(G(GEMM_NT, b, b, b, -1.0, dst, b, dst, b, 1.0, ch.Dp(t + 1), b, KLO_ZERO, KHI_K,
+                         OUT_LOWER),
+                       SB));
+        BTA_COUNT(c);
+      }
+      if (dst != Bo) CK(cudaMemcpyAsync(Bo, dst, bb * sizeof(double), cudaMemcpyDeviceToDevice, SB));
+    }
+    TM(4);
+  }
+  if (ch.fill) {  // middle partition: the fill coupling to the top boundary block (sweep.h: Fill)
+    Fill& f = *ch.fill;
+    double* LF = f.LF + t * f.lf_stride;
+    const double* LB = ch.Bout + t * ch.b_stride;
+    CK(launch_gemm(G(GEMM_NT, b, b, b, 1.0, f.Ftil, b, Dt, b, 0.0, LF, b, KLO_ZERO, KHI_NEND, OUT_FULL), SB));
+    CK(launch_gemm(G(GEMM_NT, b, b, b, -1.0, LF, b, LF, b, 1.0, f.Ds, b, KLO_ZERO, KHI_K, OUT_LOWER), SB));
+    if (t < nt - 1)
+      CK(launch_gemm(G(GEMM_NT, b, b, b, -1.0, LF, b, LB, b, 0.0, f.Ftil, b, KLO_ZERO, KHI_K, OUT_FULL), SB));
+    else
+      CK(launch_gemm(G(GEMM_NT, b, b, b, -1.0, LB, b, LF, b, 0.0, f.Bse, b, KLO_ZERO, KHI_K, OUT_FULL), SB));
+    c->launches += 3;
+    if (P > 0) {
+      CK(launch_skinny_nt(P, b, b, ch.Rout + t * ch.rout_stride, ch.ld_rout, LF, b, 0, -1.0, 1.0, f.Rs, f.ld_rs, f.Rs,
+                          f.ld_rs, SS));
       BTA_COUNT(c);
     }
-    if (dst != Bo) CK(cudaMemcpyAsync(Bo, dst, bb * sizeof(double), cudaMemcpyDeviceToDevice, SB));
-    TM(4);
   }
   return cudaSuccess;
 }
@@ -350,7 +418,16 @@ cudaError_t chain_backward_step(Chain& ch, int t, cudaStream_t st) {
   {
     if (ch.carry) {
       // carry-based reconstruction: X_t from the stored D_t - S_{t-1}, L_Bt from the re-assembled B_t
-      CK(cudaMemcpyAsync(ch.Xs, ch.D + t * ch.d_stride, bb * sizeof(double), cudaMemcpyDeviceToDevice, SB));
+      if (ch.ring) CK(cudaStreamWaitEvent(SB, ch.ring_ev[t % ch.ring], 0));  // the carry is back in its slot
+      CK(cudaMemcpyAsync(ch.Xs, ch.Dp(t), bb * sizeof(double), cudaMemcpyDeviceToDevice, SB));
+      if (ch.ring && t - ch.ring >= 0) {  // the slot is free: stream block t - ring back from the host
+        cudaEvent_t e = c->ev_sw[(c->ev_sw_next++) % BTA_NSW];
+        CK(cudaEventRecord(e, SB));
+        CK(cudaStreamWaitEvent(ch.cs, e, 0));
+        CK(cudaMemcpyAsync(ch.Dp(t), ch.hostD + (long long)(t - ch.ring) * bb, bb * sizeof(double),
+                           cudaMemcpyHostToDevice, ch.cs));
+        CK(cudaEventRecord(ch.ring_ev[t % ch.ring], ch.cs));
+      }
       CK(potrf_inv(c, lch, ch.Xs, b, 0, b, ch.W1, ch.Bs, nullptr, (long long)ch.tg(t) * b, st));
       if (has_next) {
         CK(launch_assemble_block(c, ch.which, 1, ch.tB(t), ch.transposeB ? 1 : 0, ch.Bs, SB));
@@ -358,7 +435,7 @@ cudaError_t chain_backward_step(Chain& ch, int t, cudaStream_t st) {
         BTA_COUNT(c);
       }
     }
-    const double* X = ch.carry ? ch.Xs : ch.D + t * ch.d_stride;
+    const double* X = ch.carry ? ch.Xs : ch.Dp(t);
     double* LB = has_next ? (ch.carry ? ch.LBs : ch.Bout + t * ch.b_stride) : nullptr;
     const double* LC = nullptr;
     int ld_lc = b;
@@ -387,6 +464,13 @@ cudaError_t chain_backward_step(Chain& ch, int t, cudaStream_t st) {
         u = ch.ubuf;
         ld_u = b;
       }
+      if (ch.fill) {  // - L_Ft^T x_s
+        CK(launch_skinny_nn(nr, b, b, ch.fill->xs, (int)ch.fill->ld_xs, ch.fill->LF + t * ch.fill->lf_stride, b, 0, -1.0,
+                            1.0, u, ld_u, ch.ubuf, b, ch.part, SS));
+        c->launches += 2;
+        u = ch.ubuf;
+        ld_u = b;
+      }
       CK(launch_skinny_nn(nr, b, b, u, ld_u, X, b, 1, 1.0, 0.0, nullptr, 0, ch.xout + tg * b, (int)ch.ld_x,
                           ch.part, SS));
       c->launches += 2;
@@ -402,6 +486,16 @@ cudaError_t chain_backward_step(Chain& ch, int t, cudaStream_t st) {
       CK(launch_skinny_nn(a, b, b, LC, ld_lc, X, b, 1, 1.0, 0.0, nullptr, 0, ch.Ebuf, b, ch.part, SS));  // E
       CK(launch_small_left_mul(a, a, b, ch.ZT, a, ch.Ebuf, b, 1.0, 0.0, nullptr, 0, ch.Ybuf, b, SS));   // Z_T E
       c->launches += 3;
+    }
+    Fill* fl = ch.fill;
+    double* LFt = fl ? fl->LF + t * fl->lf_stride : nullptr;
+    if (fl) {  // H = L_F X;  the arrow term Z_T E gains Sigma[T,s] H
+      CK(launch_gemm(G(GEMM_NN, b, b, b, 1.0, LFt, b, X, b, 0.0, fl->H, b, KLO_N0, KHI_K, OUT_FULL), SB));
+      BTA_COUNT(c);
+      if (arrow) {
+        CK(launch_skinny_nn(a, b, b, fl->ZCs, b, fl->H, b, 0, 1.0, 1.0, ch.Ybuf, b, ch.Ybuf, b, ch.part, SS));
+        c->launches += 2;
+      }
     }
     if (has_next) {
       double* Gm = ch.W1;
@@ -419,6 +513,24 @@ cudaError_t chain_backward_step(Chain& ch, int t, cudaStream_t st) {
         BTA_COUNT(c);
       }
       CK(launch_gemm(G(GEMM_TN, b, b, b, 1.0, X, b, X, b, 0.0, ZDcur, b, KLO_M0, KHI_K, OUT_LOWER), SB));
+      if (fl) {
+        // Sigma[s, t+1] is Z_F of the block below (stored [s][t+1]); below the last interior block it is the reduced
+        // system's Sigma[e, s], stored the other way round
+        const bool last = t == nt - 1;
+        const double* ZFn = last ? fl->ZFe : fl->LF + (t + 1) * fl->lf_stride;
+        //   Z_B -= Sigma[t+1, s] H
+        CK(launch_gemm(G(last ? GEMM_NN : GEMM_TN, b, b, b, -1.0, ZFn, b, fl->H, b, 1.0, ZB, b, KLO_ZERO, KHI_K, OUT_FULL),
+                       SB));
+        //   Z_F = -(Sigma[s, t+1] G + Sigma[s,s] H + Sigma[T,s]^T E), into the slot of L_F (dead since H)
+        CK(launch_gemm(G(last ? GEMM_TN : GEMM_NN, b, b, b, -1.0, ZFn, b, Gm, b, 0.0, LFt, b, KLO_ZERO, KHI_K, OUT_FULL),
+                       SB));
+        CK(launch_gemm(G(GEMM_NN, b, b, b, -1.0, fl->ZDs, b, fl->H, b, 1.0, LFt, b, KLO_ZERO, KHI_K, OUT_FULL), SB));
+        if (arrow)
+          CK(launch_gemm(G(GEMM_TN, b, b, a, -1.0, fl->ZCs, b, ch.Ebuf, b, 1.0, LFt, b, KLO_ZERO, KHI_K, OUT_FULL), SB));
+        //   Z_D -= Z_F^T H
+        CK(launch_gemm(G(GEMM_TN, b, b, b, -1.0, LFt, b, fl->H, b, 1.0, ZDcur, b, KLO_ZERO, KHI_K, OUT_LOWER), SB));
+        c->launches += arrow ? 5 : 4;
+      }
       CK(launch_gemm(G(GEMM_TN, b, b, b, -1.0, ZB, b, Gm, b, 1.0, ZDcur, b, KLO_ZERO, KHI_K,
                        arrow ? OUT_LOWER : OUT_LOWER_MIRROR),
                      SB));
@@ -441,11 +553,12 @@ cudaError_t chain_backward_step(Chain& ch, int t, cudaStream_t st) {
     }
     if (ch.contract) {
       CK(launch_trace_stencil(c, ch.chain, (int)tg, 0, ZDcur, b, SS));
-      if (has_next) CK(launch_trace_stencil(c, ch.chain, ch.tB(t), 1, LB, b, SS));
+      if (has_next && ch.tB(t) >= 0) CK(launch_trace_stencil(c, ch.chain, ch.tB(t), 1, LB, b, SS));
+      if (fl && t == 0 && fl->tb_first >= 0) CK(launch_trace_stencil(c, ch.chain, fl->tb_first, 1, LFt, b, SS));
       if (arrow) CK(launch_noise_trace(c, (int)tg, ZDcur, b, ZCcur, b, SS));
     }
     if (ch.selinv_inplace) {
-      CK(cudaMemcpyAsync(ch.D + t * ch.d_stride, ZDcur, bb * sizeof(double), cudaMemcpyDeviceToDevice, SB));
+      CK(cudaMemcpyAsync(ch.Dp(t), ZDcur, bb * sizeof(double), cudaMemcpyDeviceToDevice, SB));
       if (arrow && ch.Cout)
         CK(cudaMemcpyAsync(ch.Cout + t * ch.cout_stride, ZCcur, (size_t)a * b * sizeof(double),
                            cudaMemcpyDeviceToDevice, SB));

@@ -2,6 +2,27 @@
 #pragma once
 #include "common.cuh"
 
+// Middle partition of the time-domain partitioning (§III-C a): the interior
+// blocks t = s+1 .. e-1 of a partition [s, e] are eliminated downwards BEFORE its two boundary blocks, so every interior
+// block carries a fill coupling F~_t = Q~[s, t] to the top boundary s next to its coupling B_t to block t+1:
+//   forward :  L_Ft = F~_t X_t^T,   D~_s -= L_Ft L_Ft^T,   [C~_s; r~_s] -= [L_Ct; z_t] L_Ft^T,   F~_{t+1} = -L_Ft L_Bt^T
+//              (after the last interior block: Q~[e, s] = -L_Bt L_Ft^T goes to the reduced system)
+//   backward:  H = L_Ft X_t,   Z_Bt -= Z_F{t+1}^T H,   Z_Ft = Sigma[s,t] = -(Z_F{t+1} G + Sigma[s,s] H + Sigma[T,s]^T E),
+//              Z_Ct -= Sigma[T,s] H,   Z_Dt -= Z_Ft^T H,   x_t -= X_t^T L_Ft^T x_s.
+struct Fill {
+  double* LF = nullptr; long long lf_stride = 0;   // L_F(t), later Z_F(t), per interior block (local index)
+  double* Ftil = nullptr;                          // scratch: F~_t of the current step (starts as B_s^T)
+  double* H = nullptr;                             // scratch: H = L_F X (backward)
+  double* Ds = nullptr;                            // forward: the top boundary block D~_s (reduced system)
+  double* Rs = nullptr; int ld_rs = 0;             // forward: its stack rows [C~_s; r~_s]
+  double* Bse = nullptr;                           // forward: where Q~[e, s] goes (reduced sub-diagonal block)
+  const double* ZDs = nullptr;                     // backward: Sigma[s,s] (both triangles)
+  const double* ZCs = nullptr;                     // backward: Sigma[T,s]  (a x b)
+  const double* xs = nullptr; long long ld_xs = 0; // backward: x_s rows
+  const double* ZFe = nullptr;                     // backward: Sigma[e,s] (stored [e][s]) for the last interior block
+  int tb_first = -1;                               // global index of the pattern block B_s (trace of Z_F at t = s+1)
+};
+
 struct Chain {
   bta_ctx* c = nullptr;
   int chain = CH_COND;         // slot of the partial-sum buffers (CH_PRIOR / CH_COND)
@@ -31,8 +52,30 @@ struct Chain {
   bool lanes_bwd = true;       // use the small lane in the backward sweep too
   int trace_id = -1;           // BTA_TRACE label of this chain
   cudaStream_t xs = nullptr;   // optional side stream: work of a forward step that is off its dependent chain
-  int tg(int s) const { return t0 + tdir * s; }
-  int tB(int s) const { return tdir > 0 ? tg(s) : tg(s) - 1; }   // index of the sub-diagonal block between s, s+1
+  // Forward pipelining (sweep.cu: chain_forward_step): three events of this chain -- [0] the top-left part of the next
+  // diagonal block has its Schur update, [1] L_B of this step is complete, [2] all products of this step are done.
+  cudaEvent_t* pipe_ev = nullptr;
+  bool pipe_armed = false;     // the previous step recorded pipe_ev (its products were issued in split form)
+  // Host-staged carries (BTA_STORE_HOST): the diagonal-block slots are a ring of `ring` device blocks
+  // (local block s lives in slot s % ring); each carry D_s - S_{s-1} is copied to pinned host memory (hostD + s b^2) on
+  // the copy stream `cs` during the forward sweep and streamed back `ring` steps ahead in the backward sweep.
+  // ring_ev[slot]: the last copy from / into that slot has finished.
+  int ring = 0;
+  double* hostD = nullptr;
+  cudaStream_t cs = nullptr;
+  cudaEvent_t* ring_ev = nullptr;
+  double* Dp(int s) const {
+    return dmap ? dmap[s] : (ring ? D + (long long)(s % ring) * b * b : D + s * d_stride);
+  }
+  // Reduced system of the partitioning: the local blocks are the boundary blocks of the partitions -- their global time
+  // index, the global index of the pattern block between local s and s+1 (-1: a fill block, no trace), and their
+  // device pointers come from host tables.
+  const int* tmap = nullptr;
+  const int* bmap = nullptr;
+  double* const* dmap = nullptr;
+  Fill* fill = nullptr;        // this chain is the interior of a middle partition
+  int tg(int s) const { return tmap ? tmap[s] : t0 + tdir * s; }
+  int tB(int s) const { return bmap ? bmap[s] : (tdir > 0 ? tg(s) : tg(s) - 1); }   // sub-diagonal block between s, s+1
 
   int P() const { return (arrow_rows ? a : 0) + nr; }
   bool arrow() const { return arrow_rows || arrow_given; }
@@ -59,8 +102,10 @@ struct Chain {
   double* Cout = nullptr; long long cout_stride = 0;                    // selinv_inplace: Z_Ct destination
 };
 
+// phase 0: the whole POTRF + TRTRI; 1: only the first half of the top level (A11); 2: everything but that half
 cudaError_t potrf_inv(bta_ctx* c, Chain* lanes, double* A, int ld, int lo, int hi, double* T1, double* T2,
-                      double* diagL, long long grow0, cudaStream_t st);
+                      double* diagL, long long grow0, cudaStream_t st, int phase = 0);
+int potrf_split(int n);  // size of the first half of the top level of potrf_inv on an n x n block
 cudaError_t chain_to_big(Chain& ch, cudaStream_t big);  // join the small lane back into the chain's main stream
 cudaError_t chain_forward(Chain& ch, cudaStream_t st);
 cudaError_t chain_forward_begin(Chain& ch, cudaStream_t st);

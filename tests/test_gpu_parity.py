@@ -377,3 +377,47 @@ def test_second_device_ordinal():
         assert torch.cuda.current_device() == 0
         M.close()
         assert abs(f - ref["f"]) <= TOL_F * abs(ref["f"]) and grad_ok(g, ref["grad"])
+
+
+@pytest.mark.parametrize("name", ["nt3_twist_min", "nt4_twist", "b81_two_tiles", "mv_k2_a8", "mv_k3_b300", "cfg1"])
+def test_host_staged_carries(name):
+    """SURVEY.md §8(f) NEXT-4 / PAPER.md:185 (§III-C c): the carries are written to pinned host memory in the forward
+    sweep and streamed back in the backward sweep; the device keeps a ring of 4 diagonal-block slots per sub-chain.
+    Same f, grad as carry mode; device workspace independent of nt."""
+    model, obs, th = CASES[name]()
+    ref = O.value_and_grad(model, obs, th)
+    M = _model(model, obs)
+    M.bta_set_store_mode(1)
+    ws_carry = M.workspace_bytes()
+    f1, g1 = M.inla_value_and_grad(th)
+    M.bta_set_store_mode(2)
+    assert M.bta_get_store_mode() == 2
+    assert M.bta_host_bytes() == 2 * (model.nt - 1) * model.b * model.b * 8
+    ws_host = M.workspace_bytes()
+    f2, g2 = M.inla_value_and_grad(th)
+    f3, g3 = M.inla_value_and_grad(th)          # again (graph replay for small b; ring events reused)
+    im = M.last_intermediates()
+    M.close()
+    assert f2 == f3 and np.array_equal(g2, g3)
+    assert abs(f2 - f1) <= 1e-12 * abs(f1) and np.max(np.abs(g2 - g1)) <= 1e-12 * np.max(np.abs(g1))
+    assert abs(f2 - ref["f"]) <= TOL_F * abs(ref["f"]) and grad_ok(g2, ref["grad"])
+    assert np.max(np.abs(im["x"] - ref["x"])) <= 1e-9 * np.max(np.abs(ref["x"]))
+    if model.nt >= 12:
+        assert ws_host < ws_carry
+
+
+def test_host_staged_workspace_is_independent_of_nt():
+    """Device workspace O(b^2): growing nt from 8 to 64 adds less than two b x b blocks (the O(nt a b)
+    row stacks) in host mode, against 2 x 56 blocks in carry mode."""
+    from paper_2605_06392_b200 import BtaModel
+    ws = {}
+    for nt in (8, 64):
+        model = make_model(20, 1, nt, 2)
+        M = BtaModel.from_workload(model, draw_obs(model, 10, 1), device=0)
+        for mode in (1, 2):
+            M.bta_set_store_mode(mode)
+            ws[mode, nt] = M.workspace_bytes()
+        M.close()
+    block = 400 * 400 * 8
+    assert ws[2, 64] - ws[2, 8] < 2 * block, ws
+    assert ws[1, 64] - ws[1, 8] > 100 * block, ws

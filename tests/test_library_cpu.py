@@ -80,3 +80,21 @@ def test_product_never_imports_the_oracle():
         if f.endswith(".py"):
             assert "paper_2605_06392_b200" not in open(os.path.join(ROOT, "oracle", f)).read().replace(
                 "`paper_2605_06392_b200/`", "")
+
+
+def test_gemm_flop_count_matches_brute_force(lib):
+    """Host logic behind bench.py's in-step TFLOP/s: the element-exact flop count of a GEMM launch with a restricted
+    k-range (KLO_*/KHI_* of csrc/common.cuh) and a lower-only output, against a triple loop."""
+    import itertools
+    from paper_2605_06392_b200.binding import gemm_alg_flop
+    for (M, N, K) in [(7, 7, 7), (5, 9, 6), (9, 5, 12), (1, 1, 1), (13, 13, 4)]:
+        for klo, khi, out in itertools.product((0, 1, 2), (0, 1, 2), (0, 1, 2)):
+            want = 0
+            for m in range(M):
+                for n in range(N):
+                    if out != 0 and n > m:
+                        continue
+                    lo = {0: 0, 1: n, 2: m}[klo]
+                    hi = {0: K, 1: min(K, n + 1), 2: min(K, m + 1)}[khi]
+                    want += 2 * max(0, hi - lo)
+            assert gemm_alg_flop(M, N, K, klo, khi, out) == want, (M, N, K, klo, khi, out)
