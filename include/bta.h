@@ -169,6 +169,16 @@ BTA_API int inla_hessian(bta_ctx* ctx, const double* theta, double h, double* f,
 BTA_API int inla_optimize(bta_ctx* ctx, const double* theta0, int max_iter, double gtol, double* theta_opt, double* f_opt,
                   double* grad_opt, int* iters, int* evals, void* ws, void* stream);
 
+/* Time-domain partitioning (§III-C a-b).  The nt time blocks are cut into P
+ * contiguous partitions; partition 0 ends at one boundary block, every other partition has two; the interior blocks of
+ * all partitions are eliminated concurrently (a partition p >= 1 carries a fill coupling to its top boundary), the
+ * 2P-1 boundary blocks form a reduced BTA system that is factored and selectively inverted, and the interiors are
+ * swept backwards concurrently, seeded by the reduced system's Sigma blocks.  Inside one GPU it is selected with
+ * bta_set_option(ctx, BTA_OPT_PARTITIONS, P) (include/bta_diag.h) and inla_value_and_grad runs it whole.
+ * bta_partition_plan returns the number of partitions actually used for a request of `partitions` (>= 2, <= 8,
+ * clipped so that nt >= 2P-1) and their first / last time blocks (HOST arrays of >= 8 entries, may be NULL). */
+BTA_API int bta_partition_plan(const bta_ctx* ctx, int partitions, int32_t* first, int32_t* last);
+
 enum {
   BTA_STAGE_ASSEMBLE = 0,
   BTA_STAGE_FWD_QC = 1,

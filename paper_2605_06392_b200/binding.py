@@ -86,6 +86,7 @@ def lib():
     L.bta_diag_gemm_flop.restype = C.c_double
     L.bta_diag_ktime_begin.argtypes = []
     L.bta_diag_ktime_end.argtypes = [dp, dp, dp, C.POINTER(C.c_int64)]
+    L.bta_partition_plan.argtypes = [vp, i32, C.POINTER(C.c_int32), C.POINTER(C.c_int32)]
     L.bta_set_option.argtypes = [vp, i32, i32]
     L.bta_get_option.argtypes = [vp, i32]
     _lib = L
@@ -126,7 +127,7 @@ class Blocks:
 
 BTA_PRIOR, BTA_COND = 0, 1
 BTA_STORE_FACTOR, BTA_STORE_CARRY, BTA_STORE_HOST = 0, 1, 2
-OPT_TWIST, OPT_LANES, OPT_SPLIT, OPT_GRAPH, OPT_SERIAL, OPT_PIPELINE = range(6)
+OPT_TWIST, OPT_LANES, OPT_SPLIT, OPT_GRAPH, OPT_SERIAL, OPT_PIPELINE, OPT_TILE_THRESH, OPT_TILE_WAVES, OPT_PARTITIONS = range(9)
 STAGES = ("assemble", "fwd_Qc", "bwd_Qc", "fwd_Qp", "bwd_Qp", "scalars", "total")
 
 
@@ -309,6 +310,19 @@ class BtaModel:
 
     def bta_get_option(self, option):
         return lib().bta_get_option(self._h, int(option))
+
+    def bta_set_partitions(self, P):
+        """P >= 2: time-domain partitioning with P partitions inside the GPU (0: two-way elimination).  Re-sizes the
+        workspace."""
+        self.bta_set_option(OPT_PARTITIONS, P)
+        self._ws = None
+
+    def bta_partition_plan(self, P):
+        """-> [(first, last)] time blocks of the partitions a request for P partitions yields."""
+        first = (C.c_int32 * 8)()
+        last = (C.c_int32 * 8)()
+        n = lib().bta_partition_plan(self._h, int(P), first, last)
+        return [(first[i], last[i]) for i in range(n)]
 
     def kernel_launches(self):
         return lib().bta_kernel_launches(self._h)

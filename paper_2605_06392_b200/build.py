@@ -13,7 +13,7 @@ CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libbta_b200.so")
 INCLUDE = os.path.join(HERE, "..", "include")
-SOURCES = ["gemm.cu", "diag.cu", "leaf.cu", "skinny.cu", "assemble.cu", "contract.cu", "sweep.cu", "ktime.cu",
+SOURCES = ["gemm.cu", "diag.cu", "leaf.cu", "skinny.cu", "assemble.cu", "contract.cu", "sweep.cu", "partition.cu", "ktime.cu",
            "model.cu", "api.cu", "api_misc.cu", "peak.cu"]
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
          "-Xcompiler", "-fPIC,-fvisibility=hidden"]

@@ -792,8 +792,9 @@ int value_and_grad_impl(bta_ctx* c, const double* theta, double* f, double* grad
       const long long n0 = c->launches;
       cudaGraph_t graph = nullptr;
       BTA_CUDA_OK(cudaStreamBeginCapture(c->s_main, cudaStreamCaptureModeThreadLocal));
-      int rc = use_twist(c) ? enqueue_gradient_twisted(c, ws, c->s_main, false, value_only)
-                             : enqueue_gradient(c, ws, c->s_main, c->s_side, false, value_only);
+      int rc = use_partitions(c) ? enqueue_gradient_partitioned(c, ws, c->s_main, false, value_only)
+               : use_twist(c)    ? enqueue_gradient_twisted(c, ws, c->s_main, false, value_only)
+                                 : enqueue_gradient(c, ws, c->s_main, c->s_side, false, value_only);
       cudaError_t ce = cudaStreamEndCapture(c->s_main, &graph);
       if (rc != BTA_OK) return rc;
       BTA_CUDA_OK(ce);
@@ -814,7 +815,16 @@ int value_and_grad_impl(bta_ctx* c, const double* theta, double* f, double* grad
     timed = false;
   } else {
     int rc;
-    if (use_twist(c) && !serial) {
+    if (use_partitions(c)) {
+      BTA_CUDA_OK(cudaEventRecord(ev[11], s0));
+      BTA_CUDA_OK(cudaStreamWaitEvent(c->s_main, ev[11], 0));
+      rc = enqueue_gradient_partitioned(c, ws, c->s_main, true, value_only);
+      if (rc != BTA_OK) return rc;
+      BTA_CUDA_OK(cudaEventRecord(ev[20], c->s_main));
+      BTA_CUDA_OK(cudaStreamWaitEvent(s0, ev[20], 0));
+      sync_stream = c->s_main;
+      timed = false;  // only the total is timed in this mode
+    } else if (use_twist(c) && !serial) {
       // run on the library's own prioritised streams; the caller's stream only orders the call
       BTA_CUDA_OK(cudaEventRecord(ev[11], s0));
       BTA_CUDA_OK(cudaStreamWaitEvent(c->s_main, ev[11], 0));
@@ -1052,6 +1062,7 @@ extern "C" size_t bta_workspace_bytes(const bta_ctx* c) {
   if (!c) return 0;
   const size_t one = grad_ws_bytes(c->md, c->store_mode);
   const size_t two = c->md.nt >= 3 ? twist_ws_bytes(c->md, c->store_mode) : (size_t)0;
+  if (use_partitions(c)) return part_ws_bytes(c);
   if (c->store_mode == BTA_STORE_HOST && use_twist(c)) return two;  // O(b^2): the point of the mode
   return one > two ? one : two;
 }

@@ -22,4 +22,4 @@ inline int bad(const char* msg) {
 constexpr int BTA_PMAX = 8;
 bool use_partitions(const bta_ctx* c);              // opt.partitions >= 2 and the model is long enough
 size_t part_ws_bytes(const bta_ctx* c);
-int enqueue_gradient_partitioned(bta_ctx* c, void* ws, cudaStream_t s0, bool value_only);
+int enqueue_gradient_partitioned(bta_ctx* c, void* ws, cudaStream_t s0, bool timed, bool value_only);

@@ -170,6 +170,7 @@ struct Options {
   int graph = -1;     // CUDA-graph replay from the second call on: -1 = by size (b <= 1024), 0 off, 1 on
   int serial = 0;     // both matrices on one stream, single chain (exclusive per-stage times)
   int pipeline = 1;   // forward sweeps: start the next block's factorisation under the tail of this block's products
+  int partitions = 0; // >= 2: time-domain partitioning with that many partitions and a reduced system (partition.cu)
 };
 
 struct bta_ctx {
@@ -203,7 +204,8 @@ struct bta_ctx {
   size_t host_bytes;
   cudaStream_t s_copy[4];            // its copy streams (one per sub-chain) and ring-slot events
   cudaEvent_t ev_ring[4][8];
-  cudaEvent_t ev_pipe[4][3];         // forward pipelining events of the four chains (sweep.h: Chain::pipe_ev)
+  cudaEvent_t ev_pipe[20][3];        // forward pipelining events per chain (sweep.h: Chain::pipe_ev)
+  cudaStream_t s_part[2][8], s_part_hi[2][8], s_part_x[2][8];  // partition.cu: streams per (matrix, partition), lazily
   cudaEvent_t ev_sw[256];            // lane-switch events, used round-robin
   unsigned ev_sw_next;
   long long launches;

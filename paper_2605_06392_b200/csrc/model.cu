@@ -127,6 +127,7 @@ int create_impl(bta_ctx* c, const bta_model_desc* desc, const bta_obs* obs) {
     c->opt.graph = env("BTA_GRAPH", c->opt.graph);
     c->opt.serial = env("BTA_SERIAL_CHAINS", c->opt.serial);
     c->opt.pipeline = env("BTA_PIPELINE", c->opt.pipeline);
+    c->opt.partitions = env("BTA_PARTITIONS", c->opt.partitions);
     g_tile_thresh = env("BTA_TILE_THRESH", (int)g_tile_thresh);
     g_tile_waves = env("BTA_TILE_WAVES", g_tile_waves);
   }
@@ -189,6 +190,12 @@ extern "C" int bta_destroy(bta_ctx* c) {
   for (auto& q : c->s_hi) kill_stream(q);
   for (auto& q : c->s_x) kill_stream(q);
   for (auto& q : c->s_copy) kill_stream(q);
+  for (int m = 0; m < 2; ++m)
+    for (int p = 0; p < 8; ++p) {
+      kill_stream(c->s_part[m][p]);
+      kill_stream(c->s_part_hi[m][p]);
+      kill_stream(c->s_part_x[m][p]);
+    }
   for (auto& q : c->ev_ring)
     for (auto& e : q) kill_event(e);
   for (auto& e : c->ev) kill_event(e);
@@ -247,6 +254,7 @@ int* option_slot(bta_ctx* c, int option) {
     case BTA_OPT_GRAPH: return &c->opt.graph;
     case BTA_OPT_SERIAL: return &c->opt.serial;
     case BTA_OPT_PIPELINE: return &c->opt.pipeline;
+    case BTA_OPT_PARTITIONS: return &c->opt.partitions;
   }
   return nullptr;
 }

@@ -421,3 +421,46 @@ def test_host_staged_workspace_is_independent_of_nt():
     block = 400 * 400 * 8
     assert ws[2, 64] - ws[2, 8] < 2 * block, ws
     assert ws[1, 64] - ws[1, 8] > 100 * block, ws
+
+
+PART_CASES = {
+    "nt3": lambda: CASES["nt3_twist_min"](),
+    "nt5_b25": lambda: (lambda m: (m, draw_obs(m, 300, 61), draw_theta(m, 61)))(make_model(5, 1, 5, 3)),
+    "nt7_b36": lambda: (lambda m: (m, draw_obs(m, 400, 62), draw_theta(m, 62)))(make_model(6, 1, 7, 2)),
+    "nt12_mv_b162": lambda: (lambda m: (m, draw_obs(m, 900, 63), draw_theta(m, 63)))(make_model(9, 2, 12, 4)),
+    "nt9_b144_a8": lambda: (lambda m: (m, draw_obs(m, 700, 64), draw_theta(m, 64)))(make_model(12, 1, 9, 8)),
+    "cfg1": lambda: make_config(1),
+}
+
+
+@pytest.mark.parametrize("P", [2, 3, 4])
+@pytest.mark.parametrize("name", list(PART_CASES))
+def test_time_domain_partitioning(name, P):
+    """SURVEY.md §8(f) NEXT-3 / PAPER.md:177-183: P partitions inside one GPU -- interior chains with fill to the top
+    boundary, a reduced system of 2P-1 boundary blocks, reversed order in the backward pass -- against the oracle,
+    component by component, and against the two-way elimination."""
+    model, obs, th = PART_CASES[name]()
+    ref = O.value_and_grad(model, obs, th)
+    M = _model(model, obs)
+    f0, g0 = M.inla_value_and_grad(th)
+    M.bta_set_partitions(P)
+    plan = M.bta_partition_plan(P)
+    assert plan[0][0] == 0 and plan[-1][1] == model.nt - 1
+    assert all(plan[i][0] == plan[i - 1][1] + 1 and plan[i][1] > plan[i][0] for i in range(1, len(plan)))
+    assert len(plan) == min(P, (model.nt + 1) // 2) or model.nt < 2 * P - 1
+    f, g = M.inla_value_and_grad(th)
+    im = M.last_intermediates()
+    f2, g2 = M.inla_value_and_grad(th)          # graph replay for small b; bitwise repeatable
+    v = M.inla_value(th)
+    M.close()
+    assert f2 == f and np.array_equal(g, g2)
+    assert abs(v - ref["f"]) <= TOL_F * abs(ref["f"])
+    assert abs(im["ld_p"] - ref["ld_p"]) <= TOL_F * abs(ref["ld_p"])
+    assert abs(im["ld_c"] - ref["ld_c"]) <= TOL_F * abs(ref["ld_c"])
+    assert abs(f - ref["f"]) <= TOL_F * abs(ref["f"])
+    assert np.max(np.abs(im["x"] - ref["x"])) <= 1e-9 * np.max(np.abs(ref["x"]))
+    for key in ("phaseA", "phaseB", "phaseC"):
+        s = max(np.max(np.abs(ref[key])), 1e-30)
+        assert np.max(np.abs(im[key] - ref[key])) <= 1e-9 * s, (key, im[key], ref[key])
+    assert grad_ok(g, ref["grad"]), (g, ref["grad"])
+    assert abs(f - f0) <= 1e-11 * abs(f0) and np.max(np.abs(g - g0)) <= 1e-9 * np.max(np.abs(g0))
