@@ -179,6 +179,33 @@ BTA_API int inla_optimize(bta_ctx* ctx, const double* theta0, int max_iter, doub
  * clipped so that nt >= 2P-1) and their first / last time blocks (HOST arrays of >= 8 entries, may be NULL). */
 BTA_API int bta_partition_plan(const bta_ctx* ctx, int partitions, int32_t* first, int32_t* last);
 
+/* The same partitioning ACROSS ranks, one partition per rank (rank r of nranks owns partition r), with the paper's
+ * communication pattern: no communication in Phase 1; ONE all-gather of the boundary data; every rank
+ * solves the reduced system redundantly; ONE all-reduce of the partial sums.  The library does no communication
+ * itself: the caller moves two device buffers between the three calls (the Python binding uses torch.distributed --
+ * NCCL over NVLink on GPUs):
+ *   1. inla_part_phase1: assembles and eliminates the interior of partition `rank` (both matrices) and packs its
+ *      boundary data into `slab` (DEVICE, bta_part_slab_doubles(ctx) doubles): per matrix the updated boundary blocks
+ *      D~(s_r), D~(e_r), the fill block Q~[e_r, s_r] and the tip accumulator, and for Q_c the stack rows [C~; r~] of
+ *      both boundary blocks.  (The original couplings B_{e_p} are functions of theta and are assembled by every rank.)
+ *      -> all-gather the slabs in rank order into `gathered` (nranks slabs).
+ *   2. inla_part_phase2: unpacks all slabs, factors and selectively inverts the reduced system (2 nranks - 1 blocks),
+ *      sweeps the interior of partition `rank` backwards and leaves the rank's per-block partial sums (traces,
+ *      quadratic forms, log-determinant and residual partials; zeros for blocks of other ranks; the reduced system is
+ *      counted by rank 0) in `partials` (DEVICE, caller-owned, bta_part_partial_doubles(ctx) doubles).
+ *      -> all-reduce (sum) that buffer in place.
+ *   3. inla_part_finish: f and grad f (HOST) from the summed partial sums -- identical on every rank.
+ * Requires BTA_STORE_FACTOR, bta_set_option(ctx, BTA_OPT_PARTITIONS, nranks) (it sizes bta_workspace_bytes), the same
+ * theta on every rank, and nt >= 2 nranks - 1.  x* from bta_last_intermediates is then valid only on the rank's own
+ * and on the boundary blocks. */
+BTA_API size_t bta_part_slab_doubles(const bta_ctx* ctx);
+BTA_API int inla_part_phase1(bta_ctx* ctx, const double* theta, int rank, int nranks, double* slab, void* ws,
+                             void* stream);
+BTA_API size_t bta_part_partial_doubles(const bta_ctx* ctx);
+BTA_API int inla_part_phase2(bta_ctx* ctx, int rank, int nranks, const double* gathered, double* partials, void* ws,
+                             void* stream);
+BTA_API int inla_part_finish(bta_ctx* ctx, const double* partials, double* f, double* grad, void* stream);
+
 enum {
   BTA_STAGE_ASSEMBLE = 0,
   BTA_STAGE_FWD_QC = 1,

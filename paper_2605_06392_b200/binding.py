@@ -87,6 +87,13 @@ def lib():
     L.bta_diag_ktime_begin.argtypes = []
     L.bta_diag_ktime_end.argtypes = [dp, dp, dp, C.POINTER(C.c_int64)]
     L.bta_partition_plan.argtypes = [vp, i32, C.POINTER(C.c_int32), C.POINTER(C.c_int32)]
+    L.bta_part_slab_doubles.argtypes = [vp]
+    L.bta_part_slab_doubles.restype = C.c_size_t
+    L.bta_part_partial_doubles.argtypes = [vp]
+    L.bta_part_partial_doubles.restype = C.c_size_t
+    L.inla_part_phase1.argtypes = [vp, dp, i32, i32, vp, vp, vp]
+    L.inla_part_phase2.argtypes = [vp, i32, i32, vp, vp, vp, vp]
+    L.inla_part_finish.argtypes = [vp, vp, dp, dp, vp]
     L.bta_set_option.argtypes = [vp, i32, i32]
     L.bta_get_option.argtypes = [vp, i32]
     _lib = L
@@ -316,6 +323,32 @@ class BtaModel:
         workspace."""
         self.bta_set_option(OPT_PARTITIONS, P)
         self._ws = None
+
+    # ---- the multi-rank form of the partitioning (include/bta.h: inla_part_*); buffers are torch tensors
+    def inla_part_phase1(self, theta, rank, nranks):
+        """-> this rank's slab (device tensor, float64) for the all-gather."""
+        import torch
+        th = np.ascontiguousarray(theta, dtype=np.float64)
+        slab = torch.zeros(lib().bta_part_slab_doubles(self._h), dtype=torch.float64, device=self.device)
+        _check(lib().inla_part_phase1(self._h, _dptr(th), int(rank), int(nranks), slab.data_ptr(),
+                                      self._workspace().data_ptr(), _stream()))
+        return slab
+
+    def inla_part_phase2(self, rank, nranks, gathered):
+        """gathered: device tensor of nranks slabs in rank order -> this rank's partial sums (device tensor)."""
+        import torch
+        assert gathered.is_contiguous() and gathered.numel() == nranks * lib().bta_part_slab_doubles(self._h)
+        partials = torch.empty(lib().bta_part_partial_doubles(self._h), dtype=torch.float64, device=self.device)
+        _check(lib().inla_part_phase2(self._h, int(rank), int(nranks), gathered.data_ptr(), partials.data_ptr(),
+                                      self._workspace().data_ptr(), _stream()))
+        return partials
+
+    def inla_part_finish(self, partials):
+        """partials: the all-reduced partial sums -> (f, grad)."""
+        f = C.c_double()
+        grad = np.zeros(self.d)
+        _check(lib().inla_part_finish(self._h, partials.data_ptr(), C.byref(f), _dptr(grad), _stream()))
+        return f.value, grad
 
     def bta_partition_plan(self, P):
         """-> [(first, last)] time blocks of the partitions a request for P partitions yields."""

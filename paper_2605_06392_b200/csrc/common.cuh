@@ -264,6 +264,9 @@ cudaError_t launch_trace_stencil(bta_ctx* c, int chain, int t, int kind, const d
 cudaError_t launch_noise_trace(bta_ctx* c, int t, const double* ZD, int ld, const double* ZC, int ldzc,
                                cudaStream_t st);
 cudaError_t launch_quad_stencil(bta_ctx* c, const double* x, cudaStream_t st);
+// ... restricted to the time blocks [t_lo, t_hi] (a rank's partition): the other blocks' partial sums are written as 0
+cudaError_t launch_quad_stencil(bta_ctx* c, const double* x, int t_lo, int t_hi, cudaStream_t st);
+cudaError_t launch_residual(bta_ctx* c, const double* x, int t_lo, int t_hi, cudaStream_t st);
 cudaError_t launch_logdet_partial(bta_ctx* c, int chain, const double* dvec, cudaStream_t st);
 cudaError_t launch_residual(bta_ctx* c, const double* x, cudaStream_t st);
 cudaError_t launch_scalars(bta_ctx* c, cudaStream_t st);

@@ -79,13 +79,13 @@ __global__ void __launch_bounds__(256) trace_stencil_kernel(ModelDims md, const 
 }
 
 // grid (nx, k*k, nt*2): kind 0: u = x_t, v = x_t;  kind 1 (t < nt-1): u = x_{t+1}, v = x_t  (Eq. 9, R7)
-__global__ void __launch_bounds__(256) quad_stencil_kernel(ModelDims md, const double* __restrict__ xv,
-                                                           double* __restrict__ out) {
+__global__ void __launch_bounds__(256) quad_stencil_kernel(ModelDims md, const double* __restrict__ xv, int t_lo,
+                                                           int t_hi, double* __restrict__ out) {
   __shared__ double red[256];
   const int s = blockIdx.x * 256 + threadIdx.x, vi = blockIdx.y / md.k, vj = blockIdx.y % md.k, g = md.g;
   const int t = blockIdx.z >> 1, kind = blockIdx.z & 1;
   double acc[3] = {0.0, 0.0, 0.0};
-  const bool live = !(kind == 1 && t >= md.nt - 1);
+  const bool live = !(kind == 1 && t >= md.nt - 1) && t >= t_lo && t <= t_hi;
   if (live && s < md.ns) {
     const int y = s / g, x = s % g;
     const double u = xv[(long long)(t + kind) * md.b + vi * md.ns + s];
@@ -140,15 +140,17 @@ __global__ void __launch_bounds__(256) logdet_partial_kernel(long long N, const 
 __global__ void __launch_bounds__(256) residual_kernel(long long m, ModelDims md, const int* __restrict__ var,
                                                        const int* __restrict__ node, const int* __restrict__ time,
                                                        const double* __restrict__ cov, const double* __restrict__ y,
-                                                       const double* __restrict__ x, double* __restrict__ out) {
+                                                       const double* __restrict__ x, int t_lo, int t_hi,
+                                                       double* __restrict__ out) {
   __shared__ double red[256];
   const long long chunk = (m + gridDim.x - 1) / gridDim.x;
   const long long lo = min(m, (long long)blockIdx.x * chunk), hi = min(m, lo + chunk);
   double acc[KMAX] = {0.0, 0.0, 0.0, 0.0};
   const double* xT = x + (long long)md.nt * md.b;
   for (long long i = lo + threadIdx.x; i < hi; i += 256) {
-    const int v = var[i];
-    double pred = x[(long long)time[i] * md.b + v * md.ns + node[i]];
+    const int v = var[i], ti = time[i];
+    if (ti < t_lo || ti > t_hi) continue;
+    double pred = x[(long long)ti * md.b + v * md.ns + node[i]];
     for (int p = 0; p < md.apr; ++p) pred = fma(cov[i * md.apr + p], xT[v * md.apr + p], pred);
     const double r = y[i] - pred;
 #pragma unroll
@@ -307,11 +309,14 @@ cudaError_t launch_noise_trace(bta_ctx* c, int t, const double* ZD, int ld, cons
 }
 
 cudaError_t launch_quad_stencil(bta_ctx* c, const double* x, cudaStream_t st) {
+  return launch_quad_stencil(c, x, 0, c->md.nt - 1, st);
+}
+cudaError_t launch_quad_stencil(bta_ctx* c, const double* x, int t_lo, int t_hi, cudaStream_t st) {
   const ModelDims& md = c->md;
   SmallLayout L = small_layout(md);
   dim3 grid(L.nx, md.k * md.k, md.nt * 2);
   KTimeScope kt(BTA_KC_CONTRACT, st, 2.0 * 7.0 * 13.0 * md.k * (double)md.b * md.nt, 8.0 * 2.0 * md.k * (double)md.N);
-  quad_stencil_kernel<<<grid, 256, 0, st>>>(md, x, c->small + L.qd);
+  quad_stencil_kernel<<<grid, 256, 0, st>>>(md, x, t_lo, t_hi, c->small + L.qd);
   BTA_COUNT(c);
   return cudaGetLastError();
 }
@@ -325,9 +330,12 @@ cudaError_t launch_logdet_partial(bta_ctx* c, int chain, const double* dvec, cud
 }
 
 cudaError_t launch_residual(bta_ctx* c, const double* x, cudaStream_t st) {
+  return launch_residual(c, x, 0, c->md.nt - 1, st);
+}
+cudaError_t launch_residual(bta_ctx* c, const double* x, int t_lo, int t_hi, cudaStream_t st) {
   SmallLayout L = small_layout(c->md);
   KTimeScope kt(BTA_KC_OTHER, st, 0.0, (double)c->m * (12.0 + 8.0 * c->md.apr + 8.0));
-  residual_kernel<<<256, 256, 0, st>>>(c->m, c->md, c->o_var, c->o_node, c->o_time, c->o_cov, c->o_y, x,
+  residual_kernel<<<256, 256, 0, st>>>(c->m, c->md, c->o_var, c->o_node, c->o_time, c->o_cov, c->o_y, x, t_lo, t_hi,
                                        c->small + L.rsspart);
   BTA_COUNT(c);
   return cudaGetLastError();

@@ -138,14 +138,6 @@ bool use_partitions(const bta_ctx* c) {
   return c->opt.partitions >= 2 && c->md.nt >= 3 && c->store_mode == BTA_STORE_FACTOR && !c->opt.serial;
 }
 
-size_t part_ws_bytes(const bta_ctx* c) {
-  const Plan pl = make_plan(c->md.nt, c->opt.partitions);
-  Bump bp(nullptr);
-  carve_part(bp, c->md, pl, true);
-  carve_part(bp, c->md, pl, false);
-  return bp.off + 256;
-}
-
 extern "C" int bta_partition_plan(const bta_ctx* c, int partitions, int32_t* first, int32_t* last) {
   if (!c) return 0;
   const Plan pl = make_plan(c->md.nt, partitions);
@@ -156,45 +148,81 @@ extern "C" int bta_partition_plan(const bta_ctx* c, int partitions, int32_t* fir
   return pl.P;
 }
 
-// One whole gradient with P partitions per matrix.  All work is forked from and joined back into s0 (so the whole
-// call can also be captured into a CUDA graph).
-int enqueue_gradient_partitioned(bta_ctx* c, void* ws, cudaStream_t s0, bool timed, bool value_only) {
-  const ModelDims& md = c->md;
-  const Plan pl = make_plan(md.nt, c->opt.partitions);
-  const int P = pl.P, nred = pl.nred;
-  if (int rc = ensure_streams(c, P); rc != BTA_OK) return rc;
-  Bump bp(ws);
-  PartWs W[2] = {carve_part(bp, md, pl, true), carve_part(bp, md, pl, false)};
-  SmallLayout L = small_layout(md);
-  const long long bb = (long long)md.b * md.b;
-  const int b = md.b, a = md.a, PR = a + 1;
-  const long long rs = (long long)PR * b;
-  cudaEvent_t* ev = c->ev;
-  auto link = [&](cudaStream_t from, cudaStream_t to) -> cudaError_t {
+// ------------------------------------------------------------------------------------------------
+// One gradient with P partitions per matrix, in stages.  nranks == 1: all partitions are local (one GPU).  nranks > 1:
+// rank r owns partition r; the stages map onto the paper's phases:
+//   phase1  = assembly + Phase 1 of the local partitions + merge into their boundary blocks (+ pack the slab)
+//   phase2  = (unpack all slabs +) reduced system forward / backward + Phase 1' of the local partitions + the local
+//             per-block partial sums
+//   finish  = scalar assembly from the (summed) partial sums
+// All work is forked from and joined back into s0 (so a single-rank call can be captured into a CUDA graph).
+// ------------------------------------------------------------------------------------------------
+namespace {
+
+__global__ void fill_kernel(long long n, double v, double* __restrict__ dst) {
+  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) dst[i] = v;
+}
+
+struct PartRun {
+  bta_ctx* c = nullptr;
+  Plan pl;
+  PartWs W[2];
+  Chain pc[2][BTA_PMAX], red[2];
+  Fill fills[2][BTA_PMAX];
+  int tmap[2 * BTA_PMAX], bmap[2 * BTA_PMAX];
+  double* dmap[2][2 * BTA_PMAX];
+  cudaStream_t S[2][BTA_PMAX];
+  cudaStream_t s0 = nullptr;
+  SmallLayout L;
+  bool value_only = false;
+  int rank = 0, nranks = 1;
+  double* dvec_dummy = nullptr;   // ranks != 0: where the (redundant) reduced chain puts its diag(L)
+  long long bb = 0, rs = 0;
+  int b = 0, a = 0, PR = 0;
+
+  bool local(int p) const { return nranks == 1 || p == rank; }
+  cudaError_t link(cudaStream_t from, cudaStream_t to) {
     if (from == to) return cudaSuccess;
     cudaEvent_t e = c->ev_sw[(c->ev_sw_next++) % BTA_NSW];
     cudaError_t ce = cudaEventRecord(e, from);
     return ce != cudaSuccess ? ce : cudaStreamWaitEvent(to, e, 0);
-  };
+  }
+  size_t slab_doubles() const { return 2 * (3 * (size_t)bb + (size_t)a * (a + 1)) + 2 * (size_t)rs; }
+
+  int init(bta_ctx* ctx, void* ws, cudaStream_t stream, bool vonly, int rank_, int nranks_);
+  int phase1();
+  int pack(double* slab);
+  int unpack(const double* gathered);
+  int phase2();
+  int finish(bool timed);
+};
+
+int PartRun::init(bta_ctx* ctx, void* ws, cudaStream_t stream, bool vonly, int rank_, int nranks_) {
+  c = ctx;
+  s0 = stream;
+  value_only = vonly;
+  rank = rank_;
+  nranks = nranks_;
+  const ModelDims& md = c->md;
+  pl = make_plan(md.nt, nranks > 1 ? nranks : c->opt.partitions);
+  if (nranks > 1 && pl.P != nranks) return bad("inla_part_*: nt is too small for that many ranks (need nt >= 2 nranks - 1)");
+  const int P = pl.P, nred = pl.nred;
+  if (int rc = ensure_streams(c, P); rc != BTA_OK) return rc;
+  Bump bp(ws);
+  W[0] = carve_part(bp, md, pl, true);
+  W[1] = carve_part(bp, md, pl, false);
+  dvec_dummy = bp.take(md.N);
+  L = small_layout(md);
+  bb = (long long)md.b * md.b;
+  b = md.b;
+  a = md.a;
+  PR = a + 1;
+  rs = (long long)PR * b;
   // streams: [matrix][partition]; (0, 0) is the caller-ordered stream s0; the reduced chains run on [m][0]
-  cudaStream_t S[2][BTA_PMAX];
   for (int m = 0; m < 2; ++m)
     for (int p = 0; p < P; ++p) S[m][p] = (m == 0 && p == 0) ? s0 : c->s_part[m][p];
-
-  if (timed) CKP(cudaEventRecord(ev[0], s0));
-  CKP(cudaMemcpyAsync(c->theta_dev, c->host_pinned, md.d * sizeof(double), cudaMemcpyHostToDevice, s0));
-  CKP(launch_theta_prep(c, s0));
-  CKP(cudaMemsetAsync(c->pivot_flag, 0xFF, sizeof(unsigned long long), s0));
-  // stack rows of all blocks, tips
-  CKP(launch_assemble(c, BTA_COND, nullptr, bb, nullptr, 0, W[0].Rin, rs, W[0].T, a, W[0].Rin + (long long)a * b, rs,
-                      W[0].rtip, 1, s0));
-  for (int m = 0; m < 2; ++m)
-    for (int p = 0; p < P; ++p) CKP(link(s0, S[m][p]));
-  CKP(launch_assemble(c, BTA_PRIOR, nullptr, bb, nullptr, 0, nullptr, 0, W[1].T, a, nullptr, 0, nullptr, 0, S[1][0]));
-
-  // ---- host tables of the reduced system (same for both matrices but for the block pointers)
-  int tmap[2 * BTA_PMAX], bmap[2 * BTA_PMAX];
-  double* dmap[2][2 * BTA_PMAX];
+  // host tables of the reduced system (same for both matrices but for the block pointers)
   tmap[0] = pl.e[0];
   for (int p = 1; p < P; ++p) {
     tmap[pl.q_s(p)] = pl.s[p];
@@ -210,9 +238,6 @@ int enqueue_gradient_partitioned(bta_ctx* c, void* ws, cudaStream_t s0, bool tim
   for (int m = 0; m < 2; ++m)
     for (int q = 0; q < nred; ++q) dmap[m][q] = W[m].D + (long long)tmap[q] * bb;
 
-  // ---- chains
-  Chain pc[2][BTA_PMAX], red[2];
-  Fill fills[2][BTA_PMAX];
   for (int m = 0; m < 2; ++m) {
     const bool cond = m == 0;
     const int chs = cond ? CH_COND : CH_PRIOR;
@@ -252,7 +277,7 @@ int enqueue_gradient_partitioned(bta_ctx* c, void* ws, cudaStream_t s0, bool tim
         k.xout = w.x;
         k.ld_x = md.N;
       }
-      const int sp = m * (BTA_PMAX + 1) + p;  // slot of this chain's streams / events
+      const int sp = m * (BTA_PMAX + 1) + p;  // slot of this chain's events
       if (c->opt.lanes) k.hi = p < P ? c->s_part_hi[m][p] : c->s_part_hi[m][0];
       k.lanes_bwd = c->opt.lanes != 2;
       if (c->opt.split) k.xs = p < P ? c->s_part_x[m][p] : c->s_part_x[m][0];
@@ -268,7 +293,7 @@ int enqueue_gradient_partitioned(bta_ctx* c, void* ws, cudaStream_t s0, bool tim
         k.d_stride = bb;
         k.Bin = s.B + bb;   // B_t assembled into slot t+1, L_Bt written to slot t
         k.Bout = s.B;
-        k.Tt = p == 0 ? c->small + L.Tt[chs] : s.Tt;
+        k.Tt = (p == 0 && nranks == 1) ? c->small + L.Tt[chs] : s.Tt;
         if (cond) {
           k.Rin = w.Rin + (long long)i0 * rs;
           k.Rout = w.Rout + (long long)i0 * rs;
@@ -309,6 +334,10 @@ int enqueue_gradient_partitioned(bta_ctx* c, void* ws, cudaStream_t s0, bool tim
         k.Bout = w.BredOut;
         k.Tt = c->small + L.Tt[chs];
         k.selinv_inplace = !value_only;   // Sigma of the boundary blocks stays in their slots for Phase 1'
+        if (nranks > 1 && rank != 0) {    // every rank solves the reduced system; rank 0 alone counts it
+          k.contract = false;
+          k.dvec = dvec_dummy;
+        }
         if (cond) {
           k.Rin = w.RinRed;
           k.Rout = w.RoutRed;
@@ -320,14 +349,38 @@ int enqueue_gradient_partitioned(bta_ctx* c, void* ws, cudaStream_t s0, bool tim
       }
     }
   }
+  return BTA_OK;
+}
 
-  // ---- assembly per partition: its diagonal blocks (boundaries included), interior couplings, fill seed, reduced
-  //      couplings and the stack rows of its boundary blocks
+int PartRun::phase1() {
+  const ModelDims& md = c->md;
+  const int P = pl.P;
+  CKP(cudaMemcpyAsync(c->theta_dev, c->host_pinned, md.d * sizeof(double), cudaMemcpyHostToDevice, s0));
+  CKP(launch_theta_prep(c, s0));
+  CKP(cudaMemsetAsync(c->pivot_flag, 0xFF, sizeof(unsigned long long), s0));
+  if (nranks > 1) {  // partial sums of blocks this rank does not own stay zero; diag(L) entries it does not own stay 1
+    CKP(cudaMemsetAsync(c->small, 0, L.Tt[0] * sizeof(double), s0));
+    for (int m = 0; m < 2; ++m) {
+      fill_kernel<<<(unsigned)((md.N + 255) / 256), 256, 0, s0>>>(md.N, 1.0, W[m].dvec);
+      BTA_COUNT(c);
+    }
+  }
+  // stack rows of all blocks, tips
+  CKP(launch_assemble(c, BTA_COND, nullptr, bb, nullptr, 0, W[0].Rin, rs, W[0].T, a, W[0].Rin + (long long)a * b, rs,
+                      W[0].rtip, 1, s0));
+  for (int m = 0; m < 2; ++m)
+    for (int p = 0; p < P; ++p) CKP(link(s0, S[m][p]));
+  CKP(launch_assemble(c, BTA_PRIOR, nullptr, bb, nullptr, 0, nullptr, 0, W[1].T, a, nullptr, 0, nullptr, 0, S[1][0]));
+
+  // ---- assembly per local partition: its diagonal blocks (boundaries included), interior couplings, fill seed, and
+  //      the stack rows of its boundary blocks; the reduced system's original couplings B_{e_p} (every rank, all p)
   for (int m = 0; m < 2; ++m) {
     const int which = m == 0 ? BTA_COND : BTA_PRIOR;
     const PartWs& w = W[m];
     for (int p = 0; p < P; ++p) {
       cudaStream_t st = S[m][p];
+      if (p < P - 1) CKP(launch_assemble_block(c, which, 1, pl.e[p], 0, w.BredIn + (long long)pl.q_e(p) * bb, st));
+      if (!local(p)) continue;
       const int i0 = pl.first_int(p), ni = pl.nint(p);
       CKP(launch_assemble_seq(c, which, 0, pl.s[p], 1, pl.e[p] - pl.s[p] + 1, 0, w.D + (long long)pl.s[p] * bb, bb, st));
       if (ni > 0) CKP(launch_assemble_seq(c, which, 1, i0, 1, ni, 0, pc[m][p].Bin, bb, st));
@@ -337,7 +390,6 @@ int enqueue_gradient_partitioned(bta_ctx* c, void* ws, cudaStream_t s0, bool tim
         else
           CKP(launch_assemble_block(c, which, 1, pl.s[p], 0, w.BredIn + (long long)pl.q_s(p) * bb, st));
       }
-      if (p < P - 1) CKP(launch_assemble_block(c, which, 1, pl.e[p], 0, w.BredIn + (long long)pl.q_e(p) * bb, st));
       if (m == 0) {
         if (p > 0)
           CKP(cudaMemcpyAsync(w.RinRed + (long long)pl.q_s(p) * rs, w.Rin + (long long)pl.s[p] * rs, rs * sizeof(double),
@@ -348,19 +400,22 @@ int enqueue_gradient_partitioned(bta_ctx* c, void* ws, cudaStream_t s0, bool tim
     }
   }
 
-  // ---- Phase 1: the interior chains of all partitions, launches interleaved block by block
+  // ---- Phase 1: the interior chains of the local partitions, launches interleaved block by block
   int maxlen = 0;
-  for (int p = 0; p < P; ++p) maxlen = std::max(maxlen, pl.nint(p));
+  for (int p = 0; p < P; ++p)
+    if (local(p)) maxlen = std::max(maxlen, pl.nint(p));
   for (int m = 0; m < 2; ++m)
-    for (int p = 0; p < P; ++p) CKP(chain_forward_begin(pc[m][p], S[m][p]));
+    for (int p = 0; p < P; ++p)
+      if (local(p)) CKP(chain_forward_begin(pc[m][p], S[m][p]));
   for (int s = 0; s < maxlen; ++s)
     for (int m = 0; m < 2; ++m)
       for (int p = 0; p < P; ++p)
-        if (s < pc[m][p].nt) CKP(chain_forward_step(pc[m][p], s, S[m][p]));
+        if (local(p) && s < pc[m][p].nt) CKP(chain_forward_step(pc[m][p], s, S[m][p]));
   // merge into the reduced system: Schur update and stack update of e_p from the last interior block, tip sums
   for (int m = 0; m < 2; ++m) {
     const PartWs& w = W[m];
     for (int p = 0; p < P; ++p) {
+      if (!local(p)) continue;
       Chain& k = pc[m][p];
       cudaStream_t st = S[m][p];
       CKP(chain_to_big(k, st));
@@ -376,7 +431,7 @@ int enqueue_gradient_partitioned(bta_ctx* c, void* ws, cudaStream_t s0, bool tim
         CKP(launch_gemm(g, st));
         BTA_COUNT(c);
       }
-      if (p > 0) {
+      if (nranks == 1 && p > 0) {
         CKP(link(st, S[m][0]));
         if (a > 0) {
           const int n = a * (a + red[m].nr);
@@ -386,7 +441,70 @@ int enqueue_gradient_partitioned(bta_ctx* c, void* ws, cudaStream_t s0, bool tim
       }
     }
   }
+  return BTA_OK;
+}
 
+// Slab of the local partition p = rank, per matrix m: [D~(s_p) | D~(e_p) | Q~(e_p, s_p) | tip accumulator], and for
+// Q_c the stack rows [C~; r~] of s_p and e_p.  Partition 0 leaves the s_p and fill parts unused (uniform slab size).
+int PartRun::pack(double* slab) {
+  const int p = rank;
+  size_t off = 0;
+  for (int m = 0; m < 2; ++m) {
+    const PartWs& w = W[m];
+    cudaStream_t st = S[m][p];
+    auto put = [&](const double* src, size_t n) -> cudaError_t {
+      cudaError_t e = src ? cudaMemcpyAsync(slab + off, src, n * sizeof(double), cudaMemcpyDeviceToDevice, st) : cudaSuccess;
+      off += n;
+      return e;
+    };
+    CKP(put(p > 0 ? w.D + (long long)pl.s[p] * bb : nullptr, bb));
+    CKP(put(w.D + (long long)pl.e[p] * bb, bb));
+    CKP(put(p > 0 ? w.BredIn + (long long)pl.q_s(p) * bb : nullptr, bb));
+    CKP(put(pc[m][p].Tt, (size_t)a * (a + 1)));
+    if (m == 0) {
+      CKP(put(p > 0 ? w.RinRed + (long long)pl.q_s(p) * rs : nullptr, rs));
+      CKP(put(w.RinRed + (long long)pl.q_e(p) * rs, rs));
+    }
+    CKP(link(st, s0));
+  }
+  return BTA_OK;
+}
+
+int PartRun::unpack(const double* gathered) {
+  const size_t sd = slab_doubles();
+  for (int m = 0; m < 2; ++m) {
+    const PartWs& w = W[m];
+    cudaStream_t st = S[m][0];
+    CKP(link(s0, st));
+    const int ntip = a * (a + red[m].nr);
+    if (ntip > 0) CKP(cudaMemsetAsync(red[m].Tt, 0, ntip * sizeof(double), st));
+    for (int p = 0; p < pl.P; ++p) {
+      const double* src = gathered + (size_t)p * sd + (m == 0 ? 0 : 3 * (size_t)bb + (size_t)a * (a + 1) + 2 * (size_t)rs);
+      auto get = [&](double* dst, size_t n) -> cudaError_t {
+        cudaError_t e = dst ? cudaMemcpyAsync(dst, src, n * sizeof(double), cudaMemcpyDeviceToDevice, st) : cudaSuccess;
+        src += n;
+        return e;
+      };
+      CKP(get(p > 0 ? w.D + (long long)pl.s[p] * bb : nullptr, bb));
+      CKP(get(w.D + (long long)pl.e[p] * bb, bb));
+      CKP(get(p > 0 ? w.BredIn + (long long)pl.q_s(p) * bb : nullptr, bb));
+      if (ntip > 0) {
+        vec_add_kernel<<<(ntip + 127) / 128, 128, 0, st>>>(ntip, src, red[m].Tt);
+        BTA_COUNT(c);
+      }
+      src += (size_t)a * (a + 1);
+      if (m == 0) {
+        CKP(get(p > 0 ? w.RinRed + (long long)pl.q_s(p) * rs : nullptr, rs));
+        CKP(get(w.RinRed + (long long)pl.q_e(p) * rs, rs));
+      }
+    }
+  }
+  return BTA_OK;
+}
+
+int PartRun::phase2() {
+  const ModelDims& md = c->md;
+  const int P = pl.P, nred = pl.nred;
   // ---- Phase 2: the reduced system (2P-1 boundary blocks), forward + tip + log-determinant
   for (int m = 0; m < 2; ++m) {
     cudaStream_t st = S[m][0];
@@ -401,29 +519,131 @@ int enqueue_gradient_partitioned(bta_ctx* c, void* ws, cudaStream_t s0, bool tim
     cudaStream_t st = S[m][0];
     for (int q = nred - 1; q >= 0; --q) CKP(chain_backward_step(red[m], q, st));
     CKP(chain_to_big(red[m], st));
-    for (int p = 1; p < P; ++p) CKP(link(st, S[m][p]));
+    for (int p = 1; p < P; ++p)
+      if (local(p)) CKP(link(st, S[m][p]));
   }
-  // ---- Phase 1': interior backward sweeps, concurrently
+  // ---- Phase 1': interior backward sweeps of the local partitions, concurrently
+  int maxlen = 0;
+  for (int p = 0; p < P; ++p)
+    if (local(p)) maxlen = std::max(maxlen, pl.nint(p));
   for (int s = maxlen - 1; s >= 0; --s)
     for (int m = 0; m < 2; ++m) {
       if (value_only && m == 1) continue;
       for (int p = 0; p < P; ++p)
-        if (s < pc[m][p].nt) CKP(chain_backward_step(pc[m][p], s, S[m][p]));
+        if (local(p) && s < pc[m][p].nt) CKP(chain_backward_step(pc[m][p], s, S[m][p]));
     }
-  // ---- join everything back onto s0
+  // ---- join everything back onto s0; Phase B and the residual over the local time range
   for (int m = 0; m < 2; ++m)
     for (int p = 0; p < P; ++p) {
-      CKP(chain_to_big(pc[m][p], S[m][p]));
+      if (local(p)) CKP(chain_to_big(pc[m][p], S[m][p]));
       CKP(link(S[m][p], s0));
     }
   CKP(cudaMemcpyAsync(W[0].x + (long long)md.nt * b, red[0].xT, a * sizeof(double), cudaMemcpyDeviceToDevice, s0));
-  CKP(launch_quad_stencil(c, W[0].x, s0));
-  CKP(launch_residual(c, W[0].x, s0));
+  const int t_lo = nranks == 1 ? 0 : pl.s[rank], t_hi = nranks == 1 ? md.nt - 1 : pl.e[rank];
+  CKP(launch_quad_stencil(c, W[0].x, t_lo, t_hi, s0));
+  CKP(launch_residual(c, W[0].x, t_lo, t_hi, s0));
+  return BTA_OK;
+}
+
+int PartRun::finish(bool timed) {
+  const ModelDims& md = c->md;
   CKP(launch_scalars(c, s0));
   const int nout = 1 + md.d + 2 + 3 * md.d + md.k + 1;
   CKP(cudaMemcpyAsync(c->host_pinned + 64, c->small + L.out, nout * sizeof(double), cudaMemcpyDeviceToHost, s0));
   CKP(cudaMemcpyAsync(c->x_keep, W[0].x, md.N * sizeof(double), cudaMemcpyDeviceToDevice, s0));
-  if (timed) CKP(cudaEventRecord(ev[8], s0));
+  if (timed) CKP(cudaEventRecord(c->ev[8], s0));
   c->have_x = true;
+  return BTA_OK;
+}
+
+}  // namespace
+
+size_t part_ws_bytes(const bta_ctx* c) {
+  const Plan pl = make_plan(c->md.nt, c->opt.partitions);
+  Bump bp(nullptr);
+  carve_part(bp, c->md, pl, true);
+  carve_part(bp, c->md, pl, false);
+  bp.take(c->md.N);
+  return bp.off + 256;
+}
+
+int enqueue_gradient_partitioned(bta_ctx* c, void* ws, cudaStream_t s0, bool timed, bool value_only) {
+  static thread_local PartRun run;   // ~20 Chain objects: keep them off the stack
+  if (int rc = run.init(c, ws, s0, value_only, 0, 1); rc != BTA_OK) return rc;
+  if (timed) CKP(cudaEventRecord(c->ev[0], s0));
+  if (int rc = run.phase1(); rc != BTA_OK) return rc;
+  if (int rc = run.phase2(); rc != BTA_OK) return rc;
+  return run.finish(timed);
+}
+
+// ---- the multi-rank form (include/bta.h: inla_part_*)
+extern "C" size_t bta_part_slab_doubles(const bta_ctx* c) {
+  if (!c) return 0;
+  const size_t bb = (size_t)c->md.b * c->md.b, rs = (size_t)(c->md.a + 1) * c->md.b;
+  return 2 * (3 * bb + (size_t)c->md.a * (c->md.a + 1)) + 2 * rs;
+}
+
+extern "C" int inla_part_phase1(bta_ctx* c, const double* theta, int rank, int nranks, double* slab, void* ws,
+                                void* stream) {
+  if (!c || !theta || !slab || !ws) return bad("inla_part_phase1: null ctx, theta, slab or workspace");
+  if (nranks < 2 || nranks > BTA_PMAX || rank < 0 || rank >= nranks) return bad("inla_part_phase1: need 2 <= nranks <= 8, 0 <= rank < nranks");
+  if (c->store_mode != BTA_STORE_FACTOR || c->opt.partitions != nranks)
+    return bad("inla_part_phase1: set BTA_STORE_FACTOR and bta_set_option(ctx, BTA_OPT_PARTITIONS, nranks) first (they size the workspace)");
+  DeviceGuard guard(c->device);
+  cudaStream_t s0 = (cudaStream_t)stream;
+  memcpy(c->host_pinned, theta, c->md.d * sizeof(double));
+  static thread_local PartRun run;
+  if (int rc = run.init(c, ws, s0, false, rank, nranks); rc != BTA_OK) return rc;
+  if (int rc = run.phase1(); rc != BTA_OK) return rc;
+  if (int rc = run.pack(slab); rc != BTA_OK) return rc;
+  CKP(cudaStreamSynchronize(s0));   // the slab is complete; host_pinned may be reused
+  return BTA_OK;
+}
+
+extern "C" size_t bta_part_partial_doubles(const bta_ctx* c) { return c ? small_layout(c->md).Tt[0] : 0; }
+
+extern "C" int inla_part_phase2(bta_ctx* c, int rank, int nranks, const double* gathered, double* partials, void* ws,
+                                void* stream) {
+  if (!c || !gathered || !partials || !ws) return bad("inla_part_phase2: null ctx, gathered slabs, partials or workspace");
+  if (nranks < 2 || nranks > BTA_PMAX || rank < 0 || rank >= nranks || c->opt.partitions != nranks)
+    return bad("inla_part_phase2: rank / nranks do not match phase 1");
+  DeviceGuard guard(c->device);
+  cudaStream_t s0 = (cudaStream_t)stream;
+  static thread_local PartRun run;
+  if (int rc = run.init(c, ws, s0, false, rank, nranks); rc != BTA_OK) return rc;
+  if (int rc = run.unpack(gathered); rc != BTA_OK) return rc;
+  if (int rc = run.phase2(); rc != BTA_OK) return rc;
+  CKP(cudaMemcpyAsync(partials, c->small, run.L.Tt[0] * sizeof(double), cudaMemcpyDeviceToDevice, s0));
+  CKP(cudaStreamSynchronize(s0));
+  return BTA_OK;
+}
+
+extern "C" int inla_part_finish(bta_ctx* c, const double* partials, double* f, double* grad, void* stream) {
+  if (!c || !partials) return bad("inla_part_finish: null ctx or partials");
+  DeviceGuard guard(c->device);
+  cudaStream_t s0 = (cudaStream_t)stream;
+  const ModelDims& md = c->md;
+  SmallLayout L = small_layout(md);
+  CKP(cudaMemcpyAsync(c->small, partials, L.Tt[0] * sizeof(double), cudaMemcpyDeviceToDevice, s0));
+  CKP(launch_scalars(c, s0));
+  const int nout = 1 + md.d + 2 + 3 * md.d + md.k + 1;
+  CKP(cudaMemcpyAsync(c->host_pinned + 64, c->small + L.out, nout * sizeof(double), cudaMemcpyDeviceToHost, s0));
+  unsigned long long flag = 0;
+  CKP(cudaMemcpyAsync(&flag, c->pivot_flag, sizeof flag, cudaMemcpyDeviceToHost, s0));
+  CKP(cudaStreamSynchronize(s0));
+  const double* o = c->host_pinned + 64;
+  if (f) *f = o[0];
+  if (grad) memcpy(grad, o + 1, md.d * sizeof(double));
+  c->last_ld[0] = o[1 + md.d];
+  c->last_ld[1] = o[1 + md.d + 1];
+  c->last_parts.assign(o + 1 + md.d + 2, o + 1 + md.d + 2 + 3 * md.d);
+  c->last_rss.assign(o + 1 + md.d + 2 + 3 * md.d, o + 1 + md.d + 2 + 3 * md.d + md.k);
+  c->last_quad = o[1 + md.d + 2 + 3 * md.d + md.k];
+  if (flag != ~0ull) {
+    c->last_pivot = (long long)flag;
+    bta_set_error("matrix is not positive definite on this rank (bta_last_pivot)");
+    return BTA_ERR_NOTSPD;
+  }
+  c->last_pivot = 0;
   return BTA_OK;
 }

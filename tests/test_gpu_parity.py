@@ -464,3 +464,59 @@ def test_time_domain_partitioning(name, P):
         assert np.max(np.abs(im[key] - ref[key])) <= 1e-9 * s, (key, im[key], ref[key])
     assert grad_ok(g, ref["grad"]), (g, ref["grad"])
     assert abs(f - f0) <= 1e-11 * abs(f0) and np.max(np.abs(g - g0)) <= 1e-9 * np.max(np.abs(g0))
+
+
+@pytest.mark.parametrize("name,P", [("nt3", 2), ("nt5_b25", 2), ("nt7_b36", 3), ("nt12_mv_b162", 4), ("nt9_b144_a8", 3),
+                                    ("cfg1", 4), ("cfg1", 8)])
+def test_partitioning_across_ranks_emulated(name, P):
+    """The multi-rank form (include/bta.h: inla_part_*) with the ranks emulated one after the other
+    in this process: P contexts, each eliminating ONE partition; slabs concatenated in rank order (= all-gather);
+    partial sums added (= all-reduce); every rank must return the oracle's f and gradient."""
+    import torch
+    model, obs, th = PART_CASES[name]()
+    ref = O.value_and_grad(model, obs, th)
+    ranks = [_model(model, obs) for _ in range(P)]
+    for M in ranks:
+        M.bta_set_partitions(P)
+    assert len(ranks[0].bta_partition_plan(P)) == P
+    slabs = [M.inla_part_phase1(th, r, P) for r, M in enumerate(ranks)]
+    gathered = torch.cat(slabs)
+    parts = [M.inla_part_phase2(r, P, gathered) for r, M in enumerate(ranks)]
+    total = torch.stack(parts).sum(0)
+    out = [M.inla_part_finish(total.clone()) for M in ranks]
+    ims = [M.last_intermediates(want_x=False) for M in ranks]
+    for M in ranks:
+        M.close()
+    for (f, g), im in zip(out, ims):
+        assert f == out[0][0] and np.array_equal(g, out[0][1])          # identical on every rank
+        assert abs(f - ref["f"]) <= TOL_F * abs(ref["f"])
+        assert grad_ok(g, ref["grad"]), (g, ref["grad"])
+        assert abs(im["ld_p"] - ref["ld_p"]) <= TOL_F * abs(ref["ld_p"])
+        assert abs(im["ld_c"] - ref["ld_c"]) <= TOL_F * abs(ref["ld_c"])
+        for key in ("phaseA", "phaseB", "phaseC"):
+            s = max(np.max(np.abs(ref[key])), 1e-30)
+            assert np.max(np.abs(im[key] - ref[key])) <= 1e-9 * s, key
+
+
+def test_partitioning_across_ranks_two_processes():
+    """Two real processes (torch.distributed, gloo, both on cuda:0 -- the collectives are host-side, no kernel of one
+    rank waits for the other) run paper_2605_06392_b200.partitioned.value_and_grad on config 1's shapes."""
+    import json
+    import os
+    import socket
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    s = socket.socket()
+    s.bind(("127.0.0.1", 0))
+    port = s.getsockname()[1]
+    s.close()
+    out = subprocess.run([sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", "2",
+                          "--master-addr", "127.0.0.1", "--master-port", str(port),
+                          os.path.join(root, "tests", "dist_partition_worker.py")],
+                         capture_output=True, text=True, cwd=root, timeout=600)
+    assert out.returncode == 0, out.stdout[-2000:] + out.stderr[-2000:]
+    lines = [json.loads(l) for l in out.stdout.splitlines() if l.startswith("{")]
+    assert sorted(l["rank"] for l in lines) == [0, 1]
+    assert lines[0]["f"] == lines[1]["f"] and lines[0]["grad"] == lines[1]["grad"]
+    assert all(l["ok"] for l in lines), lines
