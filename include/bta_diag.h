@@ -59,12 +59,19 @@ BTA_API int bta_diag_ktime_end(double* ms, double* flop, double* bytes, long lon
  *   BTA_OPT_TILE_THRESH (BTA_TILE_THRESH), BTA_OPT_TILE_WAVES (BTA_TILE_WAVES): the GEMM tile rule (process-global):
  *                                      launches of fewer 128x128 tiles than the threshold (180) use 64x64 tiles, and
  *                                      (waves = 1) so do launches whose last wave of 128x128 tiles would be mostly empty
+ *   BTA_OPT_PDL (BTA_PDL)              1 (default): the latency-bound kernels (32x32-tile GEMMs, POTRF leaves) are
+ *                                      launched programmatically (they start while their predecessor drains and wait
+ *                                      at griddepcontrol.wait); 0: plain launches.  Process-global.
+ *   BTA_OPT_ROWS (BTA_ROWS)            1 (default): the arrow / right-hand-side rows of the forward steps and the trace
+ *                                      contractions of the backward steps run on a third stream per chain (factor
+ *                                      mode), off the chain's dependent launch sequence; 0: in line
  *   BTA_OPT_PARTITIONS (BTA_PARTITIONS) >= 2: inla_value_and_grad uses the paper's time-domain partitioning with that
  *                                      many partitions inside the GPU (include/bta.h, "Time-domain partitioning");
  *                                      0 (default): the two-way elimination.  Factor mode only.
  * Returns BTA_ERR_ARG for an unknown option.  Cached CUDA graphs are dropped. */
 enum { BTA_OPT_TWIST = 0, BTA_OPT_LANES = 1, BTA_OPT_SPLIT = 2, BTA_OPT_GRAPH = 3, BTA_OPT_SERIAL = 4,
-       BTA_OPT_PIPELINE = 5, BTA_OPT_TILE_THRESH = 6, BTA_OPT_TILE_WAVES = 7, BTA_OPT_PARTITIONS = 8 };
+       BTA_OPT_PIPELINE = 5, BTA_OPT_TILE_THRESH = 6, BTA_OPT_TILE_WAVES = 7, BTA_OPT_PARTITIONS = 8, BTA_OPT_PDL = 9,
+       BTA_OPT_ROWS = 10 };
 BTA_API int bta_set_option(bta_ctx* ctx, int option, int value);
 BTA_API int bta_get_option(const bta_ctx* ctx, int option);
 

@@ -134,7 +134,7 @@ class Blocks:
 
 BTA_PRIOR, BTA_COND = 0, 1
 BTA_STORE_FACTOR, BTA_STORE_CARRY, BTA_STORE_HOST = 0, 1, 2
-OPT_TWIST, OPT_LANES, OPT_SPLIT, OPT_GRAPH, OPT_SERIAL, OPT_PIPELINE, OPT_TILE_THRESH, OPT_TILE_WAVES, OPT_PARTITIONS = range(9)
+OPT_TWIST, OPT_LANES, OPT_SPLIT, OPT_GRAPH, OPT_SERIAL, OPT_PIPELINE, OPT_TILE_THRESH, OPT_TILE_WAVES, OPT_PARTITIONS, OPT_PDL, OPT_ROWS = range(11)
 STAGES = ("assemble", "fwd_Qc", "bwd_Qc", "fwd_Qp", "bwd_Qp", "scalars", "total")
 
 

@@ -632,6 +632,9 @@ int enqueue_gradient_twisted(bta_ctx* c, void* ws, cudaStream_t s0, bool timed, 
     for (int q = 0; q < 2; ++q) {
       if (c->opt.split) ch[m][q].xs = c->s_x[2 * m + q];
       ch[m][q].pipe_ev = c->ev_pipe[2 * m + q];
+      // rows stream: pays where a step is latency-bound (measured: config 0 -11 %, config 1 -10 %; at b = 2304 the
+      // extra concurrency costs 3 %), so only up to the size where the whole gradient is graph-replayed
+      if (c->opt.rows && md.b <= 1024) ch[m][q].rs = c->s_r[2 * m + q];
     }
 
   // ---- assemble: D (all blocks), arrow/rhs rows, tip on the up stream; coupling blocks per sub-chain

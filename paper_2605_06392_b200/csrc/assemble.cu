@@ -28,32 +28,46 @@ __global__ void theta_prep_kernel(const double* __restrict__ theta, DevParams* _
       }
 }
 
-// kind 0: D_t (lower triangle + diagonal, strict upper = 0; + tau cnt on the diagonal for Q_c);  kind 1: B_t.
-__global__ void __launch_bounds__(256) assemble_blocks_kernel(ModelDims md, const DevParams* __restrict__ P, int kind,
-                                                              int cond, const double* __restrict__ cnt,
-                                                              double* __restrict__ out, long long stride, int t0,
-                                                              int tdir, int tr) {
-  // block z of the launch is global block t0 + tdir * z; tr: write the transposed block (B_t^T)
-  const int j = blockIdx.x * 256 + threadIdx.x, i = blockIdx.y, t = t0 + tdir * (int)blockIdx.z;
-  if (j >= md.b) return;
+// Dense blocks from stencils.  kind 0: D_t (lower triangle + diagonal, strict upper = 0; + tau cnt on the diagonal for
+// Q_c);  kind 1: B_t.  Block z of a launch is global block t0 + tdir * z; tr: the transposed block (B_t^T).
+// Written as a stencil band into ZEROED memory: one thread per (row i, sub-block column vj, stencil
+// entry q of the 13-point pattern |dy| + |dx| <= 2) -- 13 k b entries per block instead of b^2 predicate evaluations;
+// the zeros come from a memset at the full HBM write rate.
+__global__ void __launch_bounds__(256) assemble_band_kernel(ModelDims md, const DevParams* __restrict__ P, int kind,
+                                                            int cond, const double* __restrict__ cnt,
+                                                            double* __restrict__ out, long long stride, int t0, int tdir,
+                                                            int tr) {
+  const long long e = (long long)blockIdx.x * 256 + threadIdx.x;
+  const int per_row = 13 * md.k;
+  if (e >= (long long)md.b * per_row) return;
+  const int t = t0 + tdir * (int)blockIdx.y;
+  const int i = (int)(e / per_row), r = (int)(e % per_row), vj = r / 13, q = r % 13;
+  // q -> (dy, dx): rows dy = -2 (1 entry), -1 (3), 0 (5), 1 (3), 2 (1)
+  int dy, dx;
+  if (q == 0) { dy = -2; dx = 0; }
+  else if (q < 4) { dy = -1; dx = q - 2; }
+  else if (q < 9) { dy = 0; dx = q - 6; }
+  else if (q < 12) { dy = 1; dx = q - 10; }
+  else { dy = 2; dx = 0; }
+  const int vi = i / md.ns, si = i % md.ns, yi = si / md.g, xi = si % md.g;
+  const int yj = yi + dy, xj = xi + dx;
+  if (yj < 0 || yj >= md.g || xj < 0 || xj >= md.g) return;
+  const int j = vj * md.ns + yj * md.g + xj;
+  // (i, j) index the block as the sweeps see it; the matrix entry is (ii, jj) (transposed coupling blocks swap them)
+  if (kind == 0 && j > i) return;
+  const int vii = tr ? vj : vi, vjj = tr ? vi : vj;
+  const int yii = tr ? yj : yi, xii = tr ? xj : xi, yjj = tr ? yi : yj, xjj = tr ? xi : xj;
+  double kv[3], mw[3];
+  st_K(md.g, md.h, yii, xii, yjj, xjj, kv);
+  if (kind == 0)
+    st_Mdiag(md.nt, t, mw);
+  else
+    st_Moff(mw);
   double v = 0.0;
-  if (kind == 1 || j <= i) {
-    const int ii = tr ? j : i, jj = tr ? i : j;
-    const int vi = ii / md.ns, si = ii % md.ns, vj = jj / md.ns, sj = jj % md.ns;
-    const int yi = si / md.g, xi = si % md.g, yj = sj / md.g, xj = sj % md.g;
-    if (abs(yi - yj) + abs(xi - xj) <= 2) {
-      double kv[3], mw[3];
-      st_K(md.g, md.h, yi, xi, yj, xj, kv);
-      if (kind == 0)
-        st_Mdiag(md.nt, t, mw);
-      else
-        st_Moff(mw);
 #pragma unroll
-      for (int c = 0; c < 3; ++c) v += mw[c] * P->W[c][vi][vj] * kv[c];
-    }
-    if (kind == 0 && cond && i == j) v += P->tau[vi] * cnt[(long long)t * md.b + i];
-  }
-  out[(long long)blockIdx.z * stride + (long long)i * md.b + j] = v;
+  for (int c = 0; c < 3; ++c) v += mw[c] * P->W[c][vii][vjj] * kv[c];
+  if (kind == 0 && cond && i == j) v += P->tau[vi] * cnt[(long long)t * md.b + i];
+  out[(long long)blockIdx.y * stride + (long long)i * md.b + j] = v;
 }
 
 __global__ void assemble_arrow_kernel(ModelDims md, const DevParams* __restrict__ P, int cond,
@@ -237,19 +251,15 @@ cudaError_t launch_assemble(bta_ctx* c, int which, double* D, long long d_stride
                             double* rhs_tip, int rhs_tip_stride, cudaStream_t st) {
   const ModelDims& md = c->md;
   const int cond = which == BTA_COND;
-  const double bb8 = 8.0 * md.b * (double)md.b;
-  KTimeScope kt(BTA_KC_ASSEMBLE, st, 0.0,
-                (D ? bb8 * md.nt : 0.0) + (B ? bb8 * (md.nt - 1) : 0.0) + (C ? 8.0 * md.a * (double)md.b * md.nt : 0.0));
-  dim3 gx((md.b + 255) / 256, md.b, md.nt);
   if (D) {
-    assemble_blocks_kernel<<<gx, 256, 0, st>>>(md, c->P, 0, cond, c->cnt, D, d_stride, 0, 1, 0);
-    BTA_COUNT(c);
+    cudaError_t e = launch_assemble_seq(c, which, 0, 0, 1, md.nt, 0, D, d_stride, st);
+    if (e != cudaSuccess) return e;
   }
   if (B && md.nt > 1) {
-    dim3 gb((md.b + 255) / 256, md.b, md.nt - 1);
-    assemble_blocks_kernel<<<gb, 256, 0, st>>>(md, c->P, 1, cond, c->cnt, B, b_stride, 0, 1, 0);
-    BTA_COUNT(c);
+    cudaError_t e = launch_assemble_seq(c, which, 1, 0, 1, md.nt - 1, 0, B, b_stride, st);
+    if (e != cudaSuccess) return e;
   }
+  KTimeScope kt(BTA_KC_ASSEMBLE, st, 0.0, C ? 8.0 * md.a * (double)md.b * md.nt : 0.0);
   if (C || rhs) {
     dim3 ga((md.b + 255) / 256, md.nt);
     assemble_arrow_kernel<<<ga, 256, 0, st>>>(md, c->P, cond, c->zsum, c->ysum, C, c_stride, rhs, rhs_stride);
@@ -271,10 +281,22 @@ cudaError_t launch_assemble_seq(bta_ctx* c, int which, int kind, int t0, int tdi
                                 double* out, long long stride, cudaStream_t st) {
   if (count <= 0) return cudaSuccess;
   const ModelDims& md = c->md;
-  dim3 g1((md.b + 255) / 256, md.b, count);
-  KTimeScope kt(BTA_KC_ASSEMBLE, st, 0.0, 8.0 * md.b * (double)md.b * count);
-  assemble_blocks_kernel<<<g1, 256, 0, st>>>(md, c->P, kind, which == BTA_COND, c->cnt, out, stride, t0, tdir,
-                                             transpose);
+  const long long bb = (long long)md.b * md.b;
+  KTimeScope kt(BTA_KC_ASSEMBLE, st, 0.0, 8.0 * (double)bb * count);
+  // zeros at the memset rate (contiguous blocks: one call), then the stencil band
+  if (count == 1 || stride == bb || stride == -bb) {
+    double* lo = (stride < 0) ? out + (long long)(count - 1) * stride : out;
+    cudaError_t e = cudaMemsetAsync(lo, 0, (size_t)bb * count * sizeof(double), st);
+    if (e != cudaSuccess) return e;
+  } else {
+    for (int z = 0; z < count; ++z) {
+      cudaError_t e = cudaMemsetAsync(out + (long long)z * stride, 0, (size_t)bb * sizeof(double), st);
+      if (e != cudaSuccess) return e;
+    }
+  }
+  const long long per_block = (long long)md.b * 13 * md.k;
+  dim3 g1((unsigned)((per_block + 255) / 256), count);
+  assemble_band_kernel<<<g1, 256, 0, st>>>(md, c->P, kind, which == BTA_COND, c->cnt, out, stride, t0, tdir, transpose);
   BTA_COUNT(c);
   return cudaGetLastError();
 }

@@ -107,6 +107,26 @@ struct GemmArgs {
 
 extern long long g_tile_thresh;
 extern int g_tile_waves;
+// Programmatic dependent launch for the latency-bound kernels (32x32-tile GEMMs, POTRF leaves): the kernel is launched
+// with cudaLaunchAttributeProgrammaticStreamSerialization, starts while its predecessor in the stream drains, and waits
+// at `griddepcontrol.wait` before touching memory (BTA_OPT_PDL, process-global).
+extern int g_pdl;
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+template <class... KArgs, class... Args>
+cudaError_t launch_pdl(void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, Args... args) {
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = grid;
+  cfg.blockDim = block;
+  cfg.dynamicSmemBytes = smem;
+  cfg.stream = st;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  at[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = at;
+  cfg.numAttrs = 1;
+  return cudaLaunchKernelEx(&cfg, kern, KArgs(args)...);
+}
 cudaError_t launch_gemm(const GemmArgs& g, cudaStream_t st);
 bool gemm_uses_small_tiles(const GemmArgs& g);  // the 64x64-tile configuration (few CTAs)
 
@@ -170,6 +190,7 @@ struct Options {
   int graph = -1;     // CUDA-graph replay from the second call on: -1 = by size (b <= 1024), 0 off, 1 on
   int serial = 0;     // both matrices on one stream, single chain (exclusive per-stage times)
   int pipeline = 1;   // forward sweeps: start the next block's factorisation under the tail of this block's products
+  int rows = 1;       // arrow / rhs rows and trace contractions on a third stream per chain (factor mode)
   int partitions = 0; // >= 2: time-domain partitioning with that many partitions and a reduced system (partition.cu)
 };
 
@@ -204,8 +225,9 @@ struct bta_ctx {
   size_t host_bytes;
   cudaStream_t s_copy[4];            // its copy streams (one per sub-chain) and ring-slot events
   cudaEvent_t ev_ring[4][8];
-  cudaEvent_t ev_pipe[20][3];        // forward pipelining events per chain (sweep.h: Chain::pipe_ev)
-  cudaStream_t s_part[2][8], s_part_hi[2][8], s_part_x[2][8];  // partition.cu: streams per (matrix, partition), lazily
+  cudaEvent_t ev_pipe[20][5];        // per chain (sweep.h: Chain::pipe_ev): forward pipelining [0..2], trace parity [3..4]
+  cudaStream_t s_r[4];               // rows streams of the four chains (sweep.h: Chain::rs)
+  cudaStream_t s_part[2][8], s_part_hi[2][8], s_part_x[2][8], s_part_r[2][8];  // partition.cu: per (matrix, partition)
   cudaEvent_t ev_sw[256];            // lane-switch events, used round-robin
   unsigned ev_sw_next;
   long long launches;

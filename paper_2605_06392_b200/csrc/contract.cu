@@ -39,15 +39,20 @@ SmallLayout small_layout(const ModelDims& md) {
 
 namespace {
 
+// Sum over the 256 threads of a CTA in a fixed order: warp-shuffle butterflies, one shared-memory stage for the eight
+// warp sums, a second butterfly in warp 0.  The result is valid in warp 0 (the callers use thread 0).
 __device__ __forceinline__ double block_sum_256(double v, double* red) {
-  red[threadIdx.x] = v;
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = v;
   __syncthreads();
-  for (int o = 128; o > 0; o >>= 1) {
-    if (threadIdx.x < o) red[threadIdx.x] += red[threadIdx.x + o];
-    __syncthreads();
+  double r = 0.0;
+  if (threadIdx.x < 32) {
+    r = threadIdx.x < 8 ? red[threadIdx.x] : 0.0;
+#pragma unroll
+    for (int o = 4; o > 0; o >>= 1) r += __shfl_xor_sync(0xffffffffu, r, o);
   }
-  double r = red[0];
-  __syncthreads();
+  __syncthreads();  // `red` may be reused by the next sum
   return r;
 }
 

@@ -149,6 +149,10 @@ __global__ void __launch_bounds__(Cfg<BM, BN, WM, WN, A_KM, B_KM, BK, STAGES>::N
   using C_ = Cfg<BM, BN, WM, WN, A_KM, B_KM, BK, STAGES>;
   constexpr int NT = C_::NT;
   extern __shared__ __align__(16) double smem[];
+  if constexpr (BM == 32) {  // latency-bound class: launched programmatically (launch_cfg)
+    pdl_wait();
+    pdl_launch_dependents();
+  }
   unsigned long long* bar = reinterpret_cast<unsigned long long*>(smem);  // 16 bytes reserved
   double* As = smem + 2;
   double* Bs = As + STAGES * C_::A_ST;
@@ -408,6 +412,7 @@ cudaError_t launch_cfg(const GemmArgs& g, cudaStream_t st) {
   }
   KTimeScope kt(BM == 128 ? BTA_KC_GEMM_BIG : (BM == 64 ? BTA_KC_GEMM_SMALL : BTA_KC_GEMM_TINY), st,
                 g_ktime_on ? gemm_alg_flop(g) : 0.0, 0.0);
+  if (BM == 32 && g_pdl) return launch_pdl(kern, grid, dim3(C_::NT), (size_t)C_::SMEM, st, ga);
   kern<<<grid, C_::NT, C_::SMEM, st>>>(ga);
   return cudaGetLastError();
 }
@@ -425,6 +430,7 @@ cudaError_t launch_mode(const GemmArgs& g, cudaStream_t st) {
 }  // namespace
 
 // Tile-choice parameters (bta_set_option: BTA_OPT_TILE_THRESH / BTA_OPT_TILE_WAVES; process-global)
+int g_pdl = 1;
 long long g_tile_thresh = 180;  // fewer big tiles than this: 64x64 tiles (measured)
 int g_tile_waves = 1;           // 1: also prefer 64x64 tiles where the last wave of big tiles would be mostly empty
 

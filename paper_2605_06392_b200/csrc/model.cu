@@ -128,13 +128,16 @@ int create_impl(bta_ctx* c, const bta_model_desc* desc, const bta_obs* obs) {
     c->opt.serial = env("BTA_SERIAL_CHAINS", c->opt.serial);
     c->opt.pipeline = env("BTA_PIPELINE", c->opt.pipeline);
     c->opt.partitions = env("BTA_PARTITIONS", c->opt.partitions);
+    c->opt.rows = env("BTA_ROWS", c->opt.rows);
     g_tile_thresh = env("BTA_TILE_THRESH", (int)g_tile_thresh);
     g_tile_waves = env("BTA_TILE_WAVES", g_tile_waves);
+    g_pdl = env("BTA_PDL", g_pdl);
   }
   c->store_mode = BTA_STORE_FACTOR;
   for (auto& e : c->ev) BTA_CUDA_OK(cudaEventCreate(&e));
   for (auto& q : c->s_hi) BTA_CUDA_OK(cudaStreamCreateWithPriority(&q, cudaStreamNonBlocking, prio_hi));
   for (auto& q : c->s_x) BTA_CUDA_OK(cudaStreamCreateWithPriority(&q, cudaStreamNonBlocking, prio_lo));
+  for (auto& q : c->s_r) BTA_CUDA_OK(cudaStreamCreateWithPriority(&q, cudaStreamNonBlocking, prio_hi));
   for (auto& e : c->ev_sw) BTA_CUDA_OK(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
   for (auto& q : c->s_copy) BTA_CUDA_OK(cudaStreamCreateWithPriority(&q, cudaStreamNonBlocking, prio_lo));
   for (auto& q : c->ev_ring)
@@ -189,12 +192,14 @@ extern "C" int bta_destroy(bta_ctx* c) {
   for (auto& q : c->s_aux) kill_stream(q);
   for (auto& q : c->s_hi) kill_stream(q);
   for (auto& q : c->s_x) kill_stream(q);
+  for (auto& q : c->s_r) kill_stream(q);
   for (auto& q : c->s_copy) kill_stream(q);
   for (int m = 0; m < 2; ++m)
     for (int p = 0; p < 8; ++p) {
       kill_stream(c->s_part[m][p]);
       kill_stream(c->s_part_hi[m][p]);
       kill_stream(c->s_part_x[m][p]);
+      kill_stream(c->s_part_r[m][p]);
     }
   for (auto& q : c->ev_ring)
     for (auto& e : q) kill_event(e);
@@ -255,15 +260,17 @@ int* option_slot(bta_ctx* c, int option) {
     case BTA_OPT_SERIAL: return &c->opt.serial;
     case BTA_OPT_PIPELINE: return &c->opt.pipeline;
     case BTA_OPT_PARTITIONS: return &c->opt.partitions;
+    case BTA_OPT_ROWS: return &c->opt.rows;
   }
   return nullptr;
 }
 }  // namespace
 
 extern "C" int bta_set_option(bta_ctx* c, int option, int value) {
-  if (option == BTA_OPT_TILE_THRESH || option == BTA_OPT_TILE_WAVES) {  // process-global GEMM tile rule
+  if (option == BTA_OPT_TILE_THRESH || option == BTA_OPT_TILE_WAVES || option == BTA_OPT_PDL) {  // process-global
     if (option == BTA_OPT_TILE_THRESH) g_tile_thresh = value;
-    else g_tile_waves = value;
+    else if (option == BTA_OPT_TILE_WAVES) g_tile_waves = value;
+    else g_pdl = value;
     if (c)
       for (int q = 0; q < 2; ++q)
         if (c->graph_exec[q]) {

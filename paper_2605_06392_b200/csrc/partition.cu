@@ -128,6 +128,7 @@ int ensure_streams(bta_ctx* c, int P) {
       if (!c->s_part[m][p]) CKP(cudaStreamCreateWithPriority(&c->s_part[m][p], cudaStreamNonBlocking, lo));
       if (!c->s_part_hi[m][p]) CKP(cudaStreamCreateWithPriority(&c->s_part_hi[m][p], cudaStreamNonBlocking, hi));
       if (!c->s_part_x[m][p]) CKP(cudaStreamCreateWithPriority(&c->s_part_x[m][p], cudaStreamNonBlocking, lo));
+      if (!c->s_part_r[m][p]) CKP(cudaStreamCreateWithPriority(&c->s_part_r[m][p], cudaStreamNonBlocking, hi));
     }
   return BTA_OK;
 }
@@ -282,6 +283,7 @@ int PartRun::init(bta_ctx* ctx, void* ws, cudaStream_t stream, bool vonly, int r
       k.lanes_bwd = c->opt.lanes != 2;
       if (c->opt.split) k.xs = p < P ? c->s_part_x[m][p] : c->s_part_x[m][0];
       k.pipe_ev = c->ev_pipe[sp];
+      if (c->opt.rows && b <= 1024) k.rs = p < P ? c->s_part_r[m][p] : c->s_part_r[m][0];
       if (p < P) {  // interior chain of partition p
         const int i0 = pl.first_int(p);
         k.nt = pl.nint(p);

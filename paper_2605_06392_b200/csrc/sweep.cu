@@ -32,6 +32,12 @@ cudaStream_t lane(Chain* ch, cudaStream_t big, bool small) {
 }
 cudaError_t chain_to_big(Chain& ch, cudaStream_t big) {
   lane(&ch, big, false);
+  if (ch.rows_pending && ch.rs && ch.rs != big) {  // fold the rows stream in as well
+    cudaEvent_t e = ch.c->ev_sw[(ch.c->ev_sw_next++) % BTA_NSW];
+    cudaEventRecord(e, ch.rs);
+    cudaStreamWaitEvent(big, e, 0);
+  }
+  ch.rows_pending = false;
   return cudaGetLastError();
 }
 #define SS lane(lch, st, true)
@@ -217,9 +223,12 @@ cudaError_t chain_forward_step(Chain& ch, int t, cudaStream_t st) {
   }
   // stack rows: arrow rows (factor mode) then right-hand-side rows.
   //   R~_t = R_t - R^_{t-1} L_B{t-1}^T  (lines 4-5), done first: in carry mode L_B{t-1} is overwritten below
+  // Factor mode with a rows stream: all row work of this step is issued at its end on that stream (see there).
+  const bool defer_rows = ch.rs && P > 0 && ch.factor_blocks && !ch.carry && !ch.Rtmp && ch.Rin != ch.Rout &&
+                          !ch.arrow_given;
   const double* src = nullptr;
   int ld_src = 0;
-  if (P > 0) {
+  if (P > 0 && !defer_rows) {
     src = ch.Rin + t * ch.rin_stride;
     ld_src = ch.ld_rin;
     if (t == 0 && ch.Rin == ch.Rout) {  // in-place factor: the stack product below must not alias its input
@@ -276,7 +285,7 @@ cudaError_t chain_forward_step(Chain& ch, int t, cudaStream_t st) {
     }
   }
   TM(1);
-  if (P > 0) {
+  if (P > 0 && !defer_rows) {
     //   R^_t = R~_t X_t^T
     double* Rh = ch.Rout + t * ch.rout_stride;
     CK(launch_skinny_nt(P, b, b, src, ld_src, Dt, b, 1, 1.0, 0.0, nullptr, 0, Rh, ch.ld_rout, SS));
@@ -350,11 +359,38 @@ cudaError_t chain_forward_step(Chain& ch, int t, cudaStream_t st) {
     else
       CK(launch_gemm(G(GEMM_NT, b, b, b, -1.0, LB, b, LF, b, 0.0, f.Bse, b, KLO_ZERO, KHI_K, OUT_FULL), SB));
     c->launches += 3;
-    if (P > 0) {
+    if (P > 0 && !defer_rows) {
       CK(launch_skinny_nt(P, b, b, ch.Rout + t * ch.rout_stride, ch.ld_rout, LF, b, 0, -1.0, 1.0, f.Rs, f.ld_rs, f.Rs,
                           f.ld_rs, SS));
       BTA_COUNT(c);
     }
+  }
+  if (defer_rows) {
+    // everything this step produced (X_t, L_Bt, L_Ft) is complete in the order of the chain's current lane
+    cudaStream_t cur = lane(lch, st, ch.on_small), rs = ch.rs;
+    cudaEvent_t e = c->ev_sw[(c->ev_sw_next++) % BTA_NSW];
+    CK(cudaEventRecord(e, cur));
+    CK(cudaStreamWaitEvent(rs, e, 0));
+    double* Rt = ch.Rin + t * ch.rin_stride;
+    double* Rh = ch.Rout + t * ch.rout_stride;
+    if (t > 0) {
+      CK(launch_skinny_nt(P, b, b, ch.Rout + (t - 1) * ch.rout_stride, ch.ld_rout, ch.Bout + (t - 1) * ch.b_stride, b, 0,
+                          -1.0, 1.0, Rt, ch.ld_rin, Rt, ch.ld_rin, rs));
+      BTA_COUNT(c);
+    }
+    CK(launch_skinny_nt(P, b, b, Rt, ch.ld_rin, Dt, b, 1, 1.0, 0.0, nullptr, 0, Rh, ch.ld_rout, rs));
+    BTA_COUNT(c);
+    if (a > 0 && ch.arrow_rows) {
+      CK(launch_small_nt(a, P, b, Rh, ch.ld_rout, Rh, ch.ld_rout, -1.0, ch.Tt, ldt, rs));
+      BTA_COUNT(c);
+    }
+    if (ch.fill) {
+      Fill& f = *ch.fill;
+      CK(launch_skinny_nt(P, b, b, Rh, ch.ld_rout, f.LF + t * f.lf_stride, b, 0, -1.0, 1.0, f.Rs, f.ld_rs, f.Rs, f.ld_rs,
+                          rs));
+      BTA_COUNT(c);
+    }
+    ch.rows_pending = true;
   }
   return cudaSuccess;
 }
@@ -362,6 +398,7 @@ cudaError_t chain_forward_step(Chain& ch, int t, cudaStream_t st) {
 cudaError_t chain_forward_end(Chain& ch, cudaStream_t st) {
   Chain* lch = &ch;
   bta_ctx* c = ch.c;
+  if (ch.rows_pending) CK(chain_to_big(ch, st));  // the tip accumulator is complete
   const int b = ch.b, nt = c->md.nt, a = ch.a;  // the tip sits after all nt blocks, whatever this chain's length
   if (a > 0) {
     CK(launch_tip(ch.Tt, a, ch.nr, ch.tip_chol ? 1 : 0, ch.LT, ch.zT, ch.xT, ch.ZT,
@@ -476,6 +513,12 @@ cudaError_t chain_backward_step(Chain& ch, int t, cudaStream_t st) {
       c->launches += 2;
     }
     if (!ch.selinv) return cudaSuccess;
+    // (not in carry mode: there Z_B sits in the one L_B buffer that the next step rebuilds)
+    const bool defer_tr = ch.contract && ch.rs && ch.pipe_ev && !ch.carry;
+    if (defer_tr && ch.tr_armed[t & 1]) {  // Z_D / Z_C buffers of this parity: their traces (two steps ago) are done
+      CK(cudaStreamWaitEvent(st, ch.pipe_ev[3 + (t & 1)], 0));
+      if (ch.hi) CK(cudaStreamWaitEvent(ch.hi, ch.pipe_ev[3 + (t & 1)], 0));
+    }
     // ---- selected inversion (R10), tensor-friendly form:  G = L_B X,  E = L_C X,
     //      Z_B = -Z_D{t+1} G - Z_C{t+1}^T E,  Z_C = -Z_C{t+1} G - Z_T E,  Z_D = X^T X - Z_B^T G - Z_C^T E
     double* ZDcur = (t & 1) ? ch.W2 : ch.W3;
@@ -552,10 +595,23 @@ cudaError_t chain_backward_step(Chain& ch, int t, cudaStream_t st) {
       BTA_COUNT(c);
     }
     if (ch.contract) {
-      CK(launch_trace_stencil(c, ch.chain, (int)tg, 0, ZDcur, b, SS));
-      if (has_next && ch.tB(t) >= 0) CK(launch_trace_stencil(c, ch.chain, ch.tB(t), 1, LB, b, SS));
-      if (fl && t == 0 && fl->tb_first >= 0) CK(launch_trace_stencil(c, ch.chain, fl->tb_first, 1, LFt, b, SS));
-      if (arrow) CK(launch_noise_trace(c, (int)tg, ZDcur, b, ZCcur, b, SS));
+      cudaStream_t ts = SS;
+      if (defer_tr) {  // on the rows stream, after everything this step wrote
+        cudaStream_t cur = lane(lch, st, lch ? ch.on_small : false);
+        cudaEvent_t e = c->ev_sw[(c->ev_sw_next++) % BTA_NSW];
+        CK(cudaEventRecord(e, cur));
+        CK(cudaStreamWaitEvent(ch.rs, e, 0));
+        ts = ch.rs;
+      }
+      CK(launch_trace_stencil(c, ch.chain, (int)tg, 0, ZDcur, b, ts));
+      if (has_next && ch.tB(t) >= 0) CK(launch_trace_stencil(c, ch.chain, ch.tB(t), 1, LB, b, ts));
+      if (fl && t == 0 && fl->tb_first >= 0) CK(launch_trace_stencil(c, ch.chain, fl->tb_first, 1, LFt, b, ts));
+      if (arrow) CK(launch_noise_trace(c, (int)tg, ZDcur, b, ZCcur, b, ts));
+      if (defer_tr) {
+        CK(cudaEventRecord(ch.pipe_ev[3 + (t & 1)], ch.rs));
+        ch.tr_armed[t & 1] = true;
+        ch.rows_pending = true;
+      }
     }
     if (ch.selinv_inplace) {
       CK(cudaMemcpyAsync(ch.Dp(t), ZDcur, bb * sizeof(double), cudaMemcpyDeviceToDevice, SB));

@@ -56,6 +56,13 @@ struct Chain {
   // diagonal block has its Schur update, [1] L_B of this step is complete, [2] all products of this step are done.
   cudaEvent_t* pipe_ev = nullptr;
   bool pipe_armed = false;     // the previous step recorded pipe_ev (its products were issued in split form)
+  // Rows stream: the arrow / right-hand-side rows of a forward step (R~_t, R^_t = [L_Ct; z_t], tip updates) and the trace
+  // contractions of a backward step do not feed the next block's factorisation or selected inversion, so (factor mode)
+  // they run on this third stream, one step behind the chain, instead of sitting in its dependent launch sequence.
+  // pipe_ev[3], [4]: the contractions of an even / odd backward step have read their Z buffers.
+  cudaStream_t rs = nullptr;
+  bool rows_pending = false;   // work is outstanding on rs (chain_to_big joins it)
+  bool tr_armed[2] = {false, false};
   // Host-staged carries (BTA_STORE_HOST): the diagonal-block slots are a ring of `ring` device blocks
   // (local block s lives in slot s % ring); each carry D_s - S_{s-1} is copied to pinned host memory (hostD + s b^2) on
   // the copy stream `cs` during the forward sweep and streamed back `ring` steps ahead in the backward sweep.
