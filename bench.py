@@ -246,7 +246,9 @@ def kernel_breakdown(M, theta, peak_tf, hbm_gbs):
     bwd = st["bwd_Qc"] + st["bwd_Qp"]
     return kt, table, {"stage_ms_exclusive": st, "kernel_ms_total": tot,
                        "beta_bwd_over_fwd": bwd / fwd if fwd > 0 else None,
-                       "note": "single stream, single chain per matrix (BTA_OPT_SERIAL): stages do not overlap"}
+                       "note": "single stream, single chain per matrix (BTA_OPT_SERIAL), the two matrices' steps "
+                               "interleaved: fwd_Qc and fwd_Qp both span the forward phase of BOTH matrices, likewise "
+                               "bwd_*; phases do not overlap each other"}
 
 
 def run_ours(args):
@@ -418,13 +420,18 @@ def run_ours(args):
         v1.record()
         torch.cuda.synchronize()
         t_eval = v0.elapsed_time(v1) / nfd
+        fwd_ph, bwd_ph = stage_acc.get("fwd_Qc", 0.0), stage_acc.get("bwd_Qc", 0.0)
         line["fd_compare"] = {"t_eval_ms": t_eval, "t_ad_ms": ms_step, "c_ad": ms_step / t_eval,
                               "fd_gradient_ms": (2 * d + 1) * t_eval,
                               "speedup_ad_vs_fd": (2 * d + 1) * t_eval / ms_step,
-                              "beta_bwd_over_fwd": bd["beta_bwd_over_fwd"] if bd else None,
-                              "note": "FD gradient = (2d+1) x inla_value (Eq. 2); beta from the exclusive stage times "
-                                      "of the serial breakdown step; paper: 4.2-7.9x per-gradient speedup, c_AD "
-                                      "2.3-3.9, beta 1.3-2.4 on GH200 (context only, BASELINE.md)"}
+                              "beta_phases": (bwd_ph / fwd_ph) if fwd_ph > 0 else None,
+                              "beta_serial": bd["beta_bwd_over_fwd"] if bd else None,
+                              "beta_by_flops": 13.0 / 8.0,
+                              "note": "FD gradient = (2d+1) x inla_value (Eq. 2); beta_phases = backward phase / forward "
+                                      "phase of the timed step (all four chains run each phase together; null when the "
+                                      "step is a graph replay), beta_serial = the same ratio in the serial breakdown "
+                                      "step; paper: 4.2-7.9x per-gradient speedup, c_AD 2.3-3.9, beta 1.3-2.4 on GH200 "
+                                      "(context only, BASELINE.md)"}
     # ---- storage policy a7: the same step in the other store mode (workspace and time side by side)
     if not args.no_store_compare and args.store == "factor" and args.partitions is None:
         M.bta_set_store_mode(1)
