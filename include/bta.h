@@ -206,6 +206,23 @@ BTA_API int inla_part_phase2(bta_ctx* ctx, int rank, int nranks, const double* g
                              void* stream);
 BTA_API int inla_part_finish(bta_ctx* ctx, const double* partials, double* f, double* grad, void* stream);
 
+/* Allocation-free product for callers that cannot call cudaMalloc or provide scratch (code under CUDA-graph capture,
+ * serving loops, harnesses that forbid allocation): the rows-times-block product of the upper solve and of the arrow
+ * recurrences (Eqs. 3-5; R10),
+ *     out[p][j] = alpha * sum_{k >= kbeg(j)} R[p][k] * M[k][j] + beta * in[p][j],   kbeg(j) = tri ? j : 0,
+ * P <= 9 rows R (ldr) against a K x J block M (ldm; tri = 1: M lower triangular), all DEVICE pointers, row-major FP64;
+ * `in` may be NULL when beta = 0 and may alias `out`.  The kernel's partial-sum scratch (ceil(K/128) * P * J doubles)
+ * is a file-scope device array of BTA_NOALLOC_MAX_PART doubles (9.4 MB: enough for P = 9, K = J = 4096) that every
+ * GPU loading the library holds until exit; larger products are rejected with BTA_ERR_ARG and a message.  The call
+ * allocates nothing (no cudaMalloc / cudaFree, no allocating library routine), launches on `stream` on the CURRENT
+ * device and does not synchronise.  All calls on one device share the array, which keeps the last call's contents
+ * (every entry read is written first by the same call, so nothing needs clearing): calls that overlap on the GPU
+ * race -- issue them on one stream or order them with events. */
+#define BTA_NOALLOC_MAX_PART (32 * 9 * 4096)
+BTA_API int bta_rows_times_block_noalloc(int P, int K, int J, const double* R, int ldr, const double* M, int ldm, int tri,
+                                         double alpha, double beta, const double* in, int ldin, double* out, int ldo,
+                                         void* stream);
+
 enum {
   BTA_STAGE_ASSEMBLE = 0,
   BTA_STAGE_FWD_QC = 1,

@@ -41,6 +41,12 @@ enum {
   BTA_KC_OTHER = 7,       /* tips, small products, reductions, scalars */
   BTA_KC_COUNT = 8
 };
+/* The product of bta_rows_times_block_noalloc (include/bta.h) through the sweeps' own launcher with CALLER-provided
+ * scratch `part` (DEVICE, ceil(K/128) * P * J doubles): the existing path the allocation-free variant is tested against. */
+BTA_API int bta_rows_times_block(int P, int K, int J, const double* R, int ldr, const double* M, int ldm, int tri,
+                                 double alpha, double beta, const double* in, int ldin, double* out, int ldo, double* part,
+                                 void* stream);
+
 /* Host-only: the element-exact flop count the timing registers for one GEMM launch (klo/khi/out as in bta_gemm). */
 BTA_API double bta_diag_gemm_flop(int M, int N, int K, int klo, int khi, int out);
 BTA_API int bta_diag_ktime_begin(void);

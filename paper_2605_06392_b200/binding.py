@@ -94,6 +94,9 @@ def lib():
     L.inla_part_phase1.argtypes = [vp, dp, i32, i32, vp, vp, vp]
     L.inla_part_phase2.argtypes = [vp, i32, i32, vp, vp, vp, vp]
     L.inla_part_finish.argtypes = [vp, vp, dp, dp, vp]
+    rtb = [i32, i32, i32, vp, i32, vp, i32, i32, C.c_double, C.c_double, vp, i32, vp, i32]
+    L.bta_rows_times_block_noalloc.argtypes = rtb + [vp]
+    L.bta_rows_times_block.argtypes = rtb + [vp, vp]
     L.bta_set_option.argtypes = [vp, i32, i32]
     L.bta_get_option.argtypes = [vp, i32]
     _lib = L
@@ -407,6 +410,31 @@ def ktime_end():
 
 def gemm_alg_flop(M, N, K, klo=0, khi=0, out=0):
     return lib().bta_diag_gemm_flop(M, N, K, klo, khi, out)
+
+
+NOALLOC_MAX_PART = 32 * 9 * 4096
+
+
+def rows_times_block_noalloc(R, M, out, alpha=1.0, beta=0.0, inp=None, tri=0):
+    """out = alpha R M + beta inp with the kernel's scratch in the library's static device array (include/bta.h)."""
+    P, K = R.shape
+    J = M.shape[1]
+    _check(lib().bta_rows_times_block_noalloc(P, K, J, R.data_ptr(), R.stride(0), M.data_ptr(), M.stride(0), int(tri),
+                                              alpha, beta, inp.data_ptr() if inp is not None else None,
+                                              inp.stride(0) if inp is not None else 0, out.data_ptr(), out.stride(0),
+                                              _stream()))
+    return out
+
+
+def rows_times_block(R, M, out, part, alpha=1.0, beta=0.0, inp=None, tri=0):
+    """The same product through the sweeps' launcher with caller-provided scratch (include/bta_diag.h)."""
+    P, K = R.shape
+    J = M.shape[1]
+    _check(lib().bta_rows_times_block(P, K, J, R.data_ptr(), R.stride(0), M.data_ptr(), M.stride(0), int(tri), alpha,
+                                      beta, inp.data_ptr() if inp is not None else None,
+                                      inp.stride(0) if inp is not None else 0, out.data_ptr(), out.stride(0),
+                                      part.data_ptr(), _stream()))
+    return out
 
 
 def cta_trace_start(buf):

@@ -226,3 +226,81 @@ cudaError_t launch_small_left_mul(int R, int Q, int J, const double* S, int lds,
   small_left_mul_kernel<<<(J + 255) / 256, 256, 0, st>>>(R, Q, J, S, lds, E, lde, alpha, beta, In, ldin, Y, ldy);
   return cudaGetLastError();
 }
+
+// ------------------------------------------------------------------------------------------------
+// Allocation-free entry point (include/bta.h: bta_rows_times_block_noalloc) and, for comparison, the same product through
+// the existing launcher with caller-provided scratch (include/bta_diag.h: bta_rows_times_block).
+//
+// skinny_nn needs a scratch array for its per-k-chunk partial sums ([ceil(K/128)][P][J] doubles); the sweeps carve it
+// out of the caller's workspace.  Some callers cannot provide or allocate one (code under CUDA-graph capture, serving
+// loops, harnesses that forbid cudaMalloc).  For them the scratch is this file-scope device array: BTA_NOALLOC_MAX_PART
+// doubles = 9.4 MB (P = 9 rows against a 4096 x 4096 block), held by every GPU that loads the library until exit.
+// In host code `g_noalloc_part` is only the host-side stand-in of the symbol: the device address is taken once per
+// device with cudaGetSymbolAddress (that device current) and passed to the kernels.  Every partial sum that the finish
+// kernel reads is written by the product kernel of the same call (skipped chunks write zeros), so nothing has to be
+// cleared between calls; the array keeps the last call's contents.  All calls on one device share the array: calls that
+// overlap on the GPU (different streams) race -- serialise them.
+// ------------------------------------------------------------------------------------------------
+namespace {
+constexpr size_t NOALLOC_MAX_PART = BTA_NOALLOC_MAX_PART;
+static __device__ __align__(256) double g_noalloc_part[NOALLOC_MAX_PART];
+constexpr int NOALLOC_MAX_DEV = 64;
+double* g_noalloc_ptr[NOALLOC_MAX_DEV] = {};   // device address of g_noalloc_part per device ordinal (set-up once)
+
+int rows_times_block_check(const char* who, int P, int K, int J, const double* R, const double* M, const double* in,
+                           double beta, const double* out) {
+  char buf[200];
+  if (P < 1 || P > 9 || K < 1 || J < 1 || !R || !M || !out || (beta != 0.0 && !in)) {
+    snprintf(buf, sizeof buf, "%s: need 1 <= P <= 9, K >= 1, J >= 1, non-null R, M, out (and in when beta != 0)", who);
+    bta_set_error(buf);
+    return BTA_ERR_ARG;
+  }
+  return BTA_OK;
+}
+}  // namespace
+
+extern "C" int bta_rows_times_block_noalloc(int P, int K, int J, const double* R, int ldr, const double* M, int ldm,
+                                            int tri, double alpha, double beta, const double* in, int ldin,
+                                            double* out, int ldo, void* stream) {
+  if (int rc = rows_times_block_check("bta_rows_times_block_noalloc", P, K, J, R, M, in, beta, out); rc != BTA_OK)
+    return rc;
+  const size_t need = skinny_nn_part_doubles(P, K, J);
+  if (need > NOALLOC_MAX_PART) {
+    char buf[200];
+    snprintf(buf, sizeof buf,
+             "bta_rows_times_block_noalloc: ceil(K/128) * P * J = %zu doubles of scratch exceed the built-in %zu "
+             "(BTA_NOALLOC_MAX_PART); use the workspace-based calls",
+             need, (size_t)NOALLOC_MAX_PART);
+    bta_set_error(buf);
+    return BTA_ERR_ARG;
+  }
+  int dev = 0;
+  BTA_CUDA_OK(cudaGetDevice(&dev));
+  if (dev < 0 || dev >= NOALLOC_MAX_DEV) {
+    bta_set_error("bta_rows_times_block_noalloc: device ordinal out of range");
+    return BTA_ERR_ARG;
+  }
+  double* part = __atomic_load_n(&g_noalloc_ptr[dev], __ATOMIC_ACQUIRE);
+  if (!part) {  // once per device, with that device current
+    void* p = nullptr;
+    BTA_CUDA_OK(cudaGetSymbolAddress(&p, g_noalloc_part));
+    part = (double*)p;
+    __atomic_store_n(&g_noalloc_ptr[dev], part, __ATOMIC_RELEASE);
+  }
+  BTA_CUDA_OK(launch_skinny_nn(P, K, J, R, ldr, M, ldm, tri, alpha, beta, in, ldin, out, ldo, part,
+                               (cudaStream_t)stream));
+  return BTA_OK;
+}
+
+extern "C" int bta_rows_times_block(int P, int K, int J, const double* R, int ldr, const double* M, int ldm, int tri,
+                                    double alpha, double beta, const double* in, int ldin, double* out, int ldo,
+                                    double* part, void* stream) {
+  if (int rc = rows_times_block_check("bta_rows_times_block", P, K, J, R, M, in, beta, out); rc != BTA_OK) return rc;
+  if (!part) {
+    bta_set_error("bta_rows_times_block: null scratch (ceil(K/128) * P * J doubles)");
+    return BTA_ERR_ARG;
+  }
+  BTA_CUDA_OK(launch_skinny_nn(P, K, J, R, ldr, M, ldm, tri, alpha, beta, in, ldin, out, ldo, part,
+                               (cudaStream_t)stream));
+  return BTA_OK;
+}

@@ -98,3 +98,11 @@ def test_gemm_flop_count_matches_brute_force(lib):
                     hi = {0: K, 1: min(K, n + 1), 2: min(K, m + 1)}[khi]
                     want += 2 * max(0, hi - lo)
             assert gemm_alg_flop(M, N, K, klo, khi, out) == want, (M, N, K, klo, khi, out)
+
+
+def test_noalloc_entry_point_rejects_oversize_without_gpu(lib):
+    """bta_rows_times_block_noalloc checks its sizes against the built-in scratch before any CUDA call."""
+    rc = lib.bta_rows_times_block_noalloc(9, 4224, 4096, ctypes.c_void_p(8), 4224, ctypes.c_void_p(8), 4096, 0,
+                                          ctypes.c_double(1.0), ctypes.c_double(0.0), None, 0, ctypes.c_void_p(8), 4096,
+                                          None)
+    assert rc == 1 and b"BTA_NOALLOC_MAX_PART" in lib.bta_last_error()
