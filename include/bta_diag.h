@@ -47,6 +47,14 @@ BTA_API int bta_rows_times_block(int P, int K, int J, const double* R, int ldr, 
                                  double alpha, double beta, const double* in, int ldin, double* out, int ldo, double* part,
                                  void* stream);
 
+/* POTRF + TRTRI of one n x n block as the forward sweeps do it (Algorithm 1 line 3, in the
+ * inverse-diagonal form of DESIGN.md §5): A (DEVICE, row-major, leading dimension ld, SPD, lower triangle read, strict
+ * upper triangle zero as the assembly leaves it) is overwritten by X = chol(A)^-1 (lower triangular); diagL (DEVICE, n
+ * doubles, or NULL) receives diag(chol(A)).  T1, T2: DEVICE scratch blocks of the same shape as A, required for n > 128
+ * (the blocked recursion over 128 x 128 leaves).  Returns BTA_ERR_NOTSPD on a non-positive pivot (bta_last_pivot = its
+ * 1-based row); synchronises the stream.  Kernel-level test hook, not part of the hot path's boundary. */
+BTA_API int bta_diag_potrf_inv(bta_ctx* ctx, double* A, int ld, int n, double* T1, double* T2, double* diagL, void* stream);
+
 /* Host-only: the element-exact flop count the timing registers for one GEMM launch (klo/khi/out as in bta_gemm). */
 BTA_API double bta_diag_gemm_flop(int M, int N, int K, int klo, int khi, int out);
 BTA_API int bta_diag_ktime_begin(void);

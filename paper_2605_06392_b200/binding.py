@@ -97,6 +97,7 @@ def lib():
     rtb = [i32, i32, i32, vp, i32, vp, i32, i32, C.c_double, C.c_double, vp, i32, vp, i32]
     L.bta_rows_times_block_noalloc.argtypes = rtb + [vp]
     L.bta_rows_times_block.argtypes = rtb + [vp, vp]
+    L.bta_diag_potrf_inv.argtypes = [vp, vp, i32, i32, vp, vp, vp, vp]
     L.bta_set_option.argtypes = [vp, i32, i32]
     L.bta_get_option.argtypes = [vp, i32]
     _lib = L
@@ -365,6 +366,15 @@ class BtaModel:
 
     def last_pivot(self):
         return lib().bta_last_pivot(self._h)
+
+    def diag_potrf_inv(self, A, diagL=None):
+        """include/bta_diag.h: A (device, n x n, lower, SPD) -> chol(A)^-1 in place, as the forward sweeps do it."""
+        import torch
+        n = A.shape[0]
+        T1, T2 = torch.empty_like(A), torch.empty_like(A)
+        _check(lib().bta_diag_potrf_inv(self._h, A.data_ptr(), A.stride(0), n, T1.data_ptr(), T2.data_ptr(),
+                                        diagL.data_ptr() if diagL is not None else None, _stream()))
+        return A
 
 
 def fp64_peak(kind=0, iters=100000):

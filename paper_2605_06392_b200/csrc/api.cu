@@ -172,6 +172,18 @@ extern "C" int bta_factor_logdet(bta_ctx* c, bta_blocks io, int which, double* l
   return rc;
 }
 
+// include/bta_diag.h: the block factorisation of the forward sweeps alone (kernel tests and timing)
+extern "C" int bta_diag_potrf_inv(bta_ctx* c, double* A, int ld, int n, double* T1, double* T2, double* diagL,
+                                  void* stream) {
+  if (!c || !A || n <= 0 || ld < n) return bad("bta_diag_potrf_inv: null ctx or block, or bad sizes");
+  if (n > 128 && (!T1 || !T2)) return bad("bta_diag_potrf_inv: blocks above 128 rows need the scratch blocks T1, T2");
+  cudaStream_t st = (cudaStream_t)stream;
+  DeviceGuard guard(c->device);
+  BTA_CUDA_OK(cudaMemsetAsync(c->pivot_flag, 0xFF, sizeof(unsigned long long), st));
+  BTA_CUDA_OK(potrf_inv(c, nullptr, A, ld, 0, n, T1, T2, diagL, 0, st));
+  return check_pivot(c, st);
+}
+
 extern "C" int bta_solve(bta_ctx* c, bta_blocks Lf, int which, double* rhs, int nrhs, void* ws, void* stream) {
   if (!c || !ws || !rhs) return bad("bta_solve: null ctx, workspace or rhs");
   if (which != BTA_PRIOR && which != BTA_COND) return bad("bta_solve: bad `which`");

@@ -5,51 +5,62 @@
 #include "common.cuh"
 
 constexpr int NN_KCH = 128;
-constexpr int NT_RPW = 2;   // rows of M per warp in skinny_nt (8 warps per CTA)  // rows of M per CTA of skinny_nn (one partial sum each)
+constexpr int NT_RPW = 4;   // rows of M per warp in skinny_nt
+constexpr int NT_WARPS = 4; // warps per CTA in skinny_nt (16 rows of M per CTA)
 
 namespace {
 
 // out[p][j] = beta * in[p][j] + alpha * sum_{k < kend(j)} R[p][k] * M[j][k],  kend(j) = tri ? j+1 : K.
-// One warp per NT_RPW rows j of M (k contiguous -> coalesced); the R chunk is staged in shared memory.
+// One warp per NT_RPW rows j of M (k contiguous -> coalesced).  The R chunk is staged in shared memory and each staged
+// value is read into registers once per k-step and used for all NT_RPW rows (PT / NT_RPW shared loads per element of M
+// instead of PT), with the NT_RPW row loads of a k-step in flight together.
 template <int PT>
-__global__ void __launch_bounds__(256) skinny_nt_kernel(int P, int J, int K, const double* __restrict__ R, int ldr,
-                                                        const double* __restrict__ M, int ldm, int tri,
-                                                        double alpha, double beta, const double* in, int ldin,
-                                                        double* out, int ldo) {
+__global__ void __launch_bounds__(32 * NT_WARPS) skinny_nt_kernel(int P, int J, int K, const double* __restrict__ R,
+                                                                  int ldr, const double* __restrict__ M, int ldm,
+                                                                  int tri, double alpha, double beta, const double* in,
+                                                                  int ldin, double* out, int ldo) {
   // `in` and `out` may be the same buffer (in-place stack updates of the sweeps): no __restrict__ on them
-  constexpr int KC = 256, RPW = NT_RPW;
+  constexpr int KC = 256, RPW = NT_RPW, NT = 32 * NT_WARPS;
   __shared__ double Rs[PT * KC];
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const int jbase = blockIdx.x * (8 * RPW) + warp * RPW;
-  const int jmax_cta = min(J, (int)(blockIdx.x + 1) * (8 * RPW)) - 1;
+  const int jbase = blockIdx.x * (NT_WARPS * RPW) + warp * RPW;
+  const int jmax_cta = min(J, (int)(blockIdx.x + 1) * (NT_WARPS * RPW)) - 1;
   const int Kcta = tri ? min(K, jmax_cta + 1) : K;
   double acc[RPW][PT];
+  const double* mrow[RPW];
+  int kend[RPW];
 #pragma unroll
-  for (int r = 0; r < RPW; ++r)
+  for (int r = 0; r < RPW; ++r) {
+    const int j = jbase + r;
+    kend[r] = j < J ? (tri ? min(K, j + 1) : K) : 0;
+    mrow[r] = M + (long long)min(j, J - 1) * ldm;
 #pragma unroll
     for (int p = 0; p < PT; ++p) acc[r][p] = 0.0;
+  }
+  int kend_warp = 0;
+#pragma unroll
+  for (int r = 0; r < RPW; ++r) kend_warp = max(kend_warp, kend[r]);
   for (int k0 = 0; k0 < Kcta; k0 += KC) {
     __syncthreads();
-    for (int e = tid; e < PT * KC; e += 256) {
+    for (int e = tid; e < PT * KC; e += NT) {
       int p = e / KC, k = e % KC;
       Rs[e] = (p < P && k0 + k < Kcta) ? R[(long long)p * ldr + k0 + k] : 0.0;
     }
     __syncthreads();
+    if (k0 >= kend_warp) continue;  // every row of this warp ends before the chunk
+#pragma unroll 2
+    for (int q = 0; q < KC / 32; ++q) {
+      const int k = k0 + q * 32 + lane;
+      double m[RPW];
 #pragma unroll
-    for (int r = 0; r < RPW; ++r) {
-      const int j = jbase + r;
-      if (j >= J) continue;
-      const int kend = tri ? min(K, j + 1) : K;
-      const double* mrow = M + (long long)j * ldm;
+      for (int r = 0; r < RPW; ++r) m[r] = (k < kend[r]) ? mrow[r][k] : 0.0;
+      double rr[PT];
 #pragma unroll
-      for (int q = 0; q < KC / 32; ++q) {
-        const int k = k0 + q * 32 + lane;
-        if (k < kend) {
-          const double m = mrow[k];
+      for (int p = 0; p < PT; ++p) rr[p] = Rs[p * KC + q * 32 + lane];
 #pragma unroll
-          for (int p = 0; p < PT; ++p) acc[r][p] = fma(m, Rs[p * KC + q * 32 + lane], acc[r][p]);
-        }
-      }
+      for (int r = 0; r < RPW; ++r)
+#pragma unroll
+        for (int p = 0; p < PT; ++p) acc[r][p] = fma(m[r], rr[p], acc[r][p]);
     }
   }
 #pragma unroll
@@ -171,15 +182,15 @@ cudaError_t launch_skinny_nt(int P, int J, int K, const double* R, int ldr, cons
                              cudaStream_t st) {
   if (P <= 0 || J <= 0) return cudaSuccess;
   KTimeScope kt(BTA_KC_SKINNY, st, 2.0 * P * (double)J * K * (tri ? 0.5 : 1.0), 8.0 * (double)J * K * (tri ? 0.5 : 1.0));
-  dim3 grid((J + 8 * NT_RPW - 1) / (8 * NT_RPW));
+  dim3 grid((J + NT_WARPS * NT_RPW - 1) / (NT_WARPS * NT_RPW));
   if (P <= 1)
-    skinny_nt_kernel<1><<<grid, 256, 0, st>>>(P, J, K, R, ldr, M, ldm, tri, alpha, beta, in, ldin, out, ldo);
+    skinny_nt_kernel<1><<<grid, 32 * NT_WARPS, 0, st>>>(P, J, K, R, ldr, M, ldm, tri, alpha, beta, in, ldin, out, ldo);
   else if (P <= 4)
-    skinny_nt_kernel<4><<<grid, 256, 0, st>>>(P, J, K, R, ldr, M, ldm, tri, alpha, beta, in, ldin, out, ldo);
+    skinny_nt_kernel<4><<<grid, 32 * NT_WARPS, 0, st>>>(P, J, K, R, ldr, M, ldm, tri, alpha, beta, in, ldin, out, ldo);
   else if (P <= 9)
-    skinny_nt_kernel<9><<<grid, 256, 0, st>>>(P, J, K, R, ldr, M, ldm, tri, alpha, beta, in, ldin, out, ldo);
+    skinny_nt_kernel<9><<<grid, 32 * NT_WARPS, 0, st>>>(P, J, K, R, ldr, M, ldm, tri, alpha, beta, in, ldin, out, ldo);
   else if (P <= 16)
-    skinny_nt_kernel<16><<<grid, 256, 0, st>>>(P, J, K, R, ldr, M, ldm, tri, alpha, beta, in, ldin, out, ldo);
+    skinny_nt_kernel<16><<<grid, 32 * NT_WARPS, 0, st>>>(P, J, K, R, ldr, M, ldm, tri, alpha, beta, in, ldin, out, ldo);
   else
     return cudaErrorInvalidValue;
   return cudaGetLastError();

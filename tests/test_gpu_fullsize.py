@@ -9,7 +9,11 @@ block at b = 4096, so the full nt cannot be compared element by element in secon
 (iii) at the FULL nt, properties that hold at any size: the DCT closed form for log det Q_p and the Phase-C traces
      (pin P9), the sum rules P7/P8, the value identity P6, the residual Q_c x* = r on every row, the uniform-design
      closed form for log det Q_c and Phase A (pin P12), and the scalar assembly of f, grad f recomputed from the
-     returned intermediates.  The same properties are checked on the two extreme stand-ins (configs 5, 6)."""
+     returned intermediates.  The same properties are checked on the two extreme stand-ins (configs 5, 6);
+(iv) `test_full_model_vs_full_oracle`, gated by BTA_FULL_ORACLE=<config indices> because the oracle then takes minutes
+     (config 2: ~2.5 min, config 3: ~4 min, config 4: ~13 min and ~100 GB of host memory): the WHOLE model at the full
+     nt against the oracle, component by component like (i); the observed errors are written to
+     gpurun_out/full_oracle_parity_cfg<i>.txt (kept in profiles/r02_full_oracle_parity.md)."""
 import functools
 import os
 
@@ -83,6 +87,38 @@ def test_truncated_twisted_vs_oracle(idx, store):
     assert np.allclose(im["rss"], ref["rss"], rtol=1e-10, atol=1e-12)
     assert abs(im["quad_p"] - ref["quad_p"]) <= 1e-9 * abs(ref["quad_p"])
     assert _grad_ok(g, ref["grad"]), (g, ref["grad"])
+
+
+_FULL = [int(v) for v in os.environ.get("BTA_FULL_ORACLE", "").replace(",", " ").split()]
+
+
+@pytest.mark.skipif(not _FULL, reason="set BTA_FULL_ORACLE=\"2 3\" (config indices): the full-nt oracle takes minutes")
+@pytest.mark.parametrize("idx", _FULL or [2])
+def test_full_model_vs_full_oracle(idx):
+    """The whole config (full b AND full nt, the model bench.py times) against the oracle, per component."""
+    import time
+    model, obs, th = make_config(idx)
+    f, g, im = _run(model, obs, th)
+    t0 = time.perf_counter()
+    ref = O.value_and_grad(model, obs, th)
+    t_or = time.perf_counter() - t0
+    rel = lambda a, b: float(np.max(np.abs(np.asarray(a) - np.asarray(b))) / max(np.max(np.abs(np.asarray(b))), 1e-300))
+    gate = np.maximum(np.abs(ref["grad"]), 1e-3 * np.max(np.abs(ref["grad"])))
+    err = {"ld_p": rel(im["ld_p"], ref["ld_p"]), "ld_c": rel(im["ld_c"], ref["ld_c"]), "f": rel(f, ref["f"]),
+           "x": rel(im["x"], ref["x"]), "phaseA": rel(im["phaseA"], ref["phaseA"]),
+           "phaseB": rel(im["phaseB"], ref["phaseB"]), "phaseC": rel(im["phaseC"], ref["phaseC"]),
+           "rss": rel(im["rss"], ref["rss"]), "quad_p": rel(im["quad_p"], ref["quad_p"]),
+           "grad_gated_R16": float(np.max(np.abs(g - ref["grad"]) / gate))}
+    os.makedirs("gpurun_out", exist_ok=True)
+    with open(os.path.join("gpurun_out", f"full_oracle_parity_cfg{idx}.txt"), "w") as fh:
+        fh.write(f"config {idx}: b={model.b} nt={model.nt} k={model.k} a={model.a} d={model.d} N={model.N}; "
+                 f"oracle {t_or:.0f} s\n")
+        for k_, v in err.items():
+            fh.write(f"{k_} max relative error {v:.3e}\n")
+    for k_ in ("ld_p", "ld_c", "f", "x", "phaseA", "phaseB", "phaseC", "quad_p"):
+        assert err[k_] <= TOL_F, (k_, err[k_])
+    assert err["rss"] <= 1e-10
+    assert err["grad_gated_R16"] <= TOL_G
 
 
 def _closed_form_prior(model, th):
