@@ -47,6 +47,13 @@ BTA_API int bta_rows_times_block(int P, int K, int J, const double* R, int ldr, 
                                  double alpha, double beta, const double* in, int ldin, double* out, int ldo, double* part,
                                  void* stream);
 
+/* The transposed twin used by the forward sweeps (Algorithm 1 lines 4-5, 9): out[p][j] = beta in[p][j] +
+ * alpha sum_k R[p][k] M[j][k] for P <= 16 rows, k restricted to k <= j when tri != 0 (M lower triangular).  DEVICE
+ * pointers, row-major; `in` may be NULL when beta == 0 and may alias `out`.  No scratch. */
+BTA_API int bta_rows_times_block_t(int P, int J, int K, const double* R, int ldr, const double* M, int ldm, int tri,
+                                   double alpha, double beta, const double* in, int ldin, double* out, int ldo,
+                                   void* stream);
+
 /* POTRF + TRTRI of one n x n block as the forward sweeps do it (Algorithm 1 line 3, in the
  * inverse-diagonal form of DESIGN.md §5): A (DEVICE, row-major, leading dimension ld, SPD, lower triangle read, strict
  * upper triangle zero as the assembly leaves it) is overwritten by X = chol(A)^-1 (lower triangular); diagL (DEVICE, n

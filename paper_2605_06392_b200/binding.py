@@ -97,6 +97,7 @@ def lib():
     rtb = [i32, i32, i32, vp, i32, vp, i32, i32, C.c_double, C.c_double, vp, i32, vp, i32]
     L.bta_rows_times_block_noalloc.argtypes = rtb + [vp]
     L.bta_rows_times_block.argtypes = rtb + [vp, vp]
+    L.bta_rows_times_block_t.argtypes = rtb + [vp]
     L.bta_diag_potrf_inv.argtypes = [vp, vp, i32, i32, vp, vp, vp, vp]
     L.bta_set_option.argtypes = [vp, i32, i32]
     L.bta_get_option.argtypes = [vp, i32]
@@ -444,6 +445,16 @@ def rows_times_block(R, M, out, part, alpha=1.0, beta=0.0, inp=None, tri=0):
                                       beta, inp.data_ptr() if inp is not None else None,
                                       inp.stride(0) if inp is not None else 0, out.data_ptr(), out.stride(0),
                                       part.data_ptr(), _stream()))
+    return out
+
+
+def rows_times_block_t(R, M, out, alpha=1.0, beta=0.0, inp=None, tri=0):
+    """out = alpha R M^T + beta inp (k <= j only when tri): the forward sweeps' skinny product (include/bta_diag.h)."""
+    P, K = R.shape
+    J = M.shape[0]
+    _check(lib().bta_rows_times_block_t(P, J, K, R.data_ptr(), R.stride(0), M.data_ptr(), M.stride(0), int(tri), alpha,
+                                        beta, inp.data_ptr() if inp is not None else None,
+                                        inp.stride(0) if inp is not None else 0, out.data_ptr(), out.stride(0), _stream()))
     return out
 
 

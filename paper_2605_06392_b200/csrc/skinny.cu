@@ -5,8 +5,14 @@
 #include "common.cuh"
 
 constexpr int NN_KCH = 128;
-constexpr int NT_RPW = 4;   // rows of M per warp in skinny_nt
-constexpr int NT_WARPS = 4; // warps per CTA in skinny_nt (16 rows of M per CTA)
+#ifndef BTA_NT_RPW
+#define BTA_NT_RPW 4
+#endif
+#ifndef BTA_NT_WARPS
+#define BTA_NT_WARPS 4
+#endif
+constexpr int NT_RPW = BTA_NT_RPW;      // rows of M per warp in skinny_nt
+constexpr int NT_WARPS = BTA_NT_WARPS;  // warps per CTA in skinny_nt (16 rows of M per CTA)
 
 namespace {
 
@@ -20,8 +26,8 @@ __global__ void __launch_bounds__(32 * NT_WARPS) skinny_nt_kernel(int P, int J, 
                                                                   int tri, double alpha, double beta, const double* in,
                                                                   int ldin, double* out, int ldo) {
   // `in` and `out` may be the same buffer (in-place stack updates of the sweeps): no __restrict__ on them
-  constexpr int KC = 256, RPW = NT_RPW, NT = 32 * NT_WARPS;
-  __shared__ double Rs[PT * KC];
+  constexpr int KC = PT > 9 ? 128 : 256, RPW = NT_RPW, NT = 32 * NT_WARPS;   // 2 PT KC doubles of static shared memory
+  __shared__ __align__(16) double Rs[2][PT * KC];   // chunk c in Rs[c & 1], staged one chunk ahead by cp.async
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int jbase = blockIdx.x * (NT_WARPS * RPW) + warp * RPW;
   const int jmax_cta = min(J, (int)(blockIdx.x + 1) * (NT_WARPS * RPW)) - 1;
@@ -40,27 +46,44 @@ __global__ void __launch_bounds__(32 * NT_WARPS) skinny_nt_kernel(int P, int J, 
   int kend_warp = 0;
 #pragma unroll
   for (int r = 0; r < RPW; ++r) kend_warp = max(kend_warp, kend[r]);
-  for (int k0 = 0; k0 < Kcta; k0 += KC) {
-    __syncthreads();
+  // R[p][k0 .. k0+KC) -> Rs[buf] (8-byte asynchronous copies; entries beyond P or Kcta are zeroed by plain stores)
+  auto stage = [&](int buf, int k0) {
     for (int e = tid; e < PT * KC; e += NT) {
-      int p = e / KC, k = e % KC;
-      Rs[e] = (p < P && k0 + k < Kcta) ? R[(long long)p * ldr + k0 + k] : 0.0;
+      const int p = e / KC, k = e % KC;
+      if (p < P && k0 + k < Kcta) {
+        const unsigned dst = (unsigned)__cvta_generic_to_shared(&Rs[buf][e]);
+        asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(dst), "l"(R + (long long)p * ldr + k0 + k) : "memory");
+      } else {
+        Rs[buf][e] = 0.0;
+      }
     }
-    __syncthreads();
-    if (k0 >= kend_warp) continue;  // every row of this warp ends before the chunk
-#pragma unroll 2
+    asm volatile("cp.async.commit_group;" ::: "memory");
+  };
+  stage(0, 0);
+  for (int k0 = 0, c = 0; k0 < Kcta; k0 += KC, ++c) {
+    // The RPW * KC / 32 loads of this chunk are issued first (8 KB per warp in flight); R of this chunk was requested
+    // one chunk ago, R of the next one is requested before the arithmetic starts.
+    double m[KC / 32][RPW];
+#pragma unroll
     for (int q = 0; q < KC / 32; ++q) {
       const int k = k0 + q * 32 + lane;
-      double m[RPW];
 #pragma unroll
-      for (int r = 0; r < RPW; ++r) m[r] = (k < kend[r]) ? mrow[r][k] : 0.0;
+      for (int r = 0; r < RPW; ++r) m[q][r] = (k < kend[r]) ? __ldcs(mrow[r] + k) : 0.0;
+    }
+    asm volatile("cp.async.wait_all;" ::: "memory");
+    __syncthreads();                       // Rs[c & 1] is complete; everybody is done with Rs[(c + 1) & 1]
+    if (k0 + KC < Kcta) stage((c + 1) & 1, k0 + KC);
+    if (k0 >= kend_warp) continue;         // every row of this warp ends before the chunk
+    const double* rs = Rs[c & 1];
+#pragma unroll
+    for (int q = 0; q < KC / 32; ++q) {
       double rr[PT];
 #pragma unroll
-      for (int p = 0; p < PT; ++p) rr[p] = Rs[p * KC + q * 32 + lane];
+      for (int p = 0; p < PT; ++p) rr[p] = rs[p * KC + q * 32 + lane];
 #pragma unroll
       for (int r = 0; r < RPW; ++r)
 #pragma unroll
-        for (int p = 0; p < PT; ++p) acc[r][p] = fma(m[r], rr[p], acc[r][p]);
+        for (int p = 0; p < PT; ++p) acc[r][p] = fma(m[q][r], rr[p], acc[r][p]);
     }
   }
 #pragma unroll
@@ -103,16 +126,27 @@ __global__ void __launch_bounds__(256) skinny_nn_kernel(int P, int K, int J, con
       Rs[e] = (p < P && k0 + k < k1) ? R[(long long)p * ldr + k0 + k] : 0.0;
     }
     __syncthreads();
-    for (int k = k0 + ty; k < k1; k += 4) {
-      const double* mrow = M + (long long)k * ldm;
-      double ma = 0.0, mb = 0.0;
-      if (ja < J && (!tri || k >= ja)) ma = mrow[ja];
-      if (jb < J && (!tri || k >= jb)) mb = mrow[jb];
+    constexpr int U = 8;   // k-rows per thread whose loads are in flight together (16 x 8 B per thread)
+    for (int kb = k0 + ty; kb < k1; kb += 4 * U) {
+      double ma[U], mb[U];
 #pragma unroll
-      for (int p = 0; p < PT; ++p) {
-        const double r = Rs[p * KCH + (k - k0)];
-        acc[p][0] = fma(r, ma, acc[p][0]);
-        acc[p][1] = fma(r, mb, acc[p][1]);
+      for (int u = 0; u < U; ++u) {
+        const int k = kb + 4 * u;
+        const double* mrow = M + (long long)k * ldm;
+        ma[u] = (k < k1 && ja < J && (!tri || k >= ja)) ? __ldcs(mrow + ja) : 0.0;
+        mb[u] = (k < k1 && jb < J && (!tri || k >= jb)) ? __ldcs(mrow + jb) : 0.0;
+      }
+#pragma unroll
+      for (int u = 0; u < U; ++u) {
+        const int k = kb + 4 * u;
+        if (k < k1) {
+#pragma unroll
+          for (int p = 0; p < PT; ++p) {
+            const double r = Rs[p * KCH + (k - k0)];
+            acc[p][0] = fma(r, ma[u], acc[p][0]);
+            acc[p][1] = fma(r, mb[u], acc[p][1]);
+          }
+        }
       }
     }
   }
@@ -313,5 +347,16 @@ extern "C" int bta_rows_times_block(int P, int K, int J, const double* R, int ld
   }
   BTA_CUDA_OK(launch_skinny_nn(P, K, J, R, ldr, M, ldm, tri, alpha, beta, in, ldin, out, ldo, part,
                                (cudaStream_t)stream));
+  return BTA_OK;
+}
+
+extern "C" int bta_rows_times_block_t(int P, int J, int K, const double* R, int ldr, const double* M, int ldm, int tri,
+                                      double alpha, double beta, const double* in, int ldin, double* out, int ldo,
+                                      void* stream) {
+  if (P < 1 || P > 16 || K < 1 || J < 1 || !R || !M || !out || (beta != 0.0 && !in)) {
+    bta_set_error("bta_rows_times_block_t: need 1 <= P <= 16, K >= 1, J >= 1, non-null R, M, out (and in when beta != 0)");
+    return BTA_ERR_ARG;
+  }
+  BTA_CUDA_OK(launch_skinny_nt(P, J, K, R, ldr, M, ldm, tri, alpha, beta, in, ldin, out, ldo, (cudaStream_t)stream));
   return BTA_OK;
 }
