@@ -176,7 +176,8 @@ extern "C" int bta_factor_logdet(bta_ctx* c, bta_blocks io, int which, double* l
 extern "C" int bta_diag_potrf_inv(bta_ctx* c, double* A, int ld, int n, double* T1, double* T2, double* diagL,
                                   void* stream) {
   if (!c || !A || n <= 0 || ld < n) return bad("bta_diag_potrf_inv: null ctx or block, or bad sizes");
-  if (n > 128 && (!T1 || !T2)) return bad("bta_diag_potrf_inv: blocks above 128 rows need the scratch blocks T1, T2");
+  if (n > leaf_max_n() && (!T1 || !T2))
+    return bad("bta_diag_potrf_inv: blocks above 144 rows need the scratch blocks T1, T2");
   cudaStream_t st = (cudaStream_t)stream;
   DeviceGuard guard(c->device);
   BTA_CUDA_OK(cudaMemsetAsync(c->pivot_flag, 0xFF, sizeof(unsigned long long), st));
@@ -450,7 +451,7 @@ int enqueue_gradient(bta_ctx* c, void* ws, cudaStream_t s0, cudaStream_t s1, boo
 // same results up to rounding order -- but four independent chains (two per matrix) instead of two, so the
 // latency-bound POTRF phases of one chain overlap the GEMMs of three others.
 struct SubWs {
-  double *B, *W1, *W2, *W3, *Xs, *LBs, *Bs, *ubuf, *Ebuf, *Ybuf, *ZC0, *ZC1, *part, *ring;
+  double *B, *W1, *W2, *W3, *Xs, *LBs, *Bs, *ubuf, *Ebuf, *Ybuf, *ZC0, *ZC1, *part, *part2, *ring;
 };
 constexpr int HOST_RING = 4;  // device slots per sub-chain for the diagonal blocks in BTA_STORE_HOST
 struct MatWs {
@@ -497,6 +498,7 @@ MatWs carve_twist(Bump& bp, const ModelDims& md, bool cond, int store_mode) {
       s.ZC0 = bp.take((size_t)md.a * md.b);
       s.ZC1 = bp.take((size_t)md.a * md.b);
       s.part = bp.take(skinny_nn_part_doubles(P, md.b, md.b));
+      s.part2 = bp.take(skinny_nn_part_doubles(1, md.b, md.b));   // the solve stream's own partial sums
     }
   }
   return w;
@@ -573,6 +575,7 @@ void make_twist_chains(bta_ctx* c, const MatWs& w, bool cond, bool value_only, C
       k.ZC[0] = s.ZC0;
       k.ZC[1] = s.ZC1;
       k.part = s.part;
+      k.part2 = s.part2;
       k.xout = w.x;
       k.ld_x = md.N;
     }
@@ -647,6 +650,8 @@ int enqueue_gradient_twisted(bta_ctx* c, void* ws, cudaStream_t s0, bool timed, 
       // rows stream: pays where a step is latency-bound (measured: config 0 -11 %, config 1 -10 %; at b = 2304 the
       // extra concurrency costs 3 %), so only up to the size where the whole gradient is graph-replayed
       if (c->opt.rows && md.b <= 1024) ch[m][q].rs = c->s_r[2 * m + q];
+      // solve stream (the forward steps' side stream is idle in the backward sweep): same size rule
+      if (c->opt.rows && md.b <= 1024 && m == 0) ch[m][q].ss = c->s_x[2 * m + q];
     }
 
   // ---- assemble: D (all blocks), arrow/rhs rows, tip on the up stream; coupling blocks per sub-chain

@@ -133,7 +133,8 @@ bool gemm_uses_small_tiles(const GemmArgs& g);  // the 64x64-tile configuration 
 // ------------------------------------------------------------------------------------------------
 // Leaf / tip kernels (diag.cu)
 // ------------------------------------------------------------------------------------------------
-// leaf.cu: POTRF + TRTRI of one n x n (n <= 128) diagonal tile in one CTA (16-wide panels, DMMA updates)
+// leaf.cu: POTRF + TRTRI of one n x n (n <= leaf_max_n() = 144) diagonal tile in one CTA (16-wide panels, DMMA updates)
+int leaf_max_n();
 cudaError_t launch_potrf_inv_blocked(double* A, int ld, int n, double* diagL, long long grow0,
                                      unsigned long long* pivot_flag, cudaStream_t st);
 cudaError_t launch_tip(const double* Tt, int a, int nr, int do_chol, double* LT, double* zT, double* xT, double* ZT,

@@ -38,6 +38,12 @@ cudaError_t chain_to_big(Chain& ch, cudaStream_t big) {
     cudaStreamWaitEvent(big, e, 0);
   }
   ch.rows_pending = false;
+  if (ch.solve_pending && ch.ss && ch.ss != big) {  // ... and the solve stream
+    cudaEvent_t e = ch.c->ev_sw[(ch.c->ev_sw_next++) % BTA_NSW];
+    cudaEventRecord(e, ch.ss);
+    cudaStreamWaitEvent(big, e, 0);
+  }
+  ch.solve_pending = false;
   return cudaGetLastError();
 }
 #define SS lane(lch, st, true)
@@ -58,20 +64,21 @@ cudaError_t gemm_lane(Chain* lch, cudaStream_t st, const GemmArgs& g) {
 }  // namespace
 
 // A[lo:hi, lo:hi] (lower, SPD) -> X = L^-1 in place; T1, T2: scratch with the same leading dimension.
-// Recursive on 128-wide tiles (leaf: diag.cu):  chol/inv(A11);  L21 = A21 X11^T;  A22 -= L21 L21^T;  chol/inv(A22);
+// Recursive on 128-wide tiles (leaf: leaf.cu):  chol/inv(A11);  L21 = A21 X11^T;  A22 -= L21 L21^T;  chol/inv(A22);
 // X21 = -X22 (L21 X11).  b^3/3 (POTRF) + b^3/3 (TRTRI) flops, all but the 128x128 leaves in DMMA GEMMs.
-constexpr int LEAF = 128;
+// Recursive on 128-wide tiles; a remainder of up to 16 rows stays with the last tile (the leaf takes 144 rows).
+constexpr int TILE = 128;
 int potrf_split(int n) {
-  if (n <= LEAF) return n;
-  const int ntile = (n + LEAF - 1) / LEAF;
-  return LEAF * ((ntile + 1) / 2);
+  if (n <= leaf_max_n()) return n;
+  const int ntile = (n - (leaf_max_n() - TILE) + TILE - 1) / TILE;
+  return TILE * ((ntile + 1) / 2);
 }
 
 cudaError_t potrf_inv(bta_ctx* c, Chain* lch, double* A, int ld, int lo, int hi, double* T1, double* T2, double* diagL,
                       long long grow0, cudaStream_t st, int phase) {
   const int n = hi - lo;
   if (n <= 0) return cudaSuccess;
-  if (n <= LEAF) {
+  if (n <= leaf_max_n()) {
     if (phase == 2) return cudaSuccess;
     BTA_COUNT(c);
     return launch_potrf_inv_blocked(A + (long long)lo * ld + lo, ld, n, diagL ? diagL + lo : nullptr, grow0 + lo,
@@ -271,7 +278,7 @@ cudaError_t chain_forward_step(Chain& ch, int t, cudaStream_t st) {
       CK(potrf_inv(c, lch, Dt, b, 0, b, ch.W1, ch.Bs, ch.dvec ? ch.dvec + tg * b : nullptr, tg * b, st));
     } else {
       const bool has_coupling = t < nt - 1 || ch.tail_coupling;
-      coupled = has_coupling && ch.xs && b > 128 && b <= split_maxb;
+      coupled = has_coupling && ch.xs && b > leaf_max_n() && b <= split_maxb;
       if (coupled) {
         double* Bi = ch.Bin + t * ch.b_stride;
         double* Bo = ch.Bout + t * ch.b_stride;
@@ -483,12 +490,22 @@ cudaError_t chain_backward_step(Chain& ch, int t, cudaStream_t st) {
       LC = ch.LCgiven + t * ch.lc_stride;
     }
     // ---- upper solve (Eqs. 3-5):  u = z_t - L_Bt^T x_{t+1} - L_Ct^T x_T ;  x_t = X_t^T u  (row-vector form)
+    const bool side_solve = nr > 0 && ch.ss && ch.part2 && ch.selinv && !ch.selinv_inplace && !ch.carry && !ch.fill;
+    cudaEvent_t ev_solve = nullptr;   // side_solve: this step's solve has read L_Bt
     if (nr > 0) {
+      double* part = side_solve ? ch.part2 : ch.part;
+      if (side_solve && !ch.solve_pending) {  // first step of this chain: x_{t+1} / x_T come from the chain's stream
+        cudaEvent_t e = c->ev_sw[(c->ev_sw_next++) % BTA_NSW];
+        CK(cudaEventRecord(e, lane(lch, st, lch ? ch.on_small : false)));
+        CK(cudaStreamWaitEvent(ch.ss, e, 0));
+        ch.solve_pending = true;
+      }
+      auto SV = [&]() { return side_solve ? ch.ss : lane(lch, st, true); };
       const double* z = ch.Rout + t * ch.rout_stride + (long long)zrow0 * ch.ld_rout;
       const double* u = z;
       int ld_u = ch.ld_rout;
       if (arrow) {
-        CK(launch_small_left_mul(nr, a, b, ch.xT, a, LC, ld_lc, -1.0, 1.0, u, ld_u, ch.ubuf, b, SS));
+        CK(launch_small_left_mul(nr, a, b, ch.xT, a, LC, ld_lc, -1.0, 1.0, u, ld_u, ch.ubuf, b, SV()));
         BTA_COUNT(c);
         u = ch.ubuf;
         ld_u = b;
@@ -496,20 +513,24 @@ cudaError_t chain_backward_step(Chain& ch, int t, cudaStream_t st) {
       if (has_next) {
         const double* xnext = (t < nt - 1) ? ch.xout + (long long)ch.tg(t + 1) * b : ch.sep_x;
         CK(launch_skinny_nn(nr, b, b, xnext, (int)ch.ld_x, LB, b, 0, -1.0, 1.0, u, ld_u,
-                            ch.ubuf, b, ch.part, SS));
+                            ch.ubuf, b, part, SV()));
         c->launches += 2;
         u = ch.ubuf;
         ld_u = b;
       }
       if (ch.fill) {  // - L_Ft^T x_s
         CK(launch_skinny_nn(nr, b, b, ch.fill->xs, (int)ch.fill->ld_xs, ch.fill->LF + t * ch.fill->lf_stride, b, 0, -1.0,
-                            1.0, u, ld_u, ch.ubuf, b, ch.part, SS));
+                            1.0, u, ld_u, ch.ubuf, b, part, SV()));
         c->launches += 2;
         u = ch.ubuf;
         ld_u = b;
       }
+      if (side_solve && has_next) {
+        ev_solve = c->ev_sw[(c->ev_sw_next++) % BTA_NSW];
+        CK(cudaEventRecord(ev_solve, ch.ss));
+      }
       CK(launch_skinny_nn(nr, b, b, u, ld_u, X, b, 1, 1.0, 0.0, nullptr, 0, ch.xout + tg * b, (int)ch.ld_x,
-                          ch.part, SS));
+                          part, SV()));
       c->launches += 2;
     }
     if (!ch.selinv) return cudaSuccess;
@@ -549,6 +570,7 @@ cudaError_t chain_backward_step(Chain& ch, int t, cudaStream_t st) {
         c->launches += 2;
       }
       double* ZB = LB;  // L_Bt is dead from here on: Z_Bt takes its slot
+      if (ev_solve) CK(cudaStreamWaitEvent(SB, ev_solve, 0));
       CK(launch_gemm(G(GEMM_NN, b, b, b, -1.0, ZDnext, b, Gm, b, 0.0, ZB, b, KLO_ZERO, KHI_K, OUT_FULL), SB));
       BTA_COUNT(c);
       if (arrow) {

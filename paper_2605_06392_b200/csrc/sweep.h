@@ -62,6 +62,13 @@ struct Chain {
   // pipe_ev[3], [4]: the contractions of an even / odd backward step have read their Z buffers.
   cudaStream_t rs = nullptr;
   bool rows_pending = false;   // work is outstanding on rs (chain_to_big joins it)
+  // Solve stream: the upper solve of a backward step (Eqs. 3-5: u = z_t - L_Bt^T x_{t+1} - L_Ct^T x_T, x_t = X_t^T u) reads
+  // only forward results and x_{t+1}, never the selected inverse, so (factor mode) its three to five small kernels run
+  // on this stream, ahead of the chain, with their own partial-sum scratch `part2`; the chain only waits, before Z_Bt
+  // overwrites the slot of L_Bt, for the solve step that read it.
+  cudaStream_t ss = nullptr;
+  bool solve_pending = false;  // work is outstanding on ss (chain_to_big joins it)
+  double* part2 = nullptr;
   bool tr_armed[2] = {false, false};
   // Host-staged carries (BTA_STORE_HOST): the diagonal-block slots are a ring of `ring` device blocks
   // (local block s lives in slot s % ring); each carry D_s - S_{s-1} is copied to pinned host memory (hostD + s b^2) on
