@@ -451,8 +451,9 @@ int enqueue_gradient(bta_ctx* c, void* ws, cudaStream_t s0, cudaStream_t s1, boo
 // same results up to rounding order -- but four independent chains (two per matrix) instead of two, so the
 // latency-bound POTRF phases of one chain overlap the GEMMs of three others.
 struct SubWs {
-  double *B, *W1, *W2, *W3, *Xs, *LBs, *Bs, *ubuf, *Ebuf, *Ybuf, *ZC0, *ZC1, *part, *part2, *ring;
+  double *B, *W1, *W2, *W3, *Xs, *LBs, *Bs, *ubuf, *Ebuf, *Ybuf, *ZC0, *ZC1, *part, *part2, *EY2, *G2, *ring;
 };
+constexpr int AHEAD_MAXB = 1024;   // block sizes whose backward steps run G, X^T X, the solve and E ahead of the chain
 constexpr int HOST_RING = 4;  // device slots per sub-chain for the diagonal blocks in BTA_STORE_HOST
 struct MatWs {
   double *D, *dvec, *T, *Rin, *Rout, *x, *rtip, *Tt2;
@@ -489,6 +490,7 @@ MatWs carve_twist(Bump& bp, const ModelDims& md, bool cond, int store_mode) {
         if (store_mode == BTA_STORE_HOST) s.ring = bp.take(bb * HOST_RING);
       } else {
         s.B = bp.take(bb * (len[q] + 1));
+        if (md.b <= AHEAD_MAXB) s.G2 = bp.take(2 * bb);   // ring of two G = L_B X (sweep.h: Chain::Gm2)
       }
     }
     if (cond) {
@@ -498,7 +500,9 @@ MatWs carve_twist(Bump& bp, const ModelDims& md, bool cond, int store_mode) {
       s.ZC0 = bp.take((size_t)md.a * md.b);
       s.ZC1 = bp.take((size_t)md.a * md.b);
       s.part = bp.take(skinny_nn_part_doubles(P, md.b, md.b));
-      s.part2 = bp.take(skinny_nn_part_doubles(1, md.b, md.b));   // the solve stream's own partial sums
+      // the solve stream's own partial sums (upper solve: 1 row; arrow product E: a rows) and its ring of E / Z_T E
+      s.part2 = bp.take(skinny_nn_part_doubles(std::max(1, md.a), md.b, md.b));
+      s.EY2 = bp.take((size_t)4 * md.a * md.b);
     }
   }
   return w;
@@ -576,12 +580,20 @@ void make_twist_chains(bta_ctx* c, const MatWs& w, bool cond, bool value_only, C
       k.ZC[1] = s.ZC1;
       k.part = s.part;
       k.part2 = s.part2;
+      for (int r = 0; r < 2; ++r) {
+        k.Ebuf2[r] = s.EY2 + (size_t)(2 * r) * md.a * md.b;
+        k.Ybuf2[r] = s.EY2 + (size_t)(2 * r + 1) * md.a * md.b;
+      }
       k.xout = w.x;
       k.ld_x = md.N;
     }
     k.T = w.T;
     k.ldT = md.a;
     k.W1 = s.W1;
+    if (s.G2) {
+      k.Gm2[0] = s.G2;
+      k.Gm2[1] = s.G2 + bb;
+    }
     k.W2 = s.W2;
     k.W3 = s.W3;
     k.dvec = w.dvec;
@@ -651,7 +663,7 @@ int enqueue_gradient_twisted(bta_ctx* c, void* ws, cudaStream_t s0, bool timed, 
       // extra concurrency costs 3 %), so only up to the size where the whole gradient is graph-replayed
       if (c->opt.rows && md.b <= 1024) ch[m][q].rs = c->s_r[2 * m + q];
       // solve stream (the forward steps' side stream is idle in the backward sweep): same size rule
-      if (c->opt.rows && md.b <= 1024 && m == 0) ch[m][q].ss = c->s_x[2 * m + q];
+      if (c->opt.rows && md.b <= AHEAD_MAXB && !carry) ch[m][q].ss = c->s_x[2 * m + q];
     }
 
   // ---- assemble: D (all blocks), arrow/rhs rows, tip on the up stream; coupling blocks per sub-chain

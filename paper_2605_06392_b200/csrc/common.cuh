@@ -226,7 +226,10 @@ struct bta_ctx {
   size_t host_bytes;
   cudaStream_t s_copy[4];            // its copy streams (one per sub-chain) and ring-slot events
   cudaEvent_t ev_ring[4][8];
-  cudaEvent_t ev_pipe[20][5];        // per chain (sweep.h: Chain::pipe_ev): forward pipelining [0..2], trace parity [3..4]
+  cudaEvent_t ev_pipe[20][17];       // per chain (sweep.h: Chain::pipe_ev): forward pipelining [0..2], trace parity [3..4];
+                                     // backward work running ahead on the solve stream, by step parity: arrow products
+                                     // E, Z_T E ready [5..6] / consumed [7..8], G and X^T X ready [9..10], G consumed
+                                     // [11..12], Z_D buffer read by the next step's Z_B product [13..14]
   cudaStream_t s_r[4];               // rows streams of the four chains (sweep.h: Chain::rs)
   cudaStream_t s_part[2][8], s_part_hi[2][8], s_part_x[2][8], s_part_r[2][8];  // partition.cu: per (matrix, partition)
   cudaEvent_t ev_sw[256];            // lane-switch events, used round-robin

@@ -490,16 +490,18 @@ cudaError_t chain_backward_step(Chain& ch, int t, cudaStream_t st) {
       LC = ch.LCgiven + t * ch.lc_stride;
     }
     // ---- upper solve (Eqs. 3-5):  u = z_t - L_Bt^T x_{t+1} - L_Ct^T x_T ;  x_t = X_t^T u  (row-vector form)
-    const bool side_solve = nr > 0 && ch.ss && ch.part2 && ch.selinv && !ch.selinv_inplace && !ch.carry && !ch.fill;
-    cudaEvent_t ev_solve = nullptr;   // side_solve: this step's solve has read L_Bt
+    const bool use_ss = ch.ss && ch.selinv && !ch.selinv_inplace && !ch.carry && !ch.fill;
+    const bool side_solve = nr > 0 && use_ss && ch.part2;
+    const bool side_g = use_ss && has_next && ch.pipe_ev && ch.Gm2[t & 1];
+    cudaEvent_t ev_solve = nullptr;   // the work of this step on the solve stream has read L_Bt
+    if ((side_solve || side_g) && !ch.solve_pending) {  // first step of this chain: its inputs come from the chain's stream
+      cudaEvent_t e = c->ev_sw[(c->ev_sw_next++) % BTA_NSW];
+      CK(cudaEventRecord(e, lane(lch, st, lch ? ch.on_small : false)));
+      CK(cudaStreamWaitEvent(ch.ss, e, 0));
+      ch.solve_pending = true;
+    }
     if (nr > 0) {
       double* part = side_solve ? ch.part2 : ch.part;
-      if (side_solve && !ch.solve_pending) {  // first step of this chain: x_{t+1} / x_T come from the chain's stream
-        cudaEvent_t e = c->ev_sw[(c->ev_sw_next++) % BTA_NSW];
-        CK(cudaEventRecord(e, lane(lch, st, lch ? ch.on_small : false)));
-        CK(cudaStreamWaitEvent(ch.ss, e, 0));
-        ch.solve_pending = true;
-      }
       auto SV = [&]() { return side_solve ? ch.ss : lane(lch, st, true); };
       const double* z = ch.Rout + t * ch.rout_stride + (long long)zrow0 * ch.ld_rout;
       const double* u = z;
@@ -525,10 +527,6 @@ cudaError_t chain_backward_step(Chain& ch, int t, cudaStream_t st) {
         u = ch.ubuf;
         ld_u = b;
       }
-      if (side_solve && has_next) {
-        ev_solve = c->ev_sw[(c->ev_sw_next++) % BTA_NSW];
-        CK(cudaEventRecord(ev_solve, ch.ss));
-      }
       CK(launch_skinny_nn(nr, b, b, u, ld_u, X, b, 1, 1.0, 0.0, nullptr, 0, ch.xout + tg * b, (int)ch.ld_x,
                           part, SV()));
       c->launches += 2;
@@ -546,38 +544,83 @@ cudaError_t chain_backward_step(Chain& ch, int t, cudaStream_t st) {
     const double* ZDnext = (t < nt - 1) ? ((t & 1) ? ch.W3 : ch.W2) : ch.sep_ZD;
     double* ZCcur = ch.ZC[t & 1];
     const double* ZCnext = (t < nt - 1) ? ch.ZC[(t & 1) ^ 1] : ch.sep_ZC;
+    double* Eb = ch.Ebuf;
+    double* Yb = ch.Ybuf;
+    cudaEvent_t ev_ey = nullptr;   // side_solve: E and Z_T E of this step are ready (recorded on the solve stream)
     if (arrow) {
-      CK(launch_skinny_nn(a, b, b, LC, ld_lc, X, b, 1, 1.0, 0.0, nullptr, 0, ch.Ebuf, b, ch.part, SS));  // E
-      CK(launch_small_left_mul(a, a, b, ch.ZT, a, ch.Ebuf, b, 1.0, 0.0, nullptr, 0, ch.Ybuf, b, SS));   // Z_T E
+      const bool side_ey = side_solve && ch.pipe_ev && ch.Ebuf2[t & 1] && ch.Ybuf2[t & 1];
+      cudaStream_t es = SS;
+      double* part = ch.part;
+      if (side_ey) {
+        Eb = ch.Ebuf2[t & 1];
+        Yb = ch.Ybuf2[t & 1];
+        es = ch.ss;
+        part = ch.part2;
+        if (ch.ey_used[t & 1]) CK(cudaStreamWaitEvent(es, ch.pipe_ev[7 + (t & 1)], 0));  // step t+2 is done with the slot
+      }
+      CK(launch_skinny_nn(a, b, b, LC, ld_lc, X, b, 1, 1.0, 0.0, nullptr, 0, Eb, b, part, es));  // E
+      CK(launch_small_left_mul(a, a, b, ch.ZT, a, Eb, b, 1.0, 0.0, nullptr, 0, Yb, b, es));     // Z_T E
       c->launches += 3;
+      if (side_ey) {
+        ev_ey = ch.pipe_ev[5 + (t & 1)];
+        CK(cudaEventRecord(ev_ey, es));
+      }
     }
     Fill* fl = ch.fill;
+    if (ev_ey) {  // the chain's lanes use E and Z_T E from here on
+      CK(cudaStreamWaitEvent(st, ev_ey, 0));
+      if (ch.hi && lch) CK(cudaStreamWaitEvent(ch.hi, ev_ey, 0));
+    }
     double* LFt = fl ? fl->LF + t * fl->lf_stride : nullptr;
     if (fl) {  // H = L_F X;  the arrow term Z_T E gains Sigma[T,s] H
       CK(launch_gemm(G(GEMM_NN, b, b, b, 1.0, LFt, b, X, b, 0.0, fl->H, b, KLO_N0, KHI_K, OUT_FULL), SB));
       BTA_COUNT(c);
       if (arrow) {
-        CK(launch_skinny_nn(a, b, b, fl->ZCs, b, fl->H, b, 0, 1.0, 1.0, ch.Ybuf, b, ch.Ybuf, b, ch.part, SS));
+        CK(launch_skinny_nn(a, b, b, fl->ZCs, b, fl->H, b, 0, 1.0, 1.0, Yb, b, Yb, b, ch.part, SS));
         c->launches += 2;
       }
     }
     if (has_next) {
-      double* Gm = ch.W1;
-      CK(launch_gemm(G(GEMM_NN, b, b, b, 1.0, LB, b, X, b, 0.0, Gm, b, KLO_N0, KHI_K, OUT_FULL), SB));
+      double* Gm = side_g ? ch.Gm2[t & 1] : ch.W1;
+      if (side_g) {
+        cudaStream_t gs = ch.ss;
+        if (ch.g_used[t & 1]) CK(cudaStreamWaitEvent(gs, ch.pipe_ev[11 + (t & 1)], 0));   // step t+2 is done with the slot
+        CK(launch_gemm(G(GEMM_NN, b, b, b, 1.0, LB, b, X, b, 0.0, Gm, b, KLO_N0, KHI_K, OUT_FULL), gs));
+        // X^T X straight into this step's Z_D buffer: step t+1's Z_B product (and the traces of step t+2) have read it
+        if (ch.zd_read[t & 1]) CK(cudaStreamWaitEvent(gs, ch.pipe_ev[13 + (t & 1)], 0));
+        if (defer_tr && ch.tr_armed[t & 1]) CK(cudaStreamWaitEvent(gs, ch.pipe_ev[3 + (t & 1)], 0));
+        CK(launch_gemm(G(GEMM_TN, b, b, b, 1.0, X, b, X, b, 0.0, ZDcur, b, KLO_M0, KHI_K, OUT_LOWER), gs));
+        CK(cudaEventRecord(ch.pipe_ev[9 + (t & 1)], gs));
+      } else {
+        CK(launch_gemm(G(GEMM_NN, b, b, b, 1.0, LB, b, X, b, 0.0, Gm, b, KLO_N0, KHI_K, OUT_FULL), SB));
+      }
       BTA_COUNT(c);
+      if (side_solve || side_g) {  // every reader of L_Bt on the solve stream has been issued
+        ev_solve = c->ev_sw[(c->ev_sw_next++) % BTA_NSW];
+        CK(cudaEventRecord(ev_solve, ch.ss));
+      }
+      if (side_g) {
+        CK(cudaStreamWaitEvent(st, ch.pipe_ev[9 + (t & 1)], 0));
+        if (ch.hi && lch) CK(cudaStreamWaitEvent(ch.hi, ch.pipe_ev[9 + (t & 1)], 0));
+      }
       if (arrow) {
-        CK(launch_skinny_nn(a, b, b, ZCnext, b, Gm, b, 0, -1.0, -1.0, ch.Ybuf, b, ZCcur, b, ch.part, SS));
+        CK(launch_skinny_nn(a, b, b, ZCnext, b, Gm, b, 0, -1.0, -1.0, Yb, b, ZCcur, b, ch.part, SS));
         c->launches += 2;
       }
       double* ZB = LB;  // L_Bt is dead from here on: Z_Bt takes its slot
       if (ev_solve) CK(cudaStreamWaitEvent(SB, ev_solve, 0));
       CK(launch_gemm(G(GEMM_NN, b, b, b, -1.0, ZDnext, b, Gm, b, 0.0, ZB, b, KLO_ZERO, KHI_K, OUT_FULL), SB));
       BTA_COUNT(c);
+      if (side_g) {  // the Z_D buffer of the other parity (Z_D{t+1}) may now receive X^T X of step t-1
+        CK(cudaEventRecord(ch.pipe_ev[13 + ((t + 1) & 1)], SB));
+        ch.zd_read[(t + 1) & 1] = true;
+      }
       if (arrow) {
-        CK(launch_gemm(G(GEMM_TN, b, b, a, -1.0, ZCnext, b, ch.Ebuf, b, 1.0, ZB, b, KLO_ZERO, KHI_K, OUT_FULL), SB));
+        CK(launch_gemm(G(GEMM_TN, b, b, a, -1.0, ZCnext, b, Eb, b, 1.0, ZB, b, KLO_ZERO, KHI_K, OUT_FULL), SB));
         BTA_COUNT(c);
       }
-      CK(launch_gemm(G(GEMM_TN, b, b, b, 1.0, X, b, X, b, 0.0, ZDcur, b, KLO_M0, KHI_K, OUT_LOWER), SB));
+      if (!side_g)
+        CK(launch_gemm(G(GEMM_TN, b, b, b, 1.0, X, b, X, b, 0.0, ZDcur, b, KLO_M0, KHI_K, OUT_LOWER), SB));
       if (fl) {
         // Sigma[s, t+1] is Z_F of the block below (stored [s][t+1]); below the last interior block it is the reduced
         // system's Sigma[e, s], stored the other way round
@@ -591,7 +634,7 @@ cudaError_t chain_backward_step(Chain& ch, int t, cudaStream_t st) {
                        SB));
         CK(launch_gemm(G(GEMM_NN, b, b, b, -1.0, fl->ZDs, b, fl->H, b, 1.0, LFt, b, KLO_ZERO, KHI_K, OUT_FULL), SB));
         if (arrow)
-          CK(launch_gemm(G(GEMM_TN, b, b, a, -1.0, fl->ZCs, b, ch.Ebuf, b, 1.0, LFt, b, KLO_ZERO, KHI_K, OUT_FULL), SB));
+          CK(launch_gemm(G(GEMM_TN, b, b, a, -1.0, fl->ZCs, b, Eb, b, 1.0, LFt, b, KLO_ZERO, KHI_K, OUT_FULL), SB));
         //   Z_D -= Z_F^T H
         CK(launch_gemm(G(GEMM_TN, b, b, b, -1.0, LFt, b, fl->H, b, 1.0, ZDcur, b, KLO_ZERO, KHI_K, OUT_LOWER), SB));
         c->launches += arrow ? 5 : 4;
@@ -600,9 +643,13 @@ cudaError_t chain_backward_step(Chain& ch, int t, cudaStream_t st) {
                        arrow ? OUT_LOWER : OUT_LOWER_MIRROR),
                      SB));
       c->launches += 2;
+      if (side_g) {  // last reader of this step's G
+        CK(cudaEventRecord(ch.pipe_ev[11 + (t & 1)], SB));
+        ch.g_used[t & 1] = true;
+      }
     } else {
       if (arrow) {
-        scale_copy_kernel<<<(unsigned)(((long long)a * b + 255) / 256), 256, 0, SS>>>((long long)a * b, -1.0, ch.Ybuf,
+        scale_copy_kernel<<<(unsigned)(((long long)a * b + 255) / 256), 256, 0, SS>>>((long long)a * b, -1.0, Yb,
                                                                                       ZCcur);
         BTA_COUNT(c);
       }
@@ -612,9 +659,13 @@ cudaError_t chain_backward_step(Chain& ch, int t, cudaStream_t st) {
       BTA_COUNT(c);
     }
     if (arrow) {
-      CK(launch_gemm(G(GEMM_TN, b, b, a, -1.0, ZCcur, b, ch.Ebuf, b, 1.0, ZDcur, b, KLO_ZERO, KHI_K, OUT_LOWER_MIRROR),
+      CK(launch_gemm(G(GEMM_TN, b, b, a, -1.0, ZCcur, b, Eb, b, 1.0, ZDcur, b, KLO_ZERO, KHI_K, OUT_LOWER_MIRROR),
                      SB));
       BTA_COUNT(c);
+      if (ev_ey) {  // every use of this step's E / Z_T E has been issued in lane order
+        CK(cudaEventRecord(ch.pipe_ev[7 + (t & 1)], lane(lch, st, lch ? ch.on_small : false)));
+        ch.ey_used[t & 1] = true;
+      }
     }
     if (ch.contract) {
       cudaStream_t ts = SS;

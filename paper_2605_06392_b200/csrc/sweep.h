@@ -66,9 +66,20 @@ struct Chain {
   // only forward results and x_{t+1}, never the selected inverse, so (factor mode) its three to five small kernels run
   // on this stream, ahead of the chain, with their own partial-sum scratch `part2`; the chain only waits, before Z_Bt
   // overwrites the slot of L_Bt, for the solve step that read it.
+  // The arrow products E = L_Ct X_t and Z_T E of the selected inversion read only forward results as well: they run on
+  // the same stream into a ring of two buffers (step parity), one step ahead of the chain; pipe_ev[5 + parity] says
+  // "ready", pipe_ev[7 + parity] "consumed".
   cudaStream_t ss = nullptr;
   bool solve_pending = false;  // work is outstanding on ss (chain_to_big joins it)
   double* part2 = nullptr;
+  double *Ebuf2[2] = {nullptr, nullptr}, *Ybuf2[2] = {nullptr, nullptr};
+  bool ey_used[2] = {false, false};
+  // So do G = L_Bt X_t (into a ring of two b x b buffers) and X_t^T X_t (straight into the step's Z_D buffer, once the
+  // next step's Z_B product and the traces two steps back have read it): the dependent chain of a backward step is then
+  // Z_C, Z_B = -Z_D{t+1} G - ..., Z_D -= Z_B^T G.  pipe_ev[9 + parity] ready, [11 + parity] G consumed, [13 + parity]
+  // Z_D buffer of that parity read.
+  double* Gm2[2] = {nullptr, nullptr};
+  bool g_used[2] = {false, false}, zd_read[2] = {false, false};
   bool tr_armed[2] = {false, false};
   // Host-staged carries (BTA_STORE_HOST): the diagonal-block slots are a ring of `ring` device blocks
   // (local block s lives in slot s % ring); each carry D_s - S_{s-1} is copied to pinned host memory (hostD + s b^2) on
