@@ -5,14 +5,8 @@
 #include "common.cuh"
 
 constexpr int NN_KCH = 128;
-#ifndef BTA_NT_RPW
-#define BTA_NT_RPW 4
-#endif
-#ifndef BTA_NT_WARPS
-#define BTA_NT_WARPS 4
-#endif
-constexpr int NT_RPW = BTA_NT_RPW;      // rows of M per warp in skinny_nt
-constexpr int NT_WARPS = BTA_NT_WARPS;  // warps per CTA in skinny_nt (16 rows of M per CTA)
+constexpr int NT_RPW = 4;    // rows of M per warp in skinny_nt (2 x 8, 2 x 4 and 4 x 2 warps were measured: DESIGN.md §6)
+constexpr int NT_WARPS = 4;  // warps per CTA in skinny_nt (16 rows of M per CTA)
 
 namespace {
 
