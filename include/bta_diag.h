@@ -80,9 +80,10 @@ BTA_API int bta_diag_ktime_end(double* ms, double* flop, double* bytes, long lon
  *   BTA_OPT_TILE_THRESH (BTA_TILE_THRESH), BTA_OPT_TILE_WAVES (BTA_TILE_WAVES): the GEMM tile rule (process-global):
  *                                      launches of fewer 128x128 tiles than the threshold (180) use 64x64 tiles, and
  *                                      (waves = 1) so do launches whose last wave of 128x128 tiles would be mostly empty
- *   BTA_OPT_PDL (BTA_PDL)              1 (default): the latency-bound kernels (32x32-tile GEMMs, POTRF leaves) are
- *                                      launched programmatically (they start while their predecessor drains and wait
- *                                      at griddepcontrol.wait); 0: plain launches.  Process-global.
+ *   BTA_OPT_PDL (BTA_PDL)              programmatic dependent launch of the latency-bound kernels (they start while their
+ *                                      predecessor drains and wait at griddepcontrol.wait): 3 (default) the POTRF leaves
+ *                                      only, 1 the leaves and the 32x32-tile GEMMs, 2 those GEMMs only, 0 plain launches.
+ *                                      Process-global.
  *   BTA_OPT_ROWS (BTA_ROWS)            1 (default): the arrow / right-hand-side rows of the forward steps and the trace
  *                                      contractions of the backward steps run on a third stream per chain (factor
  *                                      mode), off the chain's dependent launch sequence; 0: in line

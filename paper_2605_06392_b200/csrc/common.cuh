@@ -107,9 +107,10 @@ struct GemmArgs {
 
 extern long long g_tile_thresh;
 extern int g_tile_waves;
-// Programmatic dependent launch for the latency-bound kernels (32x32-tile GEMMs, POTRF leaves): the kernel is launched
+// Programmatic dependent launch for the latency-bound kernels (POTRF leaves, 32x32-tile GEMMs): the kernel is launched
 // with cudaLaunchAttributeProgrammaticStreamSerialization, starts while its predecessor in the stream drains, and waits
-// at `griddepcontrol.wait` before touching memory (BTA_OPT_PDL, process-global).
+// at `griddepcontrol.wait` before touching memory.  BTA_OPT_PDL (process-global): 0 off, 1 both kernel classes, 2 the
+// GEMMs only, 3 the leaves only (default: early-resident GEMM CTAs cost more SM slots than their start-up saves).
 extern int g_pdl;
 __device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
 __device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }

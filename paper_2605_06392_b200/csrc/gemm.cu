@@ -412,7 +412,7 @@ cudaError_t launch_cfg(const GemmArgs& g, cudaStream_t st) {
   }
   KTimeScope kt(BM == 128 ? BTA_KC_GEMM_BIG : (BM == 64 ? BTA_KC_GEMM_SMALL : BTA_KC_GEMM_TINY), st,
                 g_ktime_on ? gemm_alg_flop(g) : 0.0, 0.0);
-  if (BM == 32 && g_pdl) return launch_pdl(kern, grid, dim3(C_::NT), (size_t)C_::SMEM, st, ga);
+  if (BM == 32 && (g_pdl == 1 || g_pdl == 2)) return launch_pdl(kern, grid, dim3(C_::NT), (size_t)C_::SMEM, st, ga);
   kern<<<grid, C_::NT, C_::SMEM, st>>>(ga);
   return cudaGetLastError();
 }
@@ -430,7 +430,7 @@ cudaError_t launch_mode(const GemmArgs& g, cudaStream_t st) {
 }  // namespace
 
 // Tile-choice parameters (bta_set_option: BTA_OPT_TILE_THRESH / BTA_OPT_TILE_WAVES; process-global)
-int g_pdl = 1;
+int g_pdl = 3;   // BTA_OPT_PDL: 0 off, 1 leaves and 32x32-tile GEMMs, 2 the GEMMs only, 3 the leaves only (measured best)
 long long g_tile_thresh = 180;  // fewer big tiles than this: 64x64 tiles (measured)
 int g_tile_waves = 1;           // 1: also prefer 64x64 tiles where the last wave of big tiles would be mostly empty
 

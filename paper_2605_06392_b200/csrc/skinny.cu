@@ -5,7 +5,7 @@
 #include "common.cuh"
 
 constexpr int NN_KCH = 128;
-constexpr int NT_RPW = 4;    // rows of M per warp in skinny_nt (2 x 8, 2 x 4 and 4 x 2 warps were measured: DESIGN.md §6)
+constexpr int NT_RPW = 4;    // rows of M per warp in skinny_nt (2 x 8, 2 x 4, 4 x 2 were measured: profiles/r02_hbm_kernels.md)
 constexpr int NT_WARPS = 4;  // warps per CTA in skinny_nt (16 rows of M per CTA)
 
 namespace {
