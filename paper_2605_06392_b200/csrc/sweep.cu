@@ -98,13 +98,33 @@ cudaError_t potrf_inv(bta_ctx* c, Chain* lch, double* A, int ld, int lo, int hi,
   double* L21 = T1 + (long long)mid * ld + lo;
   double* LX = T2 + (long long)mid * ld + lo;
   CK(gemm_lane(lch, st, G(GEMM_NT, s2, s1, s1, 1.0, A21, ld, A11, ld, 0.0, L21, ld, KLO_ZERO, KHI_NEND, OUT_FULL)));
+  // L21 X11 feeds only X21 at the end of this level.  Where a step is latency-bound (b <= 1024: the chip is not full) it
+  // runs on the chain's side stream beside the update and the factorisation of A22 instead of after them.  (Above that
+  // size the same move costs 3-11 %: DESIGN.md §6.)
+  const bool lx_side = lch && lch->xs && ld <= 1024 && n < ld;
+  cudaEvent_t e_lx = nullptr;
+  if (lx_side) {
+    cudaEvent_t e0 = c->ev_sw[(c->ev_sw_next++) % BTA_NSW];
+    e_lx = c->ev_sw[(c->ev_sw_next++) % BTA_NSW];
+    CK(cudaEventRecord(e0, lane(lch, st, lch->on_small)));   // L21 (and X11) are complete in lane order
+    CK(cudaStreamWaitEvent(lch->xs, e0, 0));
+    CK(launch_gemm(G(GEMM_NN, s2, s1, s1, 1.0, L21, ld, A11, ld, 0.0, LX, ld, KLO_N0, KHI_K, OUT_FULL), lch->xs));
+    CK(cudaEventRecord(e_lx, lch->xs));
+  }
   CK(gemm_lane(lch, st, G(GEMM_NT, s2, s2, s1, -1.0, L21, ld, L21, ld, 1.0, A22, ld, KLO_ZERO, KHI_K, OUT_LOWER)));
   c->launches += 2;
   PM(11);
   CK(potrf_inv(c, lch, A, ld, mid, hi, T1, T2, diagL, grow0, st));
   PM(12);
-  CK(gemm_lane(lch, st, G(GEMM_NN, s2, s1, s1, 1.0, L21, ld, A11, ld, 0.0, LX, ld, KLO_N0, KHI_K, OUT_FULL)));
-  CK(gemm_lane(lch, st, G(GEMM_NN, s2, s1, s2, -1.0, A22, ld, LX, ld, 0.0, A21, ld, KLO_ZERO, KHI_MEND, OUT_FULL)));
+  if (lx_side) {
+    const GemmArgs gx = G(GEMM_NN, s2, s1, s2, -1.0, A22, ld, LX, ld, 0.0, A21, ld, KLO_ZERO, KHI_MEND, OUT_FULL);
+    cudaStream_t tgt = gemm_uses_small_tiles(gx) ? SS : SB;
+    CK(cudaStreamWaitEvent(tgt, e_lx, 0));
+    CK(launch_gemm(gx, tgt));
+  } else {
+    CK(gemm_lane(lch, st, G(GEMM_NN, s2, s1, s1, 1.0, L21, ld, A11, ld, 0.0, LX, ld, KLO_N0, KHI_K, OUT_FULL)));
+    CK(gemm_lane(lch, st, G(GEMM_NN, s2, s1, s2, -1.0, A22, ld, LX, ld, 0.0, A21, ld, KLO_ZERO, KHI_MEND, OUT_FULL)));
+  }
   c->launches += 2;
   return cudaSuccess;
 }
