@@ -132,9 +132,10 @@ cudaError_t potrf_inv(bta_ctx* c, Chain* lch, double* A, int ld, int lo, int hi,
 // Forward step with the coupling block folded into the top level of the POTRF+TRTRI recursion (factor mode).
 // With A = [[A11, .], [A21, A22]], X = L^-1 = [[X11, 0], [X21, X22]] and B = [B1 | B2]:
 //   L_B = B X^T = [ B1 X11^T | (B2 - L_B1 L21^T) X22^T ],   S = L_B1 L_B1^T + L_B2 L_B2^T,   X21 = -X22 (L21 X11).
-// L_B1 and its half of the Schur update need only X11, and X21 is not needed by the factorisation at all, so they
-// run on the chain's side stream `xs` next to the second half of the recursion; the dependent chain of a step is
-// potrf_inv(A11) -> L21, A22 -> potrf_inv(A22) -> L_B2 -> second half of S instead of ... -> X21 -> L_B -> S.  Same
+// L_B1, B2 - L_B1 L21^T and L_B1's half of the Schur update need only X11 (and L21), and X21 is not needed by the
+// factorisation at all, so they run on the chain's side stream `xs` next to the second half of the recursion; the
+// dependent chain of a step is potrf_inv(A11) -> L21, A22 -> potrf_inv(A22) -> (.) X22^T -> second half of S instead
+// of ... -> X21 -> L_B -> S.  Same
 // flops.  B (its right half) is updated in place; L_B goes to `dst`.
 cudaError_t potrf_inv_coupled(bta_ctx* c, Chain* lch, double* A, int b, double* Bi, double* dst, double* Dnext,
                               double* T1, double* T2, double* diagL, long long grow0, cudaStream_t st,
@@ -154,18 +155,24 @@ cudaError_t potrf_inv_coupled(bta_ctx* c, Chain* lch, double* A, int b, double* 
   //   side: L_B1 = B1 X11^T, S += L_B1 L_B1^T
   CK(launch_gemm(G(GEMM_NT, b, s1, s1, 1.0, Bi, b, A, ld, 0.0, dst, b, KLO_ZERO, KHI_NEND, OUT_FULL), xs));
   CK(cudaEventRecord(e2, xs));
-  if (Dnext)
-    CK(launch_gemm(G(GEMM_NT, b, b, s1, -1.0, dst, b, dst, b, 1.0, Dnext, b, KLO_ZERO, KHI_K, OUT_LOWER), xs));
-  CK(cudaEventRecord(e3, xs));
-  c->launches += Dnext ? 2 : 1;
   //   main: second half of the recursion
   double* A21 = A + (long long)mid * ld;
   double* A22 = A + (long long)mid * ld + mid;
   double* L21 = T1 + (long long)mid * ld;
   double* LX = T2 + (long long)mid * ld;
   CK(gemm_lane(lch, st, G(GEMM_NT, s2, s1, s1, 1.0, A21, ld, A, ld, 0.0, L21, ld, KLO_ZERO, KHI_NEND, OUT_FULL)));
+  cudaEvent_t e6 = ev_next(), e7 = ev_next();
+  CK(cudaEventRecord(e6, cur()));
   CK(gemm_lane(lch, st, G(GEMM_NT, s2, s2, s1, -1.0, L21, ld, L21, ld, 1.0, A22, ld, KLO_ZERO, KHI_K, OUT_LOWER)));
   c->launches += 2;
+  //   side: B2 -= L_B1 L21^T (needs only L_B1 and L21: beside the factorisation of A22), then S += L_B1 L_B1^T
+  CK(cudaStreamWaitEvent(xs, e6, 0));
+  CK(launch_gemm(G(GEMM_NT, b, s2, s1, -1.0, dst, b, L21, ld, 1.0, Bi + mid, b, KLO_ZERO, KHI_K, OUT_FULL), xs));
+  CK(cudaEventRecord(e7, xs));
+  if (Dnext)
+    CK(launch_gemm(G(GEMM_NT, b, b, s1, -1.0, dst, b, dst, b, 1.0, Dnext, b, KLO_ZERO, KHI_K, OUT_LOWER), xs));
+  CK(cudaEventRecord(e3, xs));
+  c->launches += Dnext ? 3 : 2;
   XM(11);
   CK(potrf_inv(c, lch, A, ld, mid, b, T1, T2, diagL, grow0, st));
   XM(12);
@@ -177,11 +184,10 @@ cudaError_t potrf_inv_coupled(bta_ctx* c, Chain* lch, double* A, int b, double* 
   CK(cudaEventRecord(e5, xs));
   c->launches += 2;
   //   main: L_B2 = (B2 - L_B1 L21^T) X22^T, S += L_B2 L_B2^T
-  CK(cudaStreamWaitEvent(SB, e2, 0));
-  CK(launch_gemm(G(GEMM_NT, b, s2, s1, -1.0, dst, b, L21, ld, 1.0, Bi + mid, b, KLO_ZERO, KHI_K, OUT_FULL), SB));
+  CK(cudaStreamWaitEvent(SB, e7, 0));
   CK(launch_gemm(G(GEMM_NT, b, s2, s2, 1.0, Bi + mid, b, A22, ld, 0.0, dst + mid, b, KLO_ZERO, KHI_NEND, OUT_FULL),
                  SB));
-  c->launches += 2;
+  c->launches += 1;
   XM(3);
   CK(cudaStreamWaitEvent(SB, e3, 0));
   if (Dnext) {
