@@ -663,7 +663,10 @@ int enqueue_gradient_twisted(bta_ctx* c, void* ws, cudaStream_t s0, bool timed, 
       // extra concurrency costs 3 %), so only up to the size where the whole gradient is graph-replayed
       if (c->opt.rows && md.b <= 1024) ch[m][q].rs = c->s_r[2 * m + q];
       // solve stream (the forward steps' side stream is idle in the backward sweep): same size rule
-      if (c->opt.rows && md.b <= AHEAD_MAXB && !carry) ch[m][q].ss = c->s_x[2 * m + q];
+      if (c->opt.rows && md.b <= AHEAD_MAXB && !carry) {
+        ch[m][q].ss = c->s_x[2 * m + q];
+        ch[m][q].gs = c->s_g[2 * m + q];
+      }
     }
 
   // ---- assemble: D (all blocks), arrow/rhs rows, tip on the up stream; coupling blocks per sub-chain

@@ -232,6 +232,7 @@ struct bta_ctx {
                                      // E, Z_T E ready [5..6] / consumed [7..8], G and X^T X ready [9..10], G consumed
                                      // [11..12], Z_D buffer read by the next step's Z_B product [13..14]
   cudaStream_t s_r[4];               // rows streams of the four chains (sweep.h: Chain::rs)
+  cudaStream_t s_g[4];               // G / X^T X streams of the four chains in the backward sweep (sweep.h: Chain::gs)
   cudaStream_t s_part[2][8], s_part_hi[2][8], s_part_x[2][8], s_part_r[2][8];  // partition.cu: per (matrix, partition)
   cudaEvent_t ev_sw[256];            // lane-switch events, used round-robin
   unsigned ev_sw_next;

@@ -138,6 +138,7 @@ int create_impl(bta_ctx* c, const bta_model_desc* desc, const bta_obs* obs) {
   for (auto& q : c->s_hi) BTA_CUDA_OK(cudaStreamCreateWithPriority(&q, cudaStreamNonBlocking, prio_hi));
   for (auto& q : c->s_x) BTA_CUDA_OK(cudaStreamCreateWithPriority(&q, cudaStreamNonBlocking, prio_lo));
   for (auto& q : c->s_r) BTA_CUDA_OK(cudaStreamCreateWithPriority(&q, cudaStreamNonBlocking, prio_hi));
+  for (auto& q : c->s_g) BTA_CUDA_OK(cudaStreamCreateWithPriority(&q, cudaStreamNonBlocking, prio_lo));
   for (auto& e : c->ev_sw) BTA_CUDA_OK(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
   for (auto& q : c->s_copy) BTA_CUDA_OK(cudaStreamCreateWithPriority(&q, cudaStreamNonBlocking, prio_lo));
   for (auto& q : c->ev_ring)
@@ -193,6 +194,7 @@ extern "C" int bta_destroy(bta_ctx* c) {
   for (auto& q : c->s_hi) kill_stream(q);
   for (auto& q : c->s_x) kill_stream(q);
   for (auto& q : c->s_r) kill_stream(q);
+  for (auto& q : c->s_g) kill_stream(q);
   for (auto& q : c->s_copy) kill_stream(q);
   for (int m = 0; m < 2; ++m)
     for (int p = 0; p < 8; ++p) {

@@ -44,6 +44,12 @@ cudaError_t chain_to_big(Chain& ch, cudaStream_t big) {
     cudaStreamWaitEvent(big, e, 0);
   }
   ch.solve_pending = false;
+  if (ch.g_pending && ch.gs && ch.gs != big) {
+    cudaEvent_t e = ch.c->ev_sw[(ch.c->ev_sw_next++) % BTA_NSW];
+    cudaEventRecord(e, ch.gs);
+    cudaStreamWaitEvent(big, e, 0);
+  }
+  ch.g_pending = false;
   return cudaGetLastError();
 }
 #define SS lane(lch, st, true)
@@ -518,13 +524,20 @@ cudaError_t chain_backward_step(Chain& ch, int t, cudaStream_t st) {
     // ---- upper solve (Eqs. 3-5):  u = z_t - L_Bt^T x_{t+1} - L_Ct^T x_T ;  x_t = X_t^T u  (row-vector form)
     const bool use_ss = ch.ss && ch.selinv && !ch.selinv_inplace && !ch.carry && !ch.fill;
     const bool side_solve = nr > 0 && use_ss && ch.part2;
-    const bool side_g = use_ss && has_next && ch.pipe_ev && ch.Gm2[t & 1];
+    const bool side_g = use_ss && ch.gs && has_next && ch.pipe_ev && ch.Gm2[t & 1];
     cudaEvent_t ev_solve = nullptr;   // the work of this step on the solve stream has read L_Bt
-    if ((side_solve || side_g) && !ch.solve_pending) {  // first step of this chain: its inputs come from the chain's stream
+    if ((side_solve && !ch.solve_pending) || (side_g && !ch.g_pending)) {
+      // first step of this chain: the inputs of the two streams come from the chain's stream
       cudaEvent_t e = c->ev_sw[(c->ev_sw_next++) % BTA_NSW];
       CK(cudaEventRecord(e, lane(lch, st, lch ? ch.on_small : false)));
-      CK(cudaStreamWaitEvent(ch.ss, e, 0));
-      ch.solve_pending = true;
+      if (side_solve && !ch.solve_pending) {
+        CK(cudaStreamWaitEvent(ch.ss, e, 0));
+        ch.solve_pending = true;
+      }
+      if (side_g && !ch.g_pending) {
+        CK(cudaStreamWaitEvent(ch.gs, e, 0));
+        ch.g_pending = true;
+      }
     }
     if (nr > 0) {
       double* part = side_solve ? ch.part2 : ch.part;
@@ -609,7 +622,7 @@ cudaError_t chain_backward_step(Chain& ch, int t, cudaStream_t st) {
     if (has_next) {
       double* Gm = side_g ? ch.Gm2[t & 1] : ch.W1;
       if (side_g) {
-        cudaStream_t gs = ch.ss;
+        cudaStream_t gs = ch.gs;
         if (ch.g_used[t & 1]) CK(cudaStreamWaitEvent(gs, ch.pipe_ev[11 + (t & 1)], 0));   // step t+2 is done with the slot
         CK(launch_gemm(G(GEMM_NN, b, b, b, 1.0, LB, b, X, b, 0.0, Gm, b, KLO_N0, KHI_K, OUT_FULL), gs));
         // X^T X straight into this step's Z_D buffer: step t+1's Z_B product (and the traces of step t+2) have read it
@@ -621,7 +634,7 @@ cudaError_t chain_backward_step(Chain& ch, int t, cudaStream_t st) {
         CK(launch_gemm(G(GEMM_NN, b, b, b, 1.0, LB, b, X, b, 0.0, Gm, b, KLO_N0, KHI_K, OUT_FULL), SB));
       }
       BTA_COUNT(c);
-      if (side_solve || side_g) {  // every reader of L_Bt on the solve stream has been issued
+      if (side_solve) {  // the solve's reader of L_Bt has been issued (G's is covered by its ready event below)
         ev_solve = c->ev_sw[(c->ev_sw_next++) % BTA_NSW];
         CK(cudaEventRecord(ev_solve, ch.ss));
       }

@@ -80,6 +80,8 @@ struct Chain {
   // Z_D buffer of that parity read.
   double* Gm2[2] = {nullptr, nullptr};
   bool g_used[2] = {false, false}, zd_read[2] = {false, false};
+  cudaStream_t gs = nullptr;   // the stream G and X^T X run on (the solve stream carries ten kernels per step already)
+  bool g_pending = false;      // work is outstanding on gs (chain_to_big joins it)
   bool tr_armed[2] = {false, false};
   // Host-staged carries (BTA_STORE_HOST): the diagonal-block slots are a ring of `ring` device blocks
   // (local block s lives in slot s % ring); each carry D_s - S_{s-1} is copied to pinned host memory (hostD + s b^2) on

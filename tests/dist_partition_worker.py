@@ -35,7 +35,10 @@ def main():
     gate = np.maximum(np.abs(ref["grad"]), 1e-3 * np.max(np.abs(ref["grad"])))
     ok = (abs(f - ref["f"]) <= 1e-9 * abs(ref["f"]) and bool(np.all(np.abs(g - ref["grad"]) <= 1e-6 * gate))
           and f2 == f and bool(np.array_equal(g, g2)))
-    print(json.dumps({"rank": dist.get_rank(), "f": f, "grad": g.tolist(), "ok": bool(ok), "backend": backend}), flush=True)
+    # one write call per rank, newline on both sides (the ranks share a pipe)
+    sys.stdout.write("\n" + json.dumps({"rank": dist.get_rank(), "f": f, "grad": g.tolist(), "ok": bool(ok),
+                                        "backend": backend}) + "\n")
+    sys.stdout.flush()
     dist.barrier()
     dist.destroy_process_group()
 

@@ -516,7 +516,14 @@ def test_partitioning_across_ranks_two_processes():
                           os.path.join(root, "tests", "dist_partition_worker.py")],
                          capture_output=True, text=True, cwd=root, timeout=600)
     assert out.returncode == 0, out.stdout[-2000:] + out.stderr[-2000:]
-    lines = [json.loads(l) for l in out.stdout.splitlines() if l.startswith("{")]
+    # the two ranks share one stdout: their lines can arrive glued together, so scan for objects, not for lines
+    lines, dec, pos = [], json.JSONDecoder(), 0
+    while True:
+        pos = out.stdout.find('{"rank"', pos)
+        if pos < 0:
+            break
+        obj, pos = dec.raw_decode(out.stdout, pos)
+        lines.append(obj)
     assert sorted(l["rank"] for l in lines) == [0, 1]
     assert lines[0]["f"] == lines[1]["f"] and lines[0]["grad"] == lines[1]["grad"]
     assert all(l["ok"] for l in lines), lines
